@@ -1,0 +1,127 @@
+/* ns.h -- C ABI of libns: batched pseudo-spectral Navier-Stokes right-hand side and SSP-RK3 step
+ * on the periodic torus [0,2pi)^3, hand-written CUDA for one NVIDIA B200 (sm_100a).
+ *
+ * Method: Rohner & Mishra, "Efficient Computation of Large-Scale Statistical Solutions to
+ * Incompressible Fluid Flows", PASC'24 (arXiv 2401.09843); cited as PAPER.md:Lnnn.
+ *   state              divergence-free velocity, spectral hyperviscosity discretisation
+ *                      eq. (2.1)-(2.4)
+ *   right-hand side    Algorithm 2 (pad 3/2, inverse FFT, u (x) u, forward FFT, dealias) and the
+ *                      Leray-projected time derivative eq. (2.5)
+ *   time step          third-order SSP Runge-Kutta eq. (2.6)
+ *   batch              Monte-Carlo samples of Algorithm 1 evolve independently;
+ *                      here they are the leading `batch` index of every array and launch
+ *   outputs            "writers" of PAPER.md:L157-167: full field, energy spectrum
+ * Readings of points the paper leaves open (Nyquist planes, form of Q_k, CFL formula, ...) are
+ * listed in DESIGN.md section 3 (A1..A18).
+ *
+ * Conventions
+ *   N         grid points per axis, a power of two, 8 <= N <= 1024.  Padded grid M = 3N/2.
+ *   spectral  complex interleaved (re,im) of `dtype`, shape [batch][3][N][N][N/2+1], index
+ *             [b][component][ikx][iky][ikz], ikz fastest (r2c half spectrum, kz >= 0).
+ *             Stored index i <-> wavenumber k = i (i < N/2) or i - N (i > N/2).  Coefficients are
+ *             NORMALISED: u(x) = sum_k u_hat(k) e^{i k.x}.  Entries with any index == N/2 (Nyquist
+ *             planes) are zero in the state and in every result (reading A3).
+ *   physical  reals of `dtype`, shape [batch][3][N][N][N], index [b][component][ix][iy][iz],
+ *             x_j = 2 pi j / N.
+ *   memspace  every caller buffer is tagged NS_HOST (pageable or pinned host memory) or NS_DEVICE
+ *             (device memory of the solver's GPU).  The caller owns every buffer it passes; the
+ *             library never frees or retains it past the call.  The library owns the handle and
+ *             all workspaces.
+ *   stream    all work is enqueued on the cudaStream_t given to ns_create (cast to void*; NULL =
+ *             the legacy default stream).  Calls that return data to NS_HOST memory, or return
+ *             host scalars, synchronise that stream before returning; all others are asynchronous.
+ *   errors    every int-returning call returns NS_OK (0) or a negative ns_status; the message is
+ *             available from ns_last_error(h) until the next call on h.  On error the state is
+ *             unchanged unless stated.  There is no CPU fallback: without a usable CUDA device
+ *             ns_create fails with NS_ERR_CUDA.
+ *   threads   no global state; handles are independent; one handle must not be used concurrently.
+ */
+#ifndef NS_H_
+#define NS_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ns_solver ns_solver; /* opaque */
+
+typedef enum { NS_F64 = 0, NS_F32 = 1 } ns_dtype;
+typedef enum { NS_HOST = 0, NS_DEVICE = 1 } ns_memspace;
+
+typedef enum {
+  NS_OK = 0,
+  NS_ERR_INVALID_ARG = -1, /* bad N / batch / dtype / NULL pointer / nbins < 1 / bad params */
+  NS_ERR_OOM = -2,         /* device allocation failed */
+  NS_ERR_CUDA = -3,        /* CUDA runtime error; text in ns_last_error */
+  NS_ERR_STATE = -4        /* ns_rhs / ns_step / getters called before an initial state was set */
+} ns_status;
+
+/* Dissipation operator of eq. (2.1)-(2.4), applied explicitly inside the RHS:
+ *   d_k = nu |k|^2 + eps_N |k|^(2s) Q_k,   eps_N = eps / N^(2s-1),
+ *   Q_k = 0 for |k| <= m_N, else (q_sharp ? 1 : 1 - (m_N/|k|)^q_exp),   |k| Euclidean. */
+typedef struct {
+  double nu;    /* Laplacian viscosity (0 disables)                                         */
+  double eps;   /* hyperviscosity constant, eps_N = eps / N^(2s-1) (0 disables)              */
+  double s;     /* hyperviscosity order s >= 1, may be fractional (paper uses 1 and 1.5)     */
+  double m_cut; /* cutoff m_N in wavenumber units; < 0 selects sqrt(N)  (theta = 1/2)        */
+  double q_exp; /* exponent (2s-1)/theta of eq. (2.3); < 0 selects (2s-1)/0.5                */
+  int q_sharp;  /* 0: smooth lower bound of eq. (2.3);  1: Q_k = 1 above the cutoff          */
+} ns_params;
+
+/* Create a solver for `batch` independent samples on an N^3 grid.  `p` may be NULL (inviscid).
+ * Allocates all device workspaces (about 40 * batch * N^3 * sizeof(complex) bytes).
+ * cuda_stream: a cudaStream_t cast to void* (NULL = default stream). */
+int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream);
+int ns_destroy(ns_solver* h);
+
+/* Set the state from PHYSICAL samples u_phys [batch][3][N][N][N] (eq. 2.1 third line,
+ * PAPER.md:L98, u(0) = P_N u_0): analysis transform with 1/N^3, Nyquist planes zeroed, Leray
+ * projector (eq. 2.5) applied for k != 0, mean mode kept.  Resets every sample's time to 0. */
+int ns_set_initial(ns_solver* h, const void* u_phys, ns_memspace ms);
+/* Set / get the state in SPECTRAL form, no projection (Nyquist planes are zeroed on set).
+ * Round trip get -> set is bit exact.  ns_set_spectral does not change the sample times. */
+int ns_set_spectral(ns_solver* h, const void* u_hat, ns_memspace ms);
+int ns_get_spectral(ns_solver* h, void* u_hat_out, ns_memspace ms);
+
+/* rhs_hat_out = R(state) = (1 - k k^T/|k|^2)(-i k^T F[u (x) u]_k) - d_k u_hat_k  (Algorithm 2 +
+ * eq. 2.5 + viscous term of eq. 2.1), spectral layout; R(0) = 0.  The state is unchanged. */
+int ns_rhs(ns_solver* h, void* rhs_hat_out, ns_memspace ms);
+
+/* One SSP-RK3 step (eq. 2.6) with the same dt for all samples; t_b += dt. */
+int ns_step(ns_solver* h, double dt);
+/* One SSP-RK3 step with a per-sample CFL step (reading A10; PAPER.md:L155 names the condition):
+ *   dt_b = min(cfl * (2 pi / N) / umax_b, t_end - t_b),  umax_b = max over the padded grid of |u|_2
+ * at the start of the step, evaluated on the device (no host round trip inside the step).
+ * Samples with t_b >= t_end are left untouched (bit exact).  dt_out: host array [batch] or NULL;
+ * when non-NULL the stream is synchronised and the steps actually taken are returned. */
+int ns_step_cfl(ns_solver* h, double cfl, double t_end, double* dt_out);
+/* One SSP-RK3 step with caller-given per-sample steps dt[batch] (host array); dt_b == 0 leaves
+ * sample b untouched.  Used to replay a recorded CFL sequence. */
+int ns_step_dts(ns_solver* h, const double* dt);
+
+/* umax_out[batch] (host): max over the padded M^3 grid of the Euclidean |u| of the current state. */
+int ns_max_velocity(ns_solver* h, double* umax_out);
+/* Physical velocity on the N grid, [batch][3][N][N][N] (the "whole flow field" writer). */
+int ns_get_fields(ns_solver* h, void* u_phys_out, ns_memspace ms);
+/* Shell energy spectrum (reading A14):
+ *   E_out[b][K] = 1/2 sum_{K-1/2 <= |k| < K+1/2} |u_hat_k|^2 over the full spectrum, K = 0..nbins-1,
+ * host array [batch][nbins] of double; sum_K E = 1/2 <|u|^2> when nbins covers all modes. */
+int ns_energy_spectrum(ns_solver* h, double* E_out, int nbins);
+/* Second-order longitudinal+transverse structure function on the N grid (reading A15):
+ *   S_out[b][l-1] = (1/3) sum_d < |u(x + l dx e_d) - u(x)|^2 >_x,  l = 1..nl (nl <= N/2), host [batch][nl]. */
+int ns_structure_function(ns_solver* h, double* S_out, int nl);
+
+/* Simulation time of one sample; NaN if `sample` is out of range. */
+double ns_time(const ns_solver* h, int sample);
+/* Number of kernels the library has launched on this handle so far (for bench.py's gpu_launches). */
+long long ns_kernel_launches(const ns_solver* h);
+/* Device bytes held by the handle. */
+long long ns_device_bytes(const ns_solver* h);
+/* Message of the last failed call on h ("" if none).  h == NULL returns the message of the last
+ * failed ns_create on this thread. */
+const char* ns_last_error(const ns_solver* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NS_H_ */

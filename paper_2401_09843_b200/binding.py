@@ -1,0 +1,223 @@
+"""Thin ctypes binding of libns.so (include/ns.h).  Argument marshalling only: every step of the
+path runs in the CUDA kernels behind the C ABI.  There is no fallback: if libns.so is missing or
+no CUDA device is usable, calls raise.
+
+Host buffers are numpy arrays, device buffers are torch CUDA tensors (PyTorch is used only for
+device memory and streams).  Complex arrays: numpy complex128/complex64, torch complex128/complex64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libns.so")
+
+NS_F64, NS_F32 = 0, 1
+NS_HOST, NS_DEVICE = 0, 1
+NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE = 0, -1, -2, -3, -4
+
+EXPORTS = [
+    "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
+    "ns_step_cfl", "ns_step_dts", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum",
+    "ns_structure_function", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
+]
+
+
+class ns_params(ctypes.Structure):
+    _fields_ = [("nu", ctypes.c_double), ("eps", ctypes.c_double), ("s", ctypes.c_double),
+                ("m_cut", ctypes.c_double), ("q_exp", ctypes.c_double), ("q_sharp", ctypes.c_int)]
+
+
+class NSError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libns error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libns.so (built by `python -m paper_2401_09843_b200.build`).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2401_09843_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i, d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        L.ns_create.argtypes = [ctypes.POINTER(vp), i, i, ctypes.POINTER(ns_params), i, vp]
+        L.ns_destroy.argtypes = [vp]
+        L.ns_set_initial.argtypes = [vp, vp, i]
+        L.ns_set_spectral.argtypes = [vp, vp, i]
+        L.ns_get_spectral.argtypes = [vp, vp, i]
+        L.ns_rhs.argtypes = [vp, vp, i]
+        L.ns_step.argtypes = [vp, d]
+        L.ns_step_cfl.argtypes = [vp, d, d, vp]
+        L.ns_step_dts.argtypes = [vp, vp]
+        L.ns_max_velocity.argtypes = [vp, vp]
+        L.ns_get_fields.argtypes = [vp, vp, i]
+        L.ns_energy_spectrum.argtypes = [vp, vp, i]
+        L.ns_structure_function.argtypes = [vp, vp, i]
+        L.ns_time.argtypes = [vp, i]
+        L.ns_time.restype = d
+        L.ns_kernel_launches.argtypes = [vp]
+        L.ns_kernel_launches.restype = ctypes.c_longlong
+        L.ns_device_bytes.argtypes = [vp]
+        L.ns_device_bytes.restype = ctypes.c_longlong
+        L.ns_last_error.argtypes = [vp]
+        L.ns_last_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _buf(x, writable=False):
+    """(pointer, memspace, keepalive) of a numpy array (host) or a torch CUDA tensor (device)."""
+    if _is_torch(x):
+        if not x.is_cuda:
+            raise ValueError("torch tensors must live on the GPU (use numpy arrays for host buffers)")
+        if not x.is_contiguous():
+            raise ValueError("device buffer must be contiguous")
+        return ctypes.c_void_p(x.data_ptr()), NS_DEVICE, x
+    a = x
+    if not isinstance(a, np.ndarray) or not a.flags["C_CONTIGUOUS"]:
+        if writable:
+            raise ValueError("output host buffer must be a C-contiguous numpy array")
+        a = np.ascontiguousarray(a)
+    return ctypes.c_void_p(a.ctypes.data), NS_HOST, a
+
+
+class Solver:
+    """Owner of one ns_solver handle.  Method names follow the C entry points without the ns_ prefix."""
+
+    def __init__(self, N, batch=1, nu=0.0, eps=0.0, s=1.0, m_cut=-1.0, q_exp=-1.0, q_sharp=0, dtype="f64", stream=None):
+        self.N, self.batch = int(N), int(batch)
+        self.dtype = {"f64": NS_F64, "f32": NS_F32, NS_F64: NS_F64, NS_F32: NS_F32}[dtype]
+        self.real = np.float64 if self.dtype == NS_F64 else np.float32
+        self.cplx = np.complex128 if self.dtype == NS_F64 else np.complex64
+        self._h = ctypes.c_void_p()
+        p = ns_params(nu, eps, s, m_cut, q_exp, q_sharp)
+        if stream is None:
+            import torch  # device memory and streams only
+            stream = torch.cuda.current_stream().cuda_stream
+        rc = lib().ns_create(ctypes.byref(self._h), self.N, self.batch, ctypes.byref(p), self.dtype, ctypes.c_void_p(stream))
+        if rc != NS_OK:
+            raise NSError(rc, lib().ns_last_error(None).decode())
+
+    # shapes ---------------------------------------------------------------------------------------
+    @property
+    def spectral_shape(self):
+        return (self.batch, 3, self.N, self.N, self.N // 2 + 1)
+
+    @property
+    def physical_shape(self):
+        return (self.batch, 3, self.N, self.N, self.N)
+
+    def _check(self, rc):
+        if rc != NS_OK:
+            raise NSError(rc, lib().ns_last_error(self._h).decode())
+
+    def _typed(self, x, kind):
+        """Cast host arrays to the solver dtype; device tensors must already match."""
+        want = self.real if kind == "real" else self.cplx
+        if _is_torch(x):
+            import torch
+            tw = {np.float64: torch.float64, np.float32: torch.float32, np.complex128: torch.complex128,
+                  np.complex64: torch.complex64}[want]
+            if x.dtype != tw:
+                raise ValueError(f"device tensor dtype {x.dtype} != {tw}")
+            return x
+        return np.ascontiguousarray(x, dtype=want)
+
+    # calls ----------------------------------------------------------------------------------------
+    def close(self):
+        if self._h:
+            lib().ns_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_initial(self, u_phys):
+        u = self._typed(u_phys, "real")
+        assert tuple(u.shape) == self.physical_shape, (tuple(u.shape), self.physical_shape)
+        p, ms, _k = _buf(u)
+        self._check(lib().ns_set_initial(self._h, p, ms))
+
+    def set_spectral(self, u_hat):
+        u = self._typed(u_hat, "cplx")
+        assert tuple(u.shape) == self.spectral_shape
+        p, ms, _k = _buf(u)
+        self._check(lib().ns_set_spectral(self._h, p, ms))
+
+    def get_spectral(self, out=None):
+        if out is None:
+            out = np.empty(self.spectral_shape, dtype=self.cplx)
+        p, ms, _k = _buf(out, writable=True)
+        self._check(lib().ns_get_spectral(self._h, p, ms))
+        return out
+
+    def rhs(self, out=None):
+        if out is None:
+            out = np.empty(self.spectral_shape, dtype=self.cplx)
+        p, ms, _k = _buf(out, writable=True)
+        self._check(lib().ns_rhs(self._h, p, ms))
+        return out
+
+    def step(self, dt):
+        self._check(lib().ns_step(self._h, float(dt)))
+
+    def step_cfl(self, cfl, t_end, return_dt=True):
+        if return_dt:
+            dts = np.empty(self.batch, dtype=np.float64)
+            self._check(lib().ns_step_cfl(self._h, float(cfl), float(t_end), ctypes.c_void_p(dts.ctypes.data)))
+            return dts
+        self._check(lib().ns_step_cfl(self._h, float(cfl), float(t_end), None))
+        return None
+
+    def step_dts(self, dts):
+        d = np.ascontiguousarray(dts, dtype=np.float64)
+        assert d.shape == (self.batch,)
+        self._check(lib().ns_step_dts(self._h, ctypes.c_void_p(d.ctypes.data)))
+
+    def max_velocity(self):
+        out = np.empty(self.batch, dtype=np.float64)
+        self._check(lib().ns_max_velocity(self._h, ctypes.c_void_p(out.ctypes.data)))
+        return out
+
+    def get_fields(self, out=None):
+        if out is None:
+            out = np.empty(self.physical_shape, dtype=self.real)
+        p, ms, _k = _buf(out, writable=True)
+        self._check(lib().ns_get_fields(self._h, p, ms))
+        return out
+
+    def energy_spectrum(self, nbins):
+        E = np.empty((self.batch, int(nbins)), dtype=np.float64)
+        self._check(lib().ns_energy_spectrum(self._h, ctypes.c_void_p(E.ctypes.data), int(nbins)))
+        return E
+
+    def structure_function(self, nl=None):
+        nl = self.N // 2 if nl is None else int(nl)
+        S = np.empty((self.batch, nl), dtype=np.float64)
+        self._check(lib().ns_structure_function(self._h, ctypes.c_void_p(S.ctypes.data), nl))
+        return S
+
+    def time(self, sample=0):
+        return float(lib().ns_time(self._h, int(sample)))
+
+    def kernel_launches(self):
+        return int(lib().ns_kernel_launches(self._h))
+
+    def device_bytes(self):
+        return int(lib().ns_device_bytes(self._h))

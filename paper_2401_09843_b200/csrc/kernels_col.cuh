@@ -1,0 +1,193 @@
+// kernels_col.cuh -- strided-axis ("column") passes of the padded 3-D transform (steps a1, a2, a5, a6
+// of SURVEY.md section 8(a); Algorithm 3 steps 1-2 of the paper, and its reverse).
+//
+// The 3/2 zero-padding (Algorithm 2 step 1) and the truncation (step 5)
+// are fused into the transform as a PRUNED radix-3 stage, so padded zeros are never read or written:
+// with M = 3L, L = N/2, the padded line has non-zeros only at k = n (stored row n) and k = n - L
+// (stored row n + L), n in [0, L); row L (the Nyquist entry) is zero by convention (A3).
+//
+//   inverse:  x[3r+q] = sum_n s_q[n] w_L^{+rn},   s_q[n] = (a_n + c_n w3^{-q}) W^{+qn}
+//   forward:  F_q[n]  = sum_r x[3r+q] w_L^{-rn},  A_n = sum_q W^{-qn} F_q[n],  C_n = sum_q W^{-qn} w3^{+q} F_q[n]
+//   with a_n / A_n = row n, c_n / C_n = row n + L, W = e^{2 pi i/(3L)}, w3 = e^{2 pi i/3}.
+//
+// The physical axis is kept in the decimated order p = q*L + r (physical index j = 3r + q): everything
+// done in physical space is pointwise, and the forward pass consumes the same order.
+//
+// Tile = TC adjacent columns (TC * sizeof(complex) = 128 B, one full cache line per row) x the whole
+// line.  Each length-L transform is two register stages R1 x R2 with one shared-memory exchange;
+// the three sub-transforms q = 0,1,2 are done one after the other by the same threads so the input
+// rows a_n, c_n are read from HBM exactly once and stay in registers.
+#pragma once
+#include "cx.cuh"
+
+namespace ns {
+
+struct ColArgs {
+    long istride, ostride;    // row strides of input / output, in complex elements
+    long in_slab, out_slab;   // slab strides, in complex elements
+    int tiles_per_slab;       // column tiles per slab (columns / TC)
+    long total_tiles;         // slabs * tiles_per_slab
+};
+
+template <int R1, int R2> struct ColP { static constexpr int value = R1 > R2 ? R1 : R2; };
+
+// ------------------------------------------------------------------------------------------------
+// inverse (spectral rows [0,2L) -> physical rows [0,3L)), exp(+i...)
+// ------------------------------------------------------------------------------------------------
+template <typename T, int L, int R1, int R2, int TC, int TPB>
+__global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
+col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
+               const cx<T>* __restrict__ tw3, const cx<T>* __restrict__ twL) {
+    static_assert(R1 * R2 == L && R2 >= 2, "two register stages");
+    constexpr int P = ColP<R1, R2>::value;
+    constexpr int TT = TC * P;  // threads per tile
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* E = reinterpret_cast<cx<T>*>(smem_raw);  // [2][TPB][L][TC]
+
+    const int tl = threadIdx.x / TT;
+    const int lt = threadIdx.x % TT;
+    const int c = lt % TC, i = lt / TC;
+    long tile = (long)blockIdx.x * TPB + tl;
+    if (tile >= g.total_tiles) tile = g.total_tiles - 1;  // duplicate work, identical writes
+    const long slab = tile / g.tiles_per_slab;
+    const int col0 = (int)(tile % g.tiles_per_slab) * TC;
+    const cx<T>* ip = in + slab * g.in_slab + col0 + c;
+    cx<T>* op = out + slab * g.out_slab + col0 + c;
+    cx<T>* Et = E + (size_t)tl * L * TC;
+    constexpr size_t EBUF = (size_t)TPB * L * TC;
+
+    cx<T> a[R1], cc[R1];
+    if (i < R2) {
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) {
+            const int n = R2 * n1 + i;
+            a[n1] = ldg(ip + (long)n * g.istride);
+        }
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) {
+            const int n = R2 * n1 + i;
+            cc[n1] = (n == 0) ? mk<T>(0, 0) : ldg(ip + (long)(L + n) * g.istride);
+        }
+    }
+    int buf = 0;
+#pragma unroll 1
+    for (int q = 0; q < 3; ++q) {
+        if (i < R2) {
+            cx<T> s[R1];
+            if (q == 0) {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) {
+                    s[n1] = a[n1] + cc[n1];
+                    // prepare t1 = a - c/2, t2 = (sqrt3/2) c for q = 1, 2
+                    a[n1] = mk<T>(a[n1].x - (T)0.5 * cc[n1].x, a[n1].y - (T)0.5 * cc[n1].y);
+                    cc[n1] = (T)0.86602540378443864676L * cc[n1];
+                }
+            } else {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) {
+                    const int n = R2 * n1 + i;
+                    // a + c w3^{-q}:  q=1: t1 - i t2,  q=2: t1 + i t2
+                    const cx<T> z = (q == 1) ? mk<T>(a[n1].x + cc[n1].y, a[n1].y - cc[n1].x)
+                                             : mk<T>(a[n1].x - cc[n1].y, a[n1].y + cc[n1].x);
+                    s[n1] = cmul(z, ldg(tw3 + q * n));
+                }
+            }
+            fft_reg<R1, +1, T>(s);
+#pragma unroll
+            for (int r1 = 0; r1 < R1; ++r1) {
+                cx<T> v = s[brev<R1>(r1)];
+                if (r1 > 0) v = cmul(v, ldg(twL + r1 * i));
+                Et[buf * EBUF + (size_t)(r1 * R2 + i) * TC + c] = v;
+            }
+        }
+        __syncthreads();
+        if (i < R1) {
+            cx<T> y[R2];
+#pragma unroll
+            for (int n2 = 0; n2 < R2; ++n2) y[n2] = Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c];
+            fft_reg<R2, +1, T>(y);
+#pragma unroll
+            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[brev<R2>(r2)];
+        }
+        buf ^= 1;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// forward (physical rows [0,3L) -> spectral rows [0,2L), truncated), exp(-i...), output * scale
+// ------------------------------------------------------------------------------------------------
+template <typename T, int L, int R1, int R2, int TC, int TPB>
+__global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
+col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale,
+               const cx<T>* __restrict__ tw3, const cx<T>* __restrict__ twL) {
+    static_assert(R1 * R2 == L && R2 >= 2, "two register stages");
+    constexpr int P = ColP<R1, R2>::value;
+    constexpr int TT = TC * P;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* E = reinterpret_cast<cx<T>*>(smem_raw);  // [2][TPB][L][TC] exchange + [TPB][L][TC] spill of G1
+
+    const int tl = threadIdx.x / TT;
+    const int lt = threadIdx.x % TT;
+    const int c = lt % TC, i = lt / TC;
+    long tile = (long)blockIdx.x * TPB + tl;
+    if (tile >= g.total_tiles) tile = g.total_tiles - 1;
+    const long slab = tile / g.tiles_per_slab;
+    const int col0 = (int)(tile % g.tiles_per_slab) * TC;
+    const cx<T>* ip = in + slab * g.in_slab + col0 + c;
+    cx<T>* op = out + slab * g.out_slab + col0 + c;
+    cx<T>* Et = E + (size_t)tl * L * TC;
+    constexpr size_t EBUF = (size_t)TPB * L * TC;
+    cx<T>* G1 = E + 2 * EBUF + (size_t)tl * L * TC;
+
+    cx<T> F0[R1];
+    int buf = 0;
+#pragma unroll 1
+    for (int q = 0; q < 3; ++q) {
+        if (i < R1) {
+            cx<T> x[R2];
+#pragma unroll
+            for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(q * L + i + R1 * r2) * g.istride);
+            fft_reg<R2, -1, T>(x);
+#pragma unroll
+            for (int n2 = 0; n2 < R2; ++n2) {
+                cx<T> v = x[brev<R2>(n2)];
+                if (n2 > 0) v = cmulc(v, ldg(twL + i * n2));
+                Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c] = v;
+            }
+        }
+        __syncthreads();
+        if (i < R2) {
+            cx<T> y[R1];
+#pragma unroll
+            for (int r1 = 0; r1 < R1; ++r1) y[r1] = Et[buf * EBUF + (size_t)(r1 * R2 + i) * TC + c];
+            fft_reg<R1, -1, T>(y);
+            if (q == 0) {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) F0[n1] = y[brev<R1>(n1)];
+            } else if (q == 1) {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) {
+                    const int n = R2 * n1 + i;
+                    G1[(size_t)n * TC + c] = cmulc(y[brev<R1>(n1)], ldg(tw3 + n));
+                }
+            } else {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) {
+                    const int n = R2 * n1 + i;
+                    const cx<T> g2 = cmulc(y[brev<R1>(n1)], ldg(tw3 + 2 * n));
+                    const cx<T> g1 = G1[(size_t)n * TC + c];
+                    const cx<T> S = g1 + g2, D = g1 - g2;
+                    constexpr T h3 = (T)0.86602540378443864676L;
+                    const cx<T> A = F0[n1] + S;
+                    // C = F0 - S/2 + i (sqrt3/2) D
+                    const cx<T> C = mk<T>(F0[n1].x - (T)0.5 * S.x - h3 * D.y, F0[n1].y - (T)0.5 * S.y + h3 * D.x);
+                    op[(long)n * g.ostride] = scale * A;
+                    op[(long)(L + n) * g.ostride] = (n == 0) ? mk<T>(0, 0) : scale * C;
+                }
+            }
+        }
+        buf ^= 1;
+    }
+}
+
+}  // namespace ns

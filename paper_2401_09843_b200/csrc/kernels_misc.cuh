@@ -1,0 +1,365 @@
+// kernels_misc.cuh -- pointwise and reduction kernels of the product path:
+//   spectral_kernel   step a7: divergence, Leray projection (eq. 2.5), dissipation
+//                     (eq. 2.1-2.4) and one line of SSP-RK3 (eq. 2.6)
+//   cfl_finalize      step a8: dt_b from max|u| (reading A10)
+//   layout converters, energy spectrum, structure-function marginals
+//   generic power-of-two FFT on the unpadded N grid, used only by ns_set_initial / ns_get_fields.
+// Internal spectral layout: [batch][comp][N][N][H], H = N/2 (the identically-zero kz = N/2 column of the
+// public layout is not stored, so rows are 128-byte aligned).
+#pragma once
+#include "cx.cuh"
+
+namespace ns {
+
+__device__ __forceinline__ int wavenum(int i, int N) { return i < N / 2 ? i : i - N; }
+
+// ------------------------------------------------------------------------------------------------
+// a7.  Bh: [b][6][N][N][H] unnormalised transforms of u_i u_j (order 11 12 13 22 23 33).
+//   b_i = -i k_j Bh_ij * scale;  Nl = b - k (k.b)/|k|^2;  R = Nl - d(|k|^2) * Us
+//   mode 0: out = R
+//   mode 1: out = alpha*Un + beta*Us + gamma*dt_b*R   (Un may be NULL when alpha == 0)
+//           dt_b == 0 marks an inactive sample: out = Un (or Us when Un is NULL), bit exact.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* __restrict__ Us, const cx<T>* __restrict__ Un,
+                cx<T>* __restrict__ out, int N, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
+                T gamma, const double* __restrict__ dt, int mode) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int H = N / 2;
+    const int iz = (int)(idx % H);
+    const int iy = (int)((idx / H) % N);
+    const int ix = (int)((idx / ((long)H * N)) % N);
+    const long b = idx / ((long)H * N * N);
+    const long plane = (long)N * N * H;
+    const long o = ((long)ix * N + iy) * H + iz;
+    const cx<T>* us = Us + b * 3 * plane + o;
+    cx<T>* op = out + b * 3 * plane + o;
+    const int kxi = wavenum(ix, N), kyi = wavenum(iy, N);
+    const int k2i = kxi * kxi + kyi * kyi + iz * iz;
+    const bool dead = (ix == N / 2) || (iy == N / 2) || (k2i == 0);
+
+    cx<T> R[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
+    cx<T> u[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) u[c] = us[c * plane];
+    if (!dead) {
+        const cx<T>* bp = Bh + b * 6 * plane + o;
+        const cx<T> B11 = ldg(bp), B12 = ldg(bp + plane), B13 = ldg(bp + 2 * plane), B22 = ldg(bp + 3 * plane),
+                    B23 = ldg(bp + 4 * plane), B33 = ldg(bp + 5 * plane);
+        const T kx = (T)kxi, ky = (T)kyi, kz = (T)iz;
+        // -i z = (z.y, -z.x)
+        cx<T> bb[3];
+        {
+            const cx<T> z0 = mk<T>(kx * B11.x + ky * B12.x + kz * B13.x, kx * B11.y + ky * B12.y + kz * B13.y);
+            const cx<T> z1 = mk<T>(kx * B12.x + ky * B22.x + kz * B23.x, kx * B12.y + ky * B22.y + kz * B23.y);
+            const cx<T> z2 = mk<T>(kx * B13.x + ky * B23.x + kz * B33.x, kx * B13.y + ky * B23.y + kz * B33.y);
+            bb[0] = mk<T>(scale * z0.y, -scale * z0.x);
+            bb[1] = mk<T>(scale * z1.y, -scale * z1.x);
+            bb[2] = mk<T>(scale * z2.y, -scale * z2.x);
+        }
+        const T ik2 = (T)1 / (T)k2i;
+        const cx<T> kb = mk<T>((kx * bb[0].x + ky * bb[1].x + kz * bb[2].x) * ik2,
+                               (kx * bb[0].y + ky * bb[1].y + kz * bb[2].y) * ik2);
+        const T d = dtab[k2i];
+        R[0] = mk<T>(bb[0].x - kx * kb.x - d * u[0].x, bb[0].y - kx * kb.y - d * u[0].y);
+        R[1] = mk<T>(bb[1].x - ky * kb.x - d * u[1].x, bb[1].y - ky * kb.y - d * u[1].y);
+        R[2] = mk<T>(bb[2].x - kz * kb.x - d * u[2].x, bb[2].y - kz * kb.y - d * u[2].y);
+    }
+    if (mode == 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) op[c * plane] = R[c];
+        return;
+    }
+    const T dtb = (T)dt[b];
+    const cx<T>* un = Un ? Un + b * 3 * plane + o : nullptr;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        cx<T> r;
+        if (un) {
+            const cx<T> n = un[c * plane];
+            if (dtb == (T)0) r = n;
+            else r = mk<T>(alpha * n.x + beta * u[c].x + gamma * dtb * R[c].x, alpha * n.y + beta * u[c].y + gamma * dtb * R[c].y);
+        } else {
+            if (dtb == (T)0) r = u[c];
+            else r = mk<T>(beta * u[c].x + gamma * dtb * R[c].x, beta * u[c].y + gamma * dtb * R[c].y);
+        }
+        op[c * plane] = r;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// time-step bookkeeping (device resident: no host sync inside a step)
+// ------------------------------------------------------------------------------------------------
+__global__ void set_dt_uniform_kernel(double* dt, double* t, double value, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) { dt[b] = value; t[b] += value; }
+}
+__global__ void set_dt_array_kernel(double* dt, double* t, const double* src, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) { dt[b] = src[b]; t[b] += src[b]; }
+}
+// dt_b = min(cfl * dx / umax_b, t_end - t_b); 0 for finished samples.  umax2 holds the bits of max |u|^2.
+__global__ void cfl_finalize_kernel(double* dt, double* t, const unsigned long long* umax2, double cfl, double dx,
+                                    double t_end, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const double remaining = t_end - t[b];
+    double v = 0.0;
+    if (remaining > 0.0) {
+        const double um = sqrt(__longlong_as_double((long long)umax2[b]));
+        v = um > 0.0 ? cfl * dx / um : remaining;
+        if (!(v < remaining)) v = remaining;
+        if (!isfinite(v)) v = 0.0;
+    }
+    dt[b] = v;
+    t[b] += v;
+}
+__global__ void umax_read_kernel(double* out, const unsigned long long* umax2, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) out[b] = sqrt(__longlong_as_double((long long)umax2[b]));
+}
+
+// ------------------------------------------------------------------------------------------------
+// layout converters: public [.][N][N][N/2+1]  <->  internal [.][N][N][N/2]
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void to_internal_kernel(const cx<T>* __restrict__ pub, cx<T>* __restrict__ in, int N, long total) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int H = N / 2;
+    const int iz = (int)(idx % H);
+    const long row = idx / H;  // (cube, ix, iy)
+    const int iy = (int)(row % N), ix = (int)((row / N) % N);
+    cx<T> v = pub[row * (H + 1) + iz];
+    if (ix == N / 2 || iy == N / 2) v = mk<T>(0, 0);
+    in[idx] = v;
+}
+template <typename T>
+__global__ void to_public_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ pub, int N, long total_pub) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total_pub) return;
+    const int H = N / 2;
+    const int iz = (int)(idx % (H + 1));
+    const long row = idx / (H + 1);
+    pub[idx] = iz == H ? mk<T>(0, 0) : in[row * H + iz];
+}
+
+// ------------------------------------------------------------------------------------------------
+// energy spectrum: E[b][K] += w/2 |u_hat|^2, K = floor(|k| + 1/2)
+// grid = (chunks, batch); dynamic smem nbins doubles
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void energy_spectrum_kernel(const cx<T>* __restrict__ U, double* __restrict__ E, int N, int nbins) {
+    extern __shared__ double bins[];
+    for (int i = threadIdx.x; i < nbins; i += blockDim.x) bins[i] = 0.0;
+    __syncthreads();
+    const int H = N / 2;
+    const long plane = (long)N * N * H;
+    const long b = blockIdx.y;
+    const cx<T>* u = U + b * 3 * plane;
+    for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < plane; idx += (long)gridDim.x * blockDim.x) {
+        const int iz = (int)(idx % H), iy = (int)((idx / H) % N), ix = (int)(idx / ((long)H * N));
+        if (ix == N / 2 || iy == N / 2) continue;
+        const double kx = wavenum(ix, N), ky = wavenum(iy, N), kz = iz;
+        const int bin = (int)floor(sqrt(kx * kx + ky * ky + kz * kz) + 0.5);
+        if (bin >= nbins) continue;
+        double e = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const cx<T> v = u[c * plane + idx];
+            e += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+        }
+        atomicAdd(&bins[bin], (iz == 0 ? 0.5 : 1.0) * e);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nbins; i += blockDim.x)
+        if (bins[i] != 0.0) atomicAdd(&E[b * nbins + i], bins[i]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// structure function through its exact spectral form:
+//   S2(l) = (1/3) sum_d sum_k 2 (1 - cos(k_d l dx)) w_k |u_hat_k|^2
+// marginals: e[b][d][i] = sum over the other two indices of w |u_hat|^2, i = stored index along d
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void sf_marginals_kernel(const cx<T>* __restrict__ U, double* __restrict__ marg, int N) {
+    extern __shared__ double bins[];  // [3][N]
+    for (int i = threadIdx.x; i < 3 * N; i += blockDim.x) bins[i] = 0.0;
+    __syncthreads();
+    const int H = N / 2;
+    const long plane = (long)N * N * H;
+    const long b = blockIdx.y;
+    const cx<T>* u = U + b * 3 * plane;
+    for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < plane; idx += (long)gridDim.x * blockDim.x) {
+        const int iz = (int)(idx % H), iy = (int)((idx / H) % N), ix = (int)(idx / ((long)H * N));
+        if (ix == N / 2 || iy == N / 2) continue;
+        double e = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const cx<T> v = u[c * plane + idx];
+            e += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+        }
+        e *= (iz == 0 ? 1.0 : 2.0);
+        atomicAdd(&bins[ix], e);
+        atomicAdd(&bins[N + iy], e);
+        atomicAdd(&bins[2 * N + iz], e);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 3 * N; i += blockDim.x)
+        if (bins[i] != 0.0) atomicAdd(&marg[b * 3 * N + i], bins[i]);
+}
+// one block per sample, thread per l
+__global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __restrict__ S, int N, int nl) {
+    const int b = blockIdx.x;
+    for (int l = 1 + threadIdx.x; l <= nl; l += blockDim.x) {
+        double acc = 0.0;
+        for (int d = 0; d < 3; ++d)
+            for (int i = 0; i < N; ++i) {
+                const double e = marg[(b * 3 + d) * N + i];
+                if (e == 0.0) continue;
+                const int k = (d == 2) ? i : wavenum(i, N);
+                // cos(2 pi k l / N) with exact argument reduction
+                const long kl = ((long)k * l) % N;
+                acc += 2.0 * (1.0 - cospi(2.0 * (double)kl / (double)N)) * e;
+            }
+        S[b * nl + (l - 1)] = acc / 3.0;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// unpadded N-grid transforms for ns_set_initial / ns_get_fields (NOT on the hot path): a plain
+// shared-memory radix-2 FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place.
+//   axis 0: element stride n*n, axis 1: n, axis 2: 1.
+// ------------------------------------------------------------------------------------------------
+template <typename T> __device__ __forceinline__ cx<T> unit_root_pi(T frac);  // exp(i*pi*frac)
+template <> __device__ __forceinline__ cx<double> unit_root_pi<double>(double f) {
+    double s, c;
+    sincospi(f, &s, &c);
+    return mk<double>(c, s);
+}
+template <> __device__ __forceinline__ cx<float> unit_root_pi<float>(float f) {
+    float s, c;
+    sincospif(f, &s, &c);
+    return mk<float>(c, s);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2n, int axis, int sign, long total_tiles) {
+    constexpr int TL = 8;  // lines per tile
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);  // [n][TL+1]
+    constexpr int PITCH = TL + 1;
+    const long tile = blockIdx.x;
+    if (tile >= total_tiles) return;
+    const long n2 = (long)n * n;
+    const long tiles_per_cube = n2 / TL;
+    const long cube = tile / tiles_per_cube;
+    const long l0 = (tile % tiles_per_cube) * TL;  // first line id within the cube
+    cx<T>* base = A + cube * n2 * n;
+    const long es = axis == 0 ? n2 : (axis == 1 ? n : 1);
+    // line id l -> offset of element 0
+    auto line_base = [&](long l) -> long {
+        if (axis == 0) return l;
+        if (axis == 1) return (l / n) * n2 + (l % n);
+        return l * n;
+    };
+    // load with bit-reversed row index
+    for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
+        int j, c;
+        if (axis == 2) { j = e % n; c = e / n; } else { c = e % TL; j = e / TL; }
+        const int jr = (int)(__brev((unsigned)j) >> (32 - log2n));
+        S[jr * PITCH + c] = base[line_base(l0 + c) + (long)j * es];
+    }
+    __syncthreads();
+    for (int s = 1; s <= log2n; ++s) {
+        const int half = 1 << (s - 1);
+        for (int e = threadIdx.x; e < (n / 2) * TL; e += blockDim.x) {
+            const int c = e % TL, bf = e / TL;
+            const int j = bf & (half - 1);
+            const int i0 = ((bf >> (s - 1)) << s) + j;
+            const cx<T> w = unit_root_pi<T>((T)sign * (T)j / (T)half);
+            const cx<T> a = S[i0 * PITCH + c];
+            const cx<T> bq = cmul(S[(i0 + half) * PITCH + c], w);
+            S[i0 * PITCH + c] = a + bq;
+            S[(i0 + half) * PITCH + c] = a - bq;
+        }
+        __syncthreads();
+    }
+    for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
+        int j, c;
+        if (axis == 2) { j = e % n; c = e / n; } else { c = e % TL; j = e / TL; }
+        base[line_base(l0 + c) + (long)j * es] = S[j * PITCH + c];
+    }
+}
+
+template <typename T>
+__global__ void real_to_complex_kernel(const T* __restrict__ in, cx<T>* __restrict__ out, long total) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < total) out[idx] = mk<T>(in[idx], 0);
+}
+template <typename T>
+__global__ void complex_to_real_kernel(const cx<T>* __restrict__ in, T* __restrict__ out, long total) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < total) out[idx] = in[idx].x;
+}
+
+// W: [batch][3][N][N][N] full complex unnormalised spectra -> U internal, scaled 1/N^3, Nyquist zeroed,
+// Leray-projected for k != 0 (eq. 2.5 projector; reading A11).
+template <typename T>
+__global__ void init_project_kernel(const cx<T>* __restrict__ W, cx<T>* __restrict__ U, int N, long total, T scale) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int H = N / 2;
+    const int iz = (int)(idx % H);
+    const int iy = (int)((idx / H) % N);
+    const int ix = (int)((idx / ((long)H * N)) % N);
+    const long b = idx / ((long)H * N * N);
+    const long plane = (long)N * N * H, cube = (long)N * N * N;
+    const long o = ((long)ix * N + iy) * H + iz;
+    cx<T> u[3];
+    const bool nyq = ix == N / 2 || iy == N / 2;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const cx<T> w = W[(b * 3 + c) * cube + ((long)ix * N + iy) * N + iz];
+        u[c] = nyq ? mk<T>(0, 0) : scale * w;
+    }
+    const int kxi = wavenum(ix, N), kyi = wavenum(iy, N);
+    const int k2i = kxi * kxi + kyi * kyi + iz * iz;
+    if (!nyq && k2i > 0) {
+        const T kx = (T)kxi, ky = (T)kyi, kz = (T)iz, ik2 = (T)1 / (T)k2i;
+        const cx<T> ku = mk<T>((kx * u[0].x + ky * u[1].x + kz * u[2].x) * ik2, (kx * u[0].y + ky * u[1].y + kz * u[2].y) * ik2);
+        u[0] = mk<T>(u[0].x - kx * ku.x, u[0].y - kx * ku.y);
+        u[1] = mk<T>(u[1].x - ky * ku.x, u[1].y - ky * ku.y);
+        u[2] = mk<T>(u[2].x - kz * ku.x, u[2].y - kz * ku.y);
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) U[(b * 3 + c) * plane + o] = u[c];
+}
+
+// U internal -> W full complex Hermitian spectrum on the N grid (kz < 0 from conj of (-k)).
+template <typename T>
+__global__ void expand_hermitian_kernel(const cx<T>* __restrict__ U, cx<T>* __restrict__ W, int N, long total) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int H = N / 2;
+    const int iz = (int)(idx % N);
+    const int iy = (int)((idx / N) % N);
+    const int ix = (int)((idx / ((long)N * N)) % N);
+    const long cubei = idx / ((long)N * N * N);
+    const long plane = (long)N * N * H;
+    cx<T> v = mk<T>(0, 0);
+    if (ix != N / 2 && iy != N / 2 && iz != N / 2) {
+        if (iz < H) {
+            v = U[cubei * plane + ((long)ix * N + iy) * H + iz];
+        } else {
+            const int jx = (N - ix) % N, jy = (N - iy) % N, jz = N - iz;
+            v = conj(U[cubei * plane + ((long)jx * N + jy) * H + jz]);
+        }
+    }
+    W[idx] = v;
+}
+
+}  // namespace ns

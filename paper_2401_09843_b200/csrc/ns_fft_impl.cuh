@@ -1,0 +1,156 @@
+// ns_fft_impl.cuh -- launch configuration of the FFT kernels, instantiated once per dtype.
+#pragma once
+#include "kernels_col.cuh"
+#include "kernels_z.cuh"
+#include "ns_internal.h"
+
+namespace ns {
+
+// Register-stage split L = R1 x R2 per supported half-length.
+template <int L> struct Split;
+template <> struct Split<8>   { static constexpr int R1 = 4,  R2 = 2;  };
+template <> struct Split<16>  { static constexpr int R1 = 4,  R2 = 4;  };
+template <> struct Split<32>  { static constexpr int R1 = 8,  R2 = 4;  };
+template <> struct Split<64>  { static constexpr int R1 = 8,  R2 = 8;  };
+template <> struct Split<128> { static constexpr int R1 = 16, R2 = 8;  };
+template <> struct Split<256> { static constexpr int R1 = 16, R2 = 16; };
+
+template <int L> struct Cfg {
+    static constexpr int R1 = Split<L>::R1, R2 = Split<L>::R2;
+    static constexpr int P = R1 > R2 ? R1 : R2;
+    // tiles per block for the column kernels: aim at 128 threads
+    template <typename T> static constexpr int tpb() {
+        constexpr int tt = tile_cols<T>() * P;
+        return tt >= 128 ? 1 : 128 / tt;
+    }
+    // lines per block for the z kernels: aim at 192 threads
+    static constexpr int lpb() { return (3 * P) >= 192 ? 1 : 192 / (3 * P); }
+};
+
+template <typename K>
+static cudaError_t set_smem(K kernel, size_t bytes) {
+    if (bytes > 48 * 1024) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    return cudaSuccess;
+}
+
+template <typename T, int L>
+static cudaError_t col_inv_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, Twiddles<T> tw) {
+    using C = Cfg<L>;
+    constexpr int TC = tile_cols<T>(), TPB = C::template tpb<T>();
+    auto k = col_inv_kernel<T, L, C::R1, C::R2, TC, TPB>;
+    const size_t smem = (size_t)2 * TPB * L * TC * sizeof(cx<T>);
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    const long blocks = (g.total_tiles + TPB - 1) / TPB;
+    k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, tw.tw3, tw.twL);
+    return cudaGetLastError();
+}
+
+template <typename T, int L>
+static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
+    using C = Cfg<L>;
+    constexpr int TC = tile_cols<T>(), TPB = C::template tpb<T>();
+    auto k = col_fwd_kernel<T, L, C::R1, C::R2, TC, TPB>;
+    const size_t smem = (size_t)3 * TPB * L * TC * sizeof(cx<T>);
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    const long blocks = (g.total_tiles + TPB - 1) / TPB;
+    k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, scale, tw.tw3, tw.twL);
+    return cudaGetLastError();
+}
+
+template <typename T, int L>
+static cudaError_t z_inv_L(cudaStream_t st, const cx<T>* in, T* phys, long MM, long batch, unsigned long long* umax2,
+                           Twiddles<T> tw) {
+    using C = Cfg<L>;
+    constexpr int LPB = C::lpb();
+    auto k = z_inv_prod_kernel<T, L, C::R1, C::R2, LPB>;
+    const size_t smem = (size_t)2 * LPB * 3 * C::R1 * (C::R2 + 1) * sizeof(cx<T>);
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    const long total = MM * batch;
+    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(in, phys, MM, total, umax2, tw.tw3, tw.twL);
+    return cudaGetLastError();
+}
+
+template <typename T, int L>
+static cudaError_t z_fwd_L(cudaStream_t st, const T* phys, cx<T>* out, long MM, long batch, Twiddles<T> tw) {
+    using C = Cfg<L>;
+    constexpr int LPB = C::lpb();
+    auto k = z_fwd_kernel<T, L, C::R1, C::R2, LPB>;
+    const size_t smem = (size_t)LPB * (3 * C::R1 * (C::R2 + 1) + 3 * L) * sizeof(cx<T>);
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    const long total = MM * batch;
+    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(phys, out, MM, total, tw.tw3, tw.twL);
+    return cudaGetLastError();
+}
+
+#define NS_DISPATCH_L(L, CALL)                                   \
+    switch (L) {                                                 \
+        case 8: return CALL(8);                                  \
+        case 16: return CALL(16);                                \
+        case 32: return CALL(32);                                \
+        case 64: return CALL(64);                                \
+        case 128: return CALL(128);                              \
+        case 256: return CALL(256);                              \
+        default: return cudaErrorInvalidValue;                   \
+    }
+
+template <typename T>
+static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab) {
+    ColArgs g;
+    g.istride = istride;
+    g.ostride = ostride;
+    g.in_slab = in_slab;
+    g.out_slab = out_slab;
+    g.tiles_per_slab = (int)(ncols / tile_cols<T>());
+    g.total_tiles = (long)g.tiles_per_slab * nslabs;
+    return g;
+}
+
+template <typename T>
+cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
+    if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
+    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
+#define CALL(LL) col_inv_L<T, LL>(st, in, out, g, tw)
+    NS_DISPATCH_L(L, CALL)
+#undef CALL
+}
+
+template <typename T>
+cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
+    if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
+    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
+#define CALL(LL) col_fwd_L<T, LL>(st, in, out, g, scale, tw)
+    NS_DISPATCH_L(L, CALL)
+#undef CALL
+}
+
+template <typename T>
+cudaError_t launch_z_inv_prod(cudaStream_t st, int L, const cx<T>* in, T* phys, long MM, long batch,
+                              unsigned long long* umax2, Twiddles<T> tw) {
+#define CALL(LL) z_inv_L<T, LL>(st, in, phys, MM, batch, umax2, tw)
+    NS_DISPATCH_L(L, CALL)
+#undef CALL
+}
+
+template <typename T>
+cudaError_t launch_z_fwd(cudaStream_t st, int L, const T* phys, cx<T>* out, long MM, long batch, Twiddles<T> tw) {
+#define CALL(LL) z_fwd_L<T, LL>(st, phys, out, MM, batch, tw)
+    NS_DISPATCH_L(L, CALL)
+#undef CALL
+}
+
+#define NS_INSTANTIATE_FFT(T)                                                                                      \
+    template cudaError_t launch_col_inv<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
+                                           long, Twiddles<T>);                                                     \
+    template cudaError_t launch_col_fwd<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
+                                           long, T, Twiddles<T>);                                                  \
+    template cudaError_t launch_z_inv_prod<T>(cudaStream_t, int, const cx<T>*, T*, long, long, unsigned long long*, \
+                                              Twiddles<T>);                                                        \
+    template cudaError_t launch_z_fwd<T>(cudaStream_t, int, const T*, cx<T>*, long, long, Twiddles<T>);
+
+}  // namespace ns

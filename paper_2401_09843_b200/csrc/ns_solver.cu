@@ -1,0 +1,486 @@
+// ns_solver.cu -- host side of libns: the C ABI of include/ns.h, the solver handle, the workspace
+// arena and the launch sequences (RHS pipeline a1..a7, SSP-RK3 driver).  Launches only; every
+// arithmetic step of the path runs in the kernels of this directory.  No CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <string>
+#include <vector>
+
+#include "../../include/ns.h"
+#include "kernels_misc.cuh"
+#include "ns_internal.h"
+
+using namespace ns;
+
+struct ns_solver {
+    std::string err;
+    long long launches = 0;
+    virtual ~ns_solver() {}
+    virtual int set_initial(const void* u, ns_memspace ms) = 0;
+    virtual int set_spectral(const void* u, ns_memspace ms) = 0;
+    virtual int get_spectral(void* u, ns_memspace ms) = 0;
+    virtual int rhs(void* out, ns_memspace ms) = 0;
+    virtual int step_uniform(double dt) = 0;
+    virtual int step_cfl(double cfl, double t_end, double* dt_out) = 0;
+    virtual int step_dts(const double* dt) = 0;
+    virtual int max_velocity(double* out) = 0;
+    virtual int get_fields(void* out, ns_memspace ms) = 0;
+    virtual int energy_spectrum(double* E, int nbins) = 0;
+    virtual int structure_function(double* S, int nl) = 0;
+    virtual double time(int sample) = 0;
+    virtual long long device_bytes() const = 0;
+};
+
+static thread_local std::string g_create_error;
+
+namespace {
+
+double dissipation_rate(const ns_params& p, int N, double k2) {
+    if (k2 <= 0.0) return 0.0;
+    double d = p.nu * k2;
+    if (p.eps != 0.0) {
+        const double kabs = std::sqrt(k2);
+        const double mN = p.m_cut < 0.0 ? std::sqrt((double)N) : p.m_cut;
+        const double qe = p.q_exp < 0.0 ? (2.0 * p.s - 1.0) * 2.0 : p.q_exp;
+        if (kabs > mN) {
+            const double Q = p.q_sharp ? 1.0 : 1.0 - std::pow(mN / kabs, qe);
+            d += p.eps / std::pow((double)N, 2.0 * p.s - 1.0) * std::pow(k2, p.s) * Q;
+        }
+    }
+    return d;
+}
+
+template <typename T>
+class Solver final : public ns_solver {
+public:
+    int N, L, M, H, batch;
+    ns_params prm;
+    cudaStream_t st;
+    bool has_state = false;
+    // arena
+    unsigned char* arena = nullptr;
+    size_t arena_bytes = 0;
+    cx<T>*U = nullptr, *V = nullptr, *X = nullptr, *Y = nullptr;
+    cx<T>*tw3 = nullptr, *twL = nullptr;
+    T* dtab = nullptr;
+    double *dt_dev = nullptr, *t_dev = nullptr, *scal_dev = nullptr, *red_dev = nullptr;
+    unsigned long long* umax2 = nullptr;
+    size_t nS, nX, nY;  // complex element counts of state, X, Y
+    size_t red_count;
+
+    Solver(int N_, int batch_, const ns_params& p, cudaStream_t s) : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), prm(p), st(s) {}
+    ~Solver() override {
+        if (arena) cudaFree(arena);
+    }
+
+    int fail(int code, const std::string& msg) {
+        err = msg;
+        return code;
+    }
+    int cuda_fail(cudaError_t e, const char* where) {
+        err = std::string(where) + ": " + cudaGetErrorString(e);
+        return NS_ERR_CUDA;
+    }
+#define NS_CK(call)                                           \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+#define NS_LAUNCHED(name)                                      \
+    do {                                                       \
+        ++launches;                                            \
+        cudaError_t e__ = cudaGetLastError();                  \
+        if (e__ != cudaSuccess) return cuda_fail(e__, name);   \
+    } while (0)
+
+    Twiddles<T> tw() const { return Twiddles<T>{tw3, twL}; }
+    static unsigned blocks_for(long total, int threads) { return (unsigned)((total + threads - 1) / threads); }
+
+    int init() {
+        const size_t b = (size_t)batch;
+        nS = b * 3 * N * N * H;
+        const size_t phys_c = b * 3 * (size_t)M * M * M;  // 6 M^3 reals = 3 M^3 complex
+        nX = phys_c;                                      // >= A1u (3 M N H), A1b (6 M N H), W (3 N^3), R (3 N^2 H)
+        nY = b * 6 * (size_t)M * M * H;                   // >= A2u, Bh, public staging
+        const size_t pub = b * 3 * (size_t)N * N * (H + 1);
+        if (nY < pub) nY = pub;
+        const size_t ndt = (size_t)3 * L * L + 1;
+        red_count = b * (size_t)(4096 > 3 * N ? 4096 : 3 * N);
+        auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+        size_t off = 0;
+        auto take = [&](size_t bytes) { size_t o = off; off += al(bytes); return o; };
+        const size_t oU = take(nS * sizeof(cx<T>)), oV = take(nS * sizeof(cx<T>));
+        const size_t oX = take(nX * sizeof(cx<T>)), oY = take(nY * sizeof(cx<T>));
+        const size_t o3 = take((size_t)2 * L * sizeof(cx<T>)), oL = take((size_t)L * sizeof(cx<T>));
+        const size_t oD = take(ndt * sizeof(T));
+        const size_t odt = take(b * sizeof(double)), ot = take(b * sizeof(double)), osc = take(b * sizeof(double));
+        const size_t oum = take(b * sizeof(unsigned long long));
+        const size_t ored = take(red_count * sizeof(double));
+        arena_bytes = off;
+        cudaError_t e = cudaMalloc(&arena, arena_bytes);
+        if (e == cudaErrorMemoryAllocation) {
+            cudaGetLastError();
+            char buf[128];
+            snprintf(buf, sizeof buf, "device allocation of %.2f GB failed", (double)arena_bytes / 1e9);
+            return fail(NS_ERR_OOM, buf);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc");
+        U = (cx<T>*)(arena + oU);
+        V = (cx<T>*)(arena + oV);
+        X = (cx<T>*)(arena + oX);
+        Y = (cx<T>*)(arena + oY);
+        tw3 = (cx<T>*)(arena + o3);
+        twL = (cx<T>*)(arena + oL);
+        dtab = (T*)(arena + oD);
+        dt_dev = (double*)(arena + odt);
+        t_dev = (double*)(arena + ot);
+        scal_dev = (double*)(arena + osc);
+        umax2 = (unsigned long long*)(arena + oum);
+        red_dev = (double*)(arena + ored);
+
+        // twiddle tables, evaluated in long double
+        const long double twopi = 6.283185307179586476925286766559005768L;
+        std::vector<cx<T>> h3((size_t)2 * L), hL((size_t)L);
+        for (int n = 0; n < 2 * L; ++n) {
+            const long double a = twopi * (long double)n / (long double)(3 * L);
+            h3[n].x = (T)cosl(a);
+            h3[n].y = (T)sinl(a);
+        }
+        for (int n = 0; n < L; ++n) {
+            const long double a = twopi * (long double)n / (long double)L;
+            hL[n].x = (T)cosl(a);
+            hL[n].y = (T)sinl(a);
+        }
+        std::vector<T> hd(ndt);
+        for (size_t k2 = 0; k2 < ndt; ++k2) hd[k2] = (T)dissipation_rate(prm, N, (double)k2);
+        NS_CK(cudaMemcpyAsync(tw3, h3.data(), h3.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
+        NS_CK(cudaMemcpyAsync(twL, hL.data(), hL.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
+        NS_CK(cudaMemcpyAsync(dtab, hd.data(), hd.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+        NS_CK(cudaMemsetAsync(t_dev, 0, b * sizeof(double), st));
+        NS_CK(cudaMemsetAsync(dt_dev, 0, b * sizeof(double), st));
+        NS_CK(cudaStreamSynchronize(st));
+        return NS_OK;
+    }
+
+    long long device_bytes() const override { return (long long)arena_bytes; }
+
+    // ---------------------------------------------------------------- RHS transform pipeline a1..a6
+    // Uin (internal layout) -> Y = Bh [b][6][N][N][H] (unnormalised)
+    int transform(const cx<T>* Uin, bool want_umax, int upto = 6) {
+        const long NH = (long)N * H, MH = (long)M * H;
+        cudaError_t e;
+        e = launch_col_inv<T>(st, L, Uin, X, NH, (long)batch * 3, NH, NH, (long)N * NH, (long)M * NH, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a1 col_inv x");
+        ++launches;
+        e = launch_col_inv<T>(st, L, X, Y, H, (long)batch * 3 * M, H, H, NH, MH, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
+        ++launches;
+        e = launch_z_inv_prod<T>(st, L, Y, reinterpret_cast<T*>(X), (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a3 z_inv_prod");
+        ++launches;
+        if (upto <= 3) return NS_OK;
+        e = launch_z_fwd<T>(st, L, reinterpret_cast<const T*>(X), Y, (long)M * M, batch, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a4 z_fwd");
+        ++launches;
+        e = launch_col_fwd<T>(st, L, Y, X, H, (long)batch * 6 * M, H, H, MH, NH, (T)1, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a5 col_fwd y");
+        ++launches;
+        e = launch_col_fwd<T>(st, L, X, Y, NH, (long)batch * 6, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a6 col_fwd x");
+        ++launches;
+        return NS_OK;
+    }
+
+    int spectral(const cx<T>* Us, const cx<T>* Un, cx<T>* out, double alpha, double beta, double gamma, int mode) {
+        const long total = (long)batch * N * N * H;
+        const T scale = (T)(1.0 / ((double)M * M * M));
+        spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y, Us, Un, out, N, total, dtab, scale, (T)alpha, (T)beta,
+                                                                    (T)gamma, dt_dev, mode);
+        NS_LAUNCHED("a7 spectral_kernel");
+        return NS_OK;
+    }
+
+    // dt_dev / t_dev must have been set before the first spectral() of the step (stream order)
+    enum DtMode { DT_UNIFORM, DT_ARRAY, DT_CFL };
+    int rk3(DtMode mode, double dt, const double* dts_host, double cfl, double t_end) {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        int rc;
+        const unsigned gb = blocks_for(batch, 128);
+        if (mode == DT_CFL) NS_CK(cudaMemsetAsync(umax2, 0, (size_t)batch * sizeof(unsigned long long), st));
+        if ((rc = transform(U, mode == DT_CFL)) != NS_OK) return rc;
+        if (mode == DT_UNIFORM) {
+            set_dt_uniform_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, dt, batch);
+            NS_LAUNCHED("set_dt_uniform");
+        } else if (mode == DT_ARRAY) {
+            NS_CK(cudaMemcpyAsync(scal_dev, dts_host, (size_t)batch * sizeof(double), cudaMemcpyHostToDevice, st));
+            set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, scal_dev, batch);
+            NS_LAUNCHED("set_dt_array");
+        } else {
+            cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, umax2, cfl, 2.0 * 3.14159265358979323846 / N, t_end, batch);
+            NS_LAUNCHED("cfl_finalize");
+        }
+        // eq. (2.6): u1 = u + dt R(u)
+        if ((rc = spectral(U, nullptr, V, 0.0, 1.0, 1.0, 1)) != NS_OK) return rc;
+        // u2 = 3/4 u + 1/4 u1 + 1/4 dt R(u1)
+        if ((rc = transform(V, false)) != NS_OK) return rc;
+        if ((rc = spectral(V, U, V, 0.75, 0.25, 0.25, 1)) != NS_OK) return rc;
+        // u+ = 1/3 u + 2/3 u2 + 2/3 dt R(u2)
+        if ((rc = transform(V, false)) != NS_OK) return rc;
+        if ((rc = spectral(V, U, U, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 1)) != NS_OK) return rc;
+        return NS_OK;
+    }
+
+    int step_uniform(double dt) override {
+        if (!(dt == dt) || std::isinf(dt)) return fail(NS_ERR_INVALID_ARG, "dt must be finite");
+        return rk3(DT_UNIFORM, dt, nullptr, 0, 0);
+    }
+    int step_dts(const double* dts) override {
+        if (!dts) return fail(NS_ERR_INVALID_ARG, "dt array is NULL");
+        int rc = rk3(DT_ARRAY, 0, dts, 0, 0);
+        if (rc != NS_OK) return rc;
+        NS_CK(cudaStreamSynchronize(st));  // dts is caller memory: do not return before it was read
+        return NS_OK;
+    }
+    int step_cfl(double cfl, double t_end, double* dt_out) override {
+        if (!(cfl > 0.0)) return fail(NS_ERR_INVALID_ARG, "cfl must be positive");
+        int rc = rk3(DT_CFL, 0, nullptr, cfl, t_end);
+        if (rc != NS_OK) return rc;
+        if (dt_out) {
+            NS_CK(cudaMemcpyAsync(dt_out, dt_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
+            NS_CK(cudaStreamSynchronize(st));
+        }
+        return NS_OK;
+    }
+
+    int max_velocity(double* out) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!out) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
+        NS_CK(cudaMemsetAsync(umax2, 0, (size_t)batch * sizeof(unsigned long long), st));
+        int rc = transform(U, true, 3);
+        if (rc != NS_OK) return rc;
+        umax_read_kernel<<<blocks_for(batch, 128), 128, 0, st>>>(scal_dev, umax2, batch);
+        NS_LAUNCHED("umax_read");
+        NS_CK(cudaMemcpyAsync(out, scal_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
+        NS_CK(cudaStreamSynchronize(st));
+        return NS_OK;
+    }
+
+    int rhs(void* out, ns_memspace ms) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!out) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
+        int rc = transform(U, false);
+        if (rc != NS_OK) return rc;
+        if ((rc = spectral(U, nullptr, X, 0, 0, 0, 0)) != NS_OK) return rc;  // R -> X (internal layout)
+        return export_spectral(X, out, ms);
+    }
+
+    // internal [b*3][N][N][H] -> public layout in caller memory
+    int export_spectral(const cx<T>* src, void* out, ns_memspace ms) {
+        const long total_pub = (long)batch * 3 * N * N * (H + 1);
+        cx<T>* dst = ms == NS_DEVICE ? (cx<T>*)out : Y;
+        to_public_kernel<T><<<blocks_for(total_pub, 256), 256, 0, st>>>(src, dst, N, total_pub);
+        NS_LAUNCHED("to_public");
+        if (ms == NS_HOST) {
+            NS_CK(cudaMemcpyAsync(out, Y, (size_t)total_pub * sizeof(cx<T>), cudaMemcpyDeviceToHost, st));
+            NS_CK(cudaStreamSynchronize(st));
+        }
+        return NS_OK;
+    }
+
+    int get_spectral(void* out, ns_memspace ms) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!out) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
+        return export_spectral(U, out, ms);
+    }
+
+    int set_spectral(const void* in, ns_memspace ms) override {
+        if (!in) return fail(NS_ERR_INVALID_ARG, "input pointer is NULL");
+        const long total_pub = (long)batch * 3 * N * N * (H + 1);
+        const cx<T>* src = (const cx<T>*)in;
+        if (ms == NS_HOST) {
+            NS_CK(cudaMemcpyAsync(Y, in, (size_t)total_pub * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
+            src = Y;
+        }
+        const long total = (long)batch * 3 * N * N * H;
+        to_internal_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, U, N, total);
+        NS_LAUNCHED("to_internal");
+        if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));  // caller buffer fully consumed
+        has_state = true;
+        return NS_OK;
+    }
+
+    int generic_fft3(cx<T>* W, long cubes, int sign) {
+        int log2n = 0;
+        while ((1 << log2n) < N) ++log2n;
+        const long tiles = cubes * (long)N * N / 8;
+        const size_t smem = (size_t)N * 9 * sizeof(cx<T>);
+        if (smem > 48 * 1024)
+            NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        for (int axis = 0; axis < 3; ++axis) {
+            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2n, axis, sign, tiles);
+            NS_LAUNCHED("generic_fft");
+        }
+        return NS_OK;
+    }
+
+    int set_initial(const void* in, ns_memspace ms) override {
+        if (!in) return fail(NS_ERR_INVALID_ARG, "input pointer is NULL");
+        const long cubes = (long)batch * 3;
+        const long total = cubes * N * N * N;
+        const T* src = (const T*)in;
+        if (ms == NS_HOST) {
+            NS_CK(cudaMemcpyAsync(Y, in, (size_t)total * sizeof(T), cudaMemcpyHostToDevice, st));
+            src = reinterpret_cast<const T*>(Y);
+        }
+        real_to_complex_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, X, total);
+        NS_LAUNCHED("real_to_complex");
+        int rc = generic_fft3(X, cubes, -1);
+        if (rc != NS_OK) return rc;
+        const long tot = (long)batch * N * N * H;
+        init_project_kernel<T><<<blocks_for(tot, 256), 256, 0, st>>>(X, U, N, tot, (T)(1.0 / ((double)N * N * N)));
+        NS_LAUNCHED("init_project");
+        NS_CK(cudaMemsetAsync(t_dev, 0, (size_t)batch * sizeof(double), st));
+        if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));
+        has_state = true;
+        return NS_OK;
+    }
+
+    int get_fields(void* out, ns_memspace ms) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!out) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
+        const long cubes = (long)batch * 3;
+        const long total = cubes * N * N * N;
+        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        NS_LAUNCHED("expand_hermitian");
+        int rc = generic_fft3(X, cubes, +1);
+        if (rc != NS_OK) return rc;
+        T* dst = ms == NS_DEVICE ? (T*)out : reinterpret_cast<T*>(Y);
+        complex_to_real_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(X, dst, total);
+        NS_LAUNCHED("complex_to_real");
+        if (ms == NS_HOST) {
+            NS_CK(cudaMemcpyAsync(out, dst, (size_t)total * sizeof(T), cudaMemcpyDeviceToHost, st));
+            NS_CK(cudaStreamSynchronize(st));
+        }
+        return NS_OK;
+    }
+
+    int energy_spectrum(double* E, int nbins) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!E || nbins < 1 || nbins > 4096) return fail(NS_ERR_INVALID_ARG, "E is NULL or nbins not in [1, 4096]");
+        NS_CK(cudaMemsetAsync(red_dev, 0, (size_t)batch * nbins * sizeof(double), st));
+        const long plane = (long)N * N * H;
+        unsigned chunks = blocks_for(plane, 256 * 16);
+        if (chunks > 1024) chunks = 1024;
+        energy_spectrum_kernel<T><<<dim3(chunks, batch), 256, (size_t)nbins * sizeof(double), st>>>(U, red_dev, N, nbins);
+        NS_LAUNCHED("energy_spectrum");
+        NS_CK(cudaMemcpyAsync(E, red_dev, (size_t)batch * nbins * sizeof(double), cudaMemcpyDeviceToHost, st));
+        NS_CK(cudaStreamSynchronize(st));
+        return NS_OK;
+    }
+
+    int structure_function(double* S, int nl) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!S || nl < 1 || nl > N / 2) return fail(NS_ERR_INVALID_ARG, "S is NULL or nl not in [1, N/2]");
+        NS_CK(cudaMemsetAsync(red_dev, 0, (size_t)batch * 3 * N * sizeof(double), st));
+        const long plane = (long)N * N * H;
+        unsigned chunks = blocks_for(plane, 256 * 16);
+        if (chunks > 1024) chunks = 1024;
+        sf_marginals_kernel<T><<<dim3(chunks, batch), 256, (size_t)3 * N * sizeof(double), st>>>(U, red_dev, N);
+        NS_LAUNCHED("sf_marginals");
+        double* out_dev = reinterpret_cast<double*>(Y);
+        sf_finalize_kernel<<<batch, 128, 0, st>>>(red_dev, out_dev, N, nl);
+        NS_LAUNCHED("sf_finalize");
+        NS_CK(cudaMemcpyAsync(S, out_dev, (size_t)batch * nl * sizeof(double), cudaMemcpyDeviceToHost, st));
+        NS_CK(cudaStreamSynchronize(st));
+        return NS_OK;
+    }
+
+    double time(int sample) override {
+        if (sample < 0 || sample >= batch) return std::numeric_limits<double>::quiet_NaN();
+        double t = 0.0;
+        if (cudaMemcpyAsync(&t, t_dev + sample, sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess)
+            return std::numeric_limits<double>::quiet_NaN();
+        return t;
+    }
+};
+
+template <typename T>
+int create_typed(ns_solver** out, int N, int batch, const ns_params& p, cudaStream_t st) {
+    Solver<T>* s = new Solver<T>(N, batch, p, st);
+    int rc = s->init();
+    if (rc != NS_OK) {
+        g_create_error = s->err;
+        delete s;
+        return rc;
+    }
+    *out = s;
+    return NS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream) {
+    g_create_error.clear();
+    if (!out) { g_create_error = "out is NULL"; return NS_ERR_INVALID_ARG; }
+    *out = nullptr;
+    const int min_n = dtype == NS_F32 ? 32 : 16;
+    if (N < min_n || N > 512 || (N & (N - 1)) != 0 || !fft_supported(N / 2)) {
+        g_create_error = "N must be a power of two in [16, 512] (fp32: [32, 512])";
+        return NS_ERR_INVALID_ARG;
+    }
+    if (batch < 1) { g_create_error = "batch must be >= 1"; return NS_ERR_INVALID_ARG; }
+    if (dtype != NS_F64 && dtype != NS_F32) { g_create_error = "unknown dtype"; return NS_ERR_INVALID_ARG; }
+    ns_params prm;
+    std::memset(&prm, 0, sizeof prm);
+    prm.s = 1.0;
+    prm.m_cut = -1.0;
+    prm.q_exp = -1.0;
+    if (p) prm = *p;
+    if (!(prm.s >= 1.0) || prm.nu < 0.0 || prm.eps < 0.0 || !(prm.nu == prm.nu) || !(prm.eps == prm.eps)) {
+        g_create_error = "params: need s >= 1, nu >= 0, eps >= 0";
+        return NS_ERR_INVALID_ARG;
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        g_create_error = std::string("no usable CUDA device (no CPU fallback): ") + (e != cudaSuccess ? cudaGetErrorString(e) : "0 devices");
+        return NS_ERR_CUDA;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return dtype == NS_F64 ? create_typed<double>(out, N, batch, prm, st) : create_typed<float>(out, N, batch, prm, st);
+}
+
+int ns_destroy(ns_solver* h) {
+    if (!h) return NS_ERR_INVALID_ARG;
+    delete h;
+    return NS_OK;
+}
+
+#define NS_H(h) if (!(h)) return NS_ERR_INVALID_ARG; (h)->err.clear()
+
+int ns_set_initial(ns_solver* h, const void* u, ns_memspace ms) { NS_H(h); return h->set_initial(u, ms); }
+int ns_set_spectral(ns_solver* h, const void* u, ns_memspace ms) { NS_H(h); return h->set_spectral(u, ms); }
+int ns_get_spectral(ns_solver* h, void* u, ns_memspace ms) { NS_H(h); return h->get_spectral(u, ms); }
+int ns_rhs(ns_solver* h, void* out, ns_memspace ms) { NS_H(h); return h->rhs(out, ms); }
+int ns_step(ns_solver* h, double dt) { NS_H(h); return h->step_uniform(dt); }
+int ns_step_cfl(ns_solver* h, double cfl, double t_end, double* dt_out) { NS_H(h); return h->step_cfl(cfl, t_end, dt_out); }
+int ns_step_dts(ns_solver* h, const double* dt) { NS_H(h); return h->step_dts(dt); }
+int ns_max_velocity(ns_solver* h, double* out) { NS_H(h); return h->max_velocity(out); }
+int ns_get_fields(ns_solver* h, void* out, ns_memspace ms) { NS_H(h); return h->get_fields(out, ms); }
+int ns_energy_spectrum(ns_solver* h, double* E, int nbins) { NS_H(h); return h->energy_spectrum(E, nbins); }
+int ns_structure_function(ns_solver* h, double* S, int nl) { NS_H(h); return h->structure_function(S, nl); }
+double ns_time(const ns_solver* h, int sample) {
+    if (!h) return std::numeric_limits<double>::quiet_NaN();
+    return const_cast<ns_solver*>(h)->time(sample);
+}
+long long ns_kernel_launches(const ns_solver* h) { return h ? h->launches : 0; }
+long long ns_device_bytes(const ns_solver* h) { return h ? h->device_bytes() : 0; }
+const char* ns_last_error(const ns_solver* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

