@@ -15,7 +15,7 @@
  * listed in DESIGN.md section 3 (A1..A18).
  *
  * Conventions
- *   N         grid points per axis, a power of two, 8 <= N <= 1024.  Padded grid M = 3N/2.
+ *   N         grid points per axis, a power of two, 16 <= N <= 512 (fp32: 32 <= N).  Padded grid M = 3N/2.
  *   spectral  complex interleaved (re,im) of `dtype`, shape [batch][3][N][N][N/2+1], index
  *             [b][component][ikx][iky][ikz], ikz fastest (r2c half spectrum, kz >= 0).
  *             Stored index i <-> wavenumber k = i (i < N/2) or i - N (i > N/2).  Coefficients are
@@ -69,7 +69,8 @@ typedef struct {
 } ns_params;
 
 /* Create a solver for `batch` independent samples on an N^3 grid.  `p` may be NULL (inviscid).
- * Allocates all device workspaces (about 40 * batch * N^3 * sizeof(complex) bytes).
+ * Allocates one device arena of about 20 * batch * N^3 * sizeof(complex) bytes (state, stage
+ * state and two ping-pong workspaces shared by all passes, cf. "Workspaces").
  * cuda_stream: a cudaStream_t cast to void* (NULL = default stream). */
 int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream);
 int ns_destroy(ns_solver* h);
@@ -113,6 +114,14 @@ int ns_structure_function(ns_solver* h, double* S_out, int nl);
 
 /* Simulation time of one sample; NaN if `sample` is out of range. */
 double ns_time(const ns_solver* h, int sample);
+/* Per-pass timing with CUDA events recorded on the solver's stream between the kernels of the RHS
+ * (measurement aid for bench.py; adds one event record per kernel when enabled).  ns_profile(h, 1)
+ * synchronises, clears the accumulators and enables; ns_profile(h, 0) disables.  ns_profile_read
+ * synchronises and returns, for the 8 passes {a1 col_inv_x, a2 col_inv_y, a3 z_inv_prod, a4 z_fwd,
+ * a5 col_fwd_y, a6 col_fwd_x, a7 spectral, other}, the accumulated milliseconds ms_out[8] and launch
+ * counts count_out[8] (host arrays) since it was enabled. */
+int ns_profile(ns_solver* h, int enable);
+int ns_profile_read(ns_solver* h, double* ms_out, long long* count_out);
 /* Number of kernels the library has launched on this handle so far (for bench.py's gpu_launches). */
 long long ns_kernel_launches(const ns_solver* h);
 /* Device bytes held by the handle. */

@@ -22,7 +22,7 @@ NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE = 0, -1, -2, -3
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
     "ns_step_cfl", "ns_step_dts", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum",
-    "ns_structure_function", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
+    "ns_structure_function", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
 
 
@@ -62,6 +62,8 @@ def lib():
         L.ns_get_fields.argtypes = [vp, vp, i]
         L.ns_energy_spectrum.argtypes = [vp, vp, i]
         L.ns_structure_function.argtypes = [vp, vp, i]
+        L.ns_profile.argtypes = [vp, i]
+        L.ns_profile_read.argtypes = [vp, vp, vp]
         L.ns_time.argtypes = [vp, i]
         L.ns_time.restype = d
         L.ns_kernel_launches.argtypes = [vp]
@@ -212,6 +214,19 @@ class Solver:
         S = np.empty((self.batch, nl), dtype=np.float64)
         self._check(lib().ns_structure_function(self._h, ctypes.c_void_p(S.ctypes.data), nl))
         return S
+
+    PASS_NAMES = ["a1_col_inv_x", "a2_col_inv_y", "a3_z_inv_prod", "a4_z_fwd", "a5_col_fwd_y", "a6_col_fwd_x",
+                  "a7_spectral", "other"]
+
+    def profile(self, enable=True):
+        self._check(lib().ns_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """{pass name: (total ms, launches)} accumulated since profile(True)."""
+        ms = np.zeros(8, dtype=np.float64)
+        cnt = np.zeros(8, dtype=np.int64)
+        self._check(lib().ns_profile_read(self._h, ctypes.c_void_p(ms.ctypes.data), ctypes.c_void_p(cnt.ctypes.data)))
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(self.PASS_NAMES)}
 
     def time(self, sample=0):
         return float(lib().ns_time(self._h, int(sample)))

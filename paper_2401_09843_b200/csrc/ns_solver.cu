@@ -31,6 +31,8 @@ struct ns_solver {
     virtual int structure_function(double* S, int nl) = 0;
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
+    virtual int profile(int enable) = 0;
+    virtual int profile_read(double* ms, long long* cnt) = 0;
 };
 
 static thread_local std::string g_create_error;
@@ -52,6 +54,50 @@ double dissipation_rate(const ns_params& p, int N, double k2) {
     return d;
 }
 
+// Optional per-pass timing with CUDA events on the solver's stream (ns_profile / ns_profile_read).
+// Passes: 0 a1 col_inv_x, 1 a2 col_inv_y, 2 a3 z_inv_prod, 3 a4 z_fwd, 4 a5 col_fwd_y, 5 a6 col_fwd_x,
+//         6 a7 spectral, 7 other (dt bookkeeping).  An event is recorded at the start of every pass.
+struct PassProfiler {
+    static constexpr int NPASS = 8;
+    static constexpr size_t MAX_EVENTS = 1 << 16;
+    bool on = false;
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> tag;
+    size_t used = 0;
+    double ms[NPASS] = {0};
+    long long cnt[NPASS] = {0};
+    ~PassProfiler() {
+        for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    }
+    void reset() {
+        used = 0;
+        for (int i = 0; i < NPASS; ++i) { ms[i] = 0; cnt[i] = 0; }
+    }
+    void tick(int pass, cudaStream_t st) {  // pass < 0: end marker
+        if (!on || used >= MAX_EVENTS) return;
+        if (used == ev.size()) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return;
+            ev.push_back(e);
+            tag.push_back(-1);
+        }
+        tag[used] = pass;
+        cudaEventRecord(ev[used], st);
+        ++used;
+    }
+    void collect() {  // stream must be synchronised
+        for (size_t i = 0; i + 1 < used; ++i) {
+            if (tag[i] < 0) continue;
+            float t = 0;
+            if (cudaEventElapsedTime(&t, ev[i], ev[i + 1]) == cudaSuccess) {
+                ms[tag[i]] += t;
+                cnt[tag[i]] += 1;
+            }
+        }
+        used = 0;
+    }
+};
+
 template <typename T>
 class Solver final : public ns_solver {
 public:
@@ -69,6 +115,7 @@ public:
     unsigned long long* umax2 = nullptr;
     size_t nS, nX, nY;  // complex element counts of state, X, Y
     size_t red_count;
+    PassProfiler prof;
 
     Solver(int N_, int batch_, const ns_params& p, cudaStream_t s) : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), prm(p), st(s) {}
     ~Solver() override {
@@ -171,34 +218,43 @@ public:
     int transform(const cx<T>* Uin, bool want_umax, int upto = 6) {
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
+        prof.tick(0, st);
         e = launch_col_inv<T>(st, L, Uin, X, NH, (long)batch * 3, NH, NH, (long)N * NH, (long)M * NH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a1 col_inv x");
         ++launches;
+        prof.tick(1, st);
         e = launch_col_inv<T>(st, L, X, Y, H, (long)batch * 3 * M, H, H, NH, MH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
         ++launches;
+        prof.tick(2, st);
         e = launch_z_inv_prod<T>(st, L, Y, reinterpret_cast<T*>(X), (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a3 z_inv_prod");
         ++launches;
-        if (upto <= 3) return NS_OK;
+        if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
+        prof.tick(3, st);
         e = launch_z_fwd<T>(st, L, reinterpret_cast<const T*>(X), Y, (long)M * M, batch, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a4 z_fwd");
         ++launches;
+        prof.tick(4, st);
         e = launch_col_fwd<T>(st, L, Y, X, H, (long)batch * 6 * M, H, H, MH, NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a5 col_fwd y");
         ++launches;
+        prof.tick(5, st);
         e = launch_col_fwd<T>(st, L, X, Y, NH, (long)batch * 6, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a6 col_fwd x");
         ++launches;
+        prof.tick(7, st);
         return NS_OK;
     }
 
     int spectral(const cx<T>* Us, const cx<T>* Un, cx<T>* out, double alpha, double beta, double gamma, int mode) {
         const long total = (long)batch * N * N * H;
         const T scale = (T)(1.0 / ((double)M * M * M));
+        prof.tick(6, st);
         spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y, Us, Un, out, N, total, dtab, scale, (T)alpha, (T)beta,
                                                                     (T)gamma, dt_dev, mode);
         NS_LAUNCHED("a7 spectral_kernel");
+        prof.tick(-1, st);
         return NS_OK;
     }
 
@@ -397,6 +453,20 @@ public:
         return NS_OK;
     }
 
+    int profile(int enable) override {
+        NS_CK(cudaStreamSynchronize(st));
+        prof.reset();
+        prof.on = enable != 0;
+        return NS_OK;
+    }
+    int profile_read(double* ms, long long* cnt) override {
+        if (!ms || !cnt) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
+        NS_CK(cudaStreamSynchronize(st));
+        prof.collect();
+        for (int i = 0; i < PassProfiler::NPASS; ++i) { ms[i] = prof.ms[i]; cnt[i] = prof.cnt[i]; }
+        return NS_OK;
+    }
+
     double time(int sample) override {
         if (sample < 0 || sample >= batch) return std::numeric_limits<double>::quiet_NaN();
         double t = 0.0;
@@ -479,6 +549,8 @@ double ns_time(const ns_solver* h, int sample) {
     if (!h) return std::numeric_limits<double>::quiet_NaN();
     return const_cast<ns_solver*>(h)->time(sample);
 }
+int ns_profile(ns_solver* h, int enable) { NS_H(h); return h->profile(enable); }
+int ns_profile_read(ns_solver* h, double* ms, long long* cnt) { NS_H(h); return h->profile_read(ms, cnt); }
 long long ns_kernel_launches(const ns_solver* h) { return h ? h->launches : 0; }
 long long ns_device_bytes(const ns_solver* h) { return h ? h->device_bytes() : 0; }
 const char* ns_last_error(const ns_solver* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
