@@ -19,6 +19,7 @@
 // rows a_n, c_n are read from HBM exactly once and stay in registers.
 #pragma once
 #include "cx.cuh"
+#include "ns_internal.h"
 
 namespace ns {
 
@@ -37,7 +38,7 @@ template <int R1, int R2> struct ColP { static constexpr int value = R1 > R2 ? R
 template <typename T, int L, int R1, int R2, int TC, int TPB>
 __global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
 col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
-               const cx<T>* __restrict__ tw3, const cx<T>* __restrict__ twL) {
+               Twiddles<T> tw) {
     static_assert(R1 * R2 == L && R2 >= 2, "two register stages");
     constexpr int P = ColP<R1, R2>::value;
     constexpr int TT = TC * P;  // threads per tile
@@ -89,14 +90,14 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
                     // a + c w3^{-q}:  q=1: t1 - i t2,  q=2: t1 + i t2
                     const cx<T> z = (q == 1) ? mk<T>(a[n1].x + cc[n1].y, a[n1].y - cc[n1].x)
                                              : mk<T>(a[n1].x - cc[n1].y, a[n1].y + cc[n1].x);
-                    s[n1] = cmul(z, ldg(tw3 + q * n));
+                    s[n1] = cmul(z, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
                 }
             }
             fft_reg<R1, +1, T>(s);
 #pragma unroll
             for (int r1 = 0; r1 < R1; ++r1) {
                 cx<T> v = s[brev<R1>(r1)];
-                if (r1 > 0) v = cmul(v, ldg(twL + r1 * i));
+                if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
                 Et[buf * EBUF + (size_t)(r1 * R2 + i) * TC + c] = v;
             }
         }
@@ -119,7 +120,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 template <typename T, int L, int R1, int R2, int TC, int TPB>
 __global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
 col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale,
-               const cx<T>* __restrict__ tw3, const cx<T>* __restrict__ twL) {
+               Twiddles<T> tw) {
     static_assert(R1 * R2 == L && R2 >= 2, "two register stages");
     constexpr int P = ColP<R1, R2>::value;
     constexpr int TT = TC * P;
@@ -151,7 +152,7 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 #pragma unroll
             for (int n2 = 0; n2 < R2; ++n2) {
                 cx<T> v = x[brev<R2>(n2)];
-                if (n2 > 0) v = cmulc(v, ldg(twL + i * n2));
+                if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
                 Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c] = v;
             }
         }
@@ -168,13 +169,13 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) {
                     const int n = R2 * n1 + i;
-                    G1[(size_t)n * TC + c] = cmulc(y[brev<R1>(n1)], ldg(tw3 + n));
+                    G1[(size_t)n * TC + c] = cmulc(y[brev<R1>(n1)], ldg(tw.w3a + n));
                 }
             } else {
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) {
                     const int n = R2 * n1 + i;
-                    const cx<T> g2 = cmulc(y[brev<R1>(n1)], ldg(tw3 + 2 * n));
+                    const cx<T> g2 = cmulc(y[brev<R1>(n1)], ldg(tw.w3b + n));
                     const cx<T> g1 = G1[(size_t)n * TC + c];
                     const cx<T> S = g1 + g2, D = g1 - g2;
                     constexpr T h3 = (T)0.86602540378443864676L;

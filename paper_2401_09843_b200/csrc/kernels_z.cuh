@@ -14,6 +14,7 @@
 // transposes for 16-byte and 8-byte elements).
 #pragma once
 #include "cx.cuh"
+#include "ns_internal.h"
 
 namespace ns {
 
@@ -22,7 +23,6 @@ template <int R1, int R2> struct ZP { static constexpr int value = R1 > R2 ? R1 
 // Products are stored in this order (same as the spectral kernel expects): 11 12 13 22 23 33.
 // Forward pairs: (11,22) (33,12) (13,23).
 
-template <typename T>
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v) {
     atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
@@ -33,8 +33,7 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, doub
 template <typename T, int L, int R1, int R2, int LPB>
 __global__ void __launch_bounds__(3 * ZP<R1, R2>::value* LPB)
 z_inv_prod_kernel(const cx<T>* __restrict__ in, T* __restrict__ out, long MM, long total_lines,
-                  unsigned long long* __restrict__ umax2, const cx<T>* __restrict__ tw3,
-                  const cx<T>* __restrict__ twL) {
+                  unsigned long long* __restrict__ umax2, Twiddles<T> tw) {
     static_assert(R1 * R2 == L && R2 >= 2, "two register stages");
     constexpr int P = ZP<R1, R2>::value;
     constexpr int PITCH = R2 + 1;
@@ -78,14 +77,14 @@ z_inv_prod_kernel(const cx<T>* __restrict__ in, T* __restrict__ out, long MM, lo
                 const cx<T> t1 = mk<T>(a.x - (T)0.5 * c.x, a.y - (T)0.5 * c.y);
                 const cx<T> t2 = h3 * c;
                 const cx<T> z = (q == 1) ? mk<T>(t1.x + t2.y, t1.y - t2.x) : mk<T>(t1.x - t2.y, t1.y + t2.x);
-                s[n1] = cmul(z, ldg(tw3 + q * n));
+                s[n1] = cmul(z, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
             }
         }
         fft_reg<R1, +1, T>(s);
 #pragma unroll
         for (int r1 = 0; r1 < R1; ++r1) {
             cx<T> v = s[brev<R1>(r1)];
-            if (r1 > 0) v = cmul(v, ldg(twL + r1 * i));
+            if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
             Eq[r1 * PITCH + i] = v;
         }
     }
@@ -117,14 +116,14 @@ z_inv_prod_kernel(const cx<T>* __restrict__ in, T* __restrict__ out, long MM, lo
                 const cx<T> t1 = mk<T>(a.x - (T)0.5 * c.x, a.y - (T)0.5 * c.y);
                 const cx<T> t2 = h3 * c;
                 const cx<T> z = (q == 1) ? mk<T>(t1.x + t2.y, t1.y - t2.x) : mk<T>(t1.x - t2.y, t1.y + t2.x);
-                s[n1] = cmul(z, ldg(tw3 + q * n));
+                s[n1] = cmul(z, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
             }
         }
         fft_reg<R1, +1, T>(s);
 #pragma unroll
         for (int r1 = 0; r1 < R1; ++r1) {
             cx<T> v = s[brev<R1>(r1)];
-            if (r1 > 0) v = cmul(v, ldg(twL + r1 * i));
+            if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
             Eq[EBUF + r1 * PITCH + i] = v;
         }
     }
@@ -158,7 +157,7 @@ z_inv_prod_kernel(const cx<T>* __restrict__ in, T* __restrict__ out, long MM, lo
             // lanes of one warp may belong to different lines but, when LPB | MM, to the same sample
             lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
         }
-        if ((threadIdx.x & 31) == 0) atomic_max_nonneg<T>(umax2 + b, (double)lmax);
+        if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax2 + b, (double)lmax);
     }
 }
 
@@ -168,7 +167,7 @@ z_inv_prod_kernel(const cx<T>* __restrict__ in, T* __restrict__ out, long MM, lo
 template <typename T, int L, int R1, int R2, int LPB>
 __global__ void __launch_bounds__(3 * ZP<R1, R2>::value* LPB)
 z_fwd_kernel(const T* __restrict__ in, cx<T>* __restrict__ out, long MM, long total_lines,
-             const cx<T>* __restrict__ tw3, const cx<T>* __restrict__ twL) {
+             Twiddles<T> tw) {
     static_assert(R1 * R2 == L && R2 >= 2, "two register stages");
     constexpr int P = ZP<R1, R2>::value;
     constexpr int PITCH = R2 + 1;
@@ -206,7 +205,7 @@ z_fwd_kernel(const T* __restrict__ in, cx<T>* __restrict__ out, long MM, long to
 #pragma unroll
             for (int n2 = 0; n2 < R2; ++n2) {
                 cx<T> v = x[brev<R2>(n2)];
-                if (n2 > 0) v = cmulc(v, ldg(twL + i * n2));
+                if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
                 Eq[i * PITCH + n2] = v;
             }
         }
@@ -220,7 +219,7 @@ z_fwd_kernel(const T* __restrict__ in, cx<T>* __restrict__ out, long MM, long to
             for (int n1 = 0; n1 < R1; ++n1) {
                 const int n = R2 * n1 + i;
                 cx<T> v = y[brev<R1>(n1)];
-                if (q > 0) v = cmulc(v, ldg(tw3 + q * n));
+                if (q > 0) v = cmulc(v, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
                 Cl[q * L + n] = v;
             }
         }

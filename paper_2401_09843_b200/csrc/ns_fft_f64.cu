@@ -3,4 +3,15 @@
 namespace ns {
 NS_INSTANTIATE_FFT(double)
 bool fft_supported(int L) { return L == 8 || L == 16 || L == 32 || L == 64 || L == 128 || L == 256; }
+void fft_split(int L, int* R1, int* R2) {
+    switch (L) {
+        case 8: *R1 = Split<8>::R1; *R2 = Split<8>::R2; break;
+        case 16: *R1 = Split<16>::R1; *R2 = Split<16>::R2; break;
+        case 32: *R1 = Split<32>::R1; *R2 = Split<32>::R2; break;
+        case 64: *R1 = Split<64>::R1; *R2 = Split<64>::R2; break;
+        case 128: *R1 = Split<128>::R1; *R2 = Split<128>::R2; break;
+        case 256: *R1 = Split<256>::R1; *R2 = Split<256>::R2; break;
+        default: *R1 = 0; *R2 = 0;
+    }
+}
 }  // namespace ns

@@ -2,6 +2,8 @@
 #pragma once
 #include "kernels_col.cuh"
 #include "kernels_z.cuh"
+#include "kernels_zfused.cuh"
+#include "kernels_zfused8.cuh"
 #include "ns_internal.h"
 
 namespace ns {
@@ -25,6 +27,10 @@ template <int L> struct Cfg {
     }
     // lines per block for the z kernels: aim at 192 threads
     static constexpr int lpb() { return (3 * P) >= 192 ? 1 : 192 / (3 * P); }
+    // lines per block for the fused z kernel: ~96 threads for the long lines (shared memory bound), 192 otherwise
+    static constexpr int lpbf() { return L >= 128 ? 2 : 192 / (3 * P); }
+    // target CTAs per SM of the fused z kernel (bounds its registers)
+    static constexpr int minbf() { return L >= 128 ? 4 : 2; }
 };
 
 template <typename K>
@@ -42,7 +48,7 @@ static cudaError_t col_inv_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
     const long blocks = (g.total_tiles + TPB - 1) / TPB;
-    k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, tw.tw3, tw.twL);
+    k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, tw);
     return cudaGetLastError();
 }
 
@@ -55,7 +61,7 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
     const long blocks = (g.total_tiles + TPB - 1) / TPB;
-    k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, scale, tw.tw3, tw.twL);
+    k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, scale, tw);
     return cudaGetLastError();
 }
 
@@ -69,7 +75,7 @@ static cudaError_t z_inv_L(cudaStream_t st, const cx<T>* in, T* phys, long MM, l
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
     const long total = MM * batch;
-    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(in, phys, MM, total, umax2, tw.tw3, tw.twL);
+    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(in, phys, MM, total, umax2, tw);
     return cudaGetLastError();
 }
 
@@ -82,7 +88,70 @@ static cudaError_t z_fwd_L(cudaStream_t st, const T* phys, cx<T>* out, long MM, 
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
     const long total = MM * batch;
-    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(phys, out, MM, total, tw.tw3, tw.twL);
+    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(phys, out, MM, total, tw);
+    return cudaGetLastError();
+}
+
+template <typename T, int L>
+static cudaError_t z_fused_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+                             Twiddles<T> tw) {
+    using C = Cfg<L>;
+    constexpr int LPB = C::lpbf();
+    constexpr bool SEP = false;
+    auto k = z_fused_kernel<T, L, C::R1, C::R2, LPB, C::minbf(), SEP>;
+    const size_t smem = (size_t)LPB * (3 * L + (SEP ? 2 : 1) * 3 * C::R1 * (C::R2 + 1)) * sizeof(cx<T>) + 16;
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
+    const long tiles = MM * batch / LPB;
+    static int num_sms = 0;
+    if (num_sms == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 3 * C::P * LPB, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    long grid = (long)num_sms * occ;
+    if (grid > tiles) grid = tiles;
+    k<<<(unsigned)grid, 3 * C::P * LPB, smem, st>>>(in, out, MM, tiles, umax2, tw);
+    return cudaGetLastError();
+}
+
+// warp-synchronous fused z kernel for L >= 64
+template <int L> struct Z8Cfg;
+template <> struct Z8Cfg<64>  { static constexpr int LPB = 8, MINB = 2; };
+template <> struct Z8Cfg<128> { static constexpr int LPB = 4, MINB = 2; };
+template <> struct Z8Cfg<256> { static constexpr int LPB = 2, MINB = 2; };
+
+template <typename T, int L>
+static cudaError_t z_fused8_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+                              Twiddles<T> tw) {
+    constexpr int LPB = Z8Cfg<L>::LPB;
+    constexpr int G = L / 8, R3 = G / 8;
+    auto k = z_fused8_kernel<T, L, LPB, Z8Cfg<L>::MINB>;
+    const size_t smem = (size_t)LPB * 3 * (L + Z8Geo<R3>::SZ) * sizeof(cx<T>) + (size_t)LPB * 8 + 8;
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
+    const long lines = MM * batch;
+    static int num_sms = 0;
+    if (num_sms == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 3 * G * LPB, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    long grid = (long)num_sms * occ;
+    if (grid > lines / LPB) grid = lines / LPB;
+    k<<<(unsigned)grid, 3 * G * LPB, smem, st>>>(in, out, MM, lines, umax2, tw);
     return cudaGetLastError();
 }
 
@@ -144,6 +213,17 @@ cudaError_t launch_z_fwd(cudaStream_t st, int L, const T* phys, cx<T>* out, long
 #undef CALL
 }
 
+template <typename T>
+cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
+                           unsigned long long* umax2, Twiddles<T> tw) {
+    if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
+    if (L == 128) return z_fused8_L<T, 128>(st, in, out, MM, batch, umax2, tw);
+    if (L == 256) return z_fused8_L<T, 256>(st, in, out, MM, batch, umax2, tw);
+#define CALL(LL) z_fused_L<T, LL>(st, in, out, MM, batch, umax2, tw)
+    NS_DISPATCH_L(L, CALL)
+#undef CALL
+}
+
 #define NS_INSTANTIATE_FFT(T)                                                                                      \
     template cudaError_t launch_col_inv<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, Twiddles<T>);                                                     \
@@ -151,6 +231,8 @@ cudaError_t launch_z_fwd(cudaStream_t st, int L, const T* phys, cx<T>* out, long
                                            long, T, Twiddles<T>);                                                  \
     template cudaError_t launch_z_inv_prod<T>(cudaStream_t, int, const cx<T>*, T*, long, long, unsigned long long*, \
                                               Twiddles<T>);                                                        \
-    template cudaError_t launch_z_fwd<T>(cudaStream_t, int, const T*, cx<T>*, long, long, Twiddles<T>);
+    template cudaError_t launch_z_fwd<T>(cudaStream_t, int, const T*, cx<T>*, long, long, Twiddles<T>);                \
+    template cudaError_t launch_z_fused<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, unsigned long long*,   \
+                                           Twiddles<T>);
 
 }  // namespace ns

@@ -7,11 +7,23 @@
 
 namespace ns {
 
+// Twiddle tables, laid out so that the lanes of a warp read consecutive entries:
+//   twA[r1 * R2 + n2] = twB[n2 * R1 + r1] = exp(+2 pi i r1 n2 / L)      (inter-stage twiddles, L = R1 R2)
+//   w3a[n] = exp(+2 pi i n / (3L)),  w3b[n] = exp(+2 pi i 2n / (3L)),  n < L   (pruned radix-3 twiddles)
 template <typename T>
 struct Twiddles {
-    const cx<T>* tw3;  // [2L]  exp(+2 pi i n / (3L))
-    const cx<T>* twL;  // [L]   exp(+2 pi i n / L)
+    const cx<T>* twA;
+    const cx<T>* twB;
+    const cx<T>* w3a;
+    const cx<T>* w3b;
+    // tables of the 8-values-per-lane z kernel (kernels_zfused8.cuh), G = L/8, R3 = G/8 (L >= 64 only):
+    //   z8A[r1*G + t] = w_L^{r1 t},  z8B[ta*G + t] = w_L^{(t/R3)(R3 ta + t%R3)},  z8C[rA*R3 + tb] = w_G^{rA tb}
+    const cx<T>* z8A;
+    const cx<T>* z8B;
+    const cx<T>* z8C;
 };
+// register-stage split L = R1 x R2 used by the kernels (needed by the host to build twA / twB)
+void fft_split(int L, int* R1, int* R2);
 
 // true if the pruned transform of half-length L = N/2 is supported
 bool fft_supported(int L);
@@ -33,5 +45,10 @@ cudaError_t launch_z_inv_prod(cudaStream_t st, int L, const cx<T>* in, T* phys, 
                               unsigned long long* umax2, Twiddles<T> tw);
 template <typename T>
 cudaError_t launch_z_fwd(cudaStream_t st, int L, const T* phys, cx<T>* out, long MM, long batch, Twiddles<T> tw);
+// fused a3+a4 (kernels_zfused.cuh): in [batch][3][MM][L] -> out [batch][6][MM][L]; persistent grid sized from
+// the SM count and the achievable CTAs per SM.
+template <typename T>
+cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
+                           unsigned long long* umax2, Twiddles<T> tw);
 
 }  // namespace ns

@@ -48,6 +48,18 @@ def pass_bytes_per_step(N: int, batch: int = 1, complex_bytes: int = 16) -> dict
     return out
 
 
+def fused_z_bytes(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
+    """Bytes the fused a3+a4 kernel must move per RHS: read 3 A2 (u_hat lines), write 6 A2 (B_hat lines)."""
+    _, _, A2, _ = sizes(N, complex_bytes)
+    return 9 * A2 * batch
+
+
+def actual_step_bytes(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
+    """Bytes per RK3 step of the pass structure actually built (a3+a4 fused)."""
+    per = pass_bytes_per_step(N, batch, complex_bytes)
+    return sum(per.values()) - per["a3_z_inv_prod"] - per["a4_z_fwd"] + 3 * fused_z_bytes(N, batch, complex_bytes)
+
+
 def step_bytes(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
     return sum(pass_bytes_per_step(N, batch, complex_bytes).values())
 
