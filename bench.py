@@ -277,12 +277,12 @@ def main():
                           "gbs": gbs, "frac": gbs / peak, "share_of_step": ms / (ms_per_step * args.steps), **extra}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_launch"] * kernels[k]["launches"])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # dram bytes per launch from the committed ncu --set full captures
     if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(f"{args.workload}_{args.dtype}", {}).get(dom)
-        except Exception:
-            traffic = None
+        for ln in open(tpath).read().splitlines()[1:]:
+            f = ln.split(",", 3)
+            if len(f) >= 3 and f[0] == f"{args.workload}_{args.dtype}" and f[1] == dom:
+                traffic = float(f[2])
     model_bytes = roofline.step_bytes(N, batch, cbytes)
     roof = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
             "frac": kernels[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
