@@ -21,11 +21,13 @@
 // Parity pins (tests/test_oracle_pins.py): P0 FFT vs O(n^2) DFT and numpy; P1 RHS vs O(N^6) direct
 // convolution; P2 Taylor-Green / ABC project to zero; P3 RK3 decay closed form; P4 energy identity;
 // P5 div-free; P6 Galilean shift; P7 padding independence; P8 spectrum/Parseval; P9 structure
-// function identity; P10 temporal order 3; P11 hyperviscous single mode.
+// function identity; P10 temporal order 3; P11 hyperviscous single mode; P12 orc_rhs_at_modes (direct
+// truncated convolution at sampled wavenumbers) vs the step-by-step RHS and vs the test's own O(N^6) sum.
 // "parity unpinned" against the authors' code (the paper gives no formula): the readings A3
 // (Nyquist planes zero), A5 (form of Q_k), A6 (constants), A10 (CFL formula), A14 (energy-spectrum
 // binning), A15 (structure function) -- they are pinned for self-consistency only.
 
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstdint>
@@ -292,6 +294,87 @@ void orc_rhs_parts(int N, int M, double nu, double eps, double s, double m_cut, 
                    const double* u_hat, double* b_hat, double* n_hat, double* r_hat, double* umax) {
     Params p{nu, eps, s, m_cut, q_exp, q_sharp};
     rhs_parts(N, M, p, (const cplx*)u_hat, (cplx*)b_hat, (cplx*)n_hat, (cplx*)r_hat, umax);
+}
+
+// The plain definition the pseudo-spectral evaluation reaches exactly (up to rounding order): with exact
+// dealiasing (reading A3/A12) the truncated transform of the pointwise product is the Galerkin-truncated
+// convolution sum  B_hat_ij(k) = sum_{p+q=k; p,q in K_N} u_hat_i(p) u_hat_j(q)  (eq. 2.5, PAPER.md:L124-126:
+// F[u (x) u]_k restricted to the retained modes, Algorithm 2 steps 1-5).  Evaluated
+// directly, O(N^3) per requested wavenumber, for sampled-output parity at sizes where rhs_parts needs
+// too much memory.  modes: [nmodes][3] stored indices (ix, iy, iz), iz <= N/2.  r_out: [nmodes][3] complex.
+// The field meant by a half spectrum is the real part of its synthesis, i.e. the kz = 0 plane enters
+// through its Hermitian part (same definition as to_physical above).
+void orc_rhs_at_modes(int N, double nu, double eps, double s, double m_cut, double q_exp, int q_sharp,
+                      const double* u_hat, int nmodes, const int* modes, double* r_out) {
+    Params prm{nu, eps, s, m_cut, q_exp, q_sharp};
+    const int Hs = N / 2 + 1, K = N / 2 - 1, W = 2 * K + 1;  // wavenumbers -K..K per axis
+    const size_t ns = (size_t)N * N * Hs, nf = (size_t)W * W * W;
+    const cplx* uh = (const cplx*)u_hat;
+    // full spectrum F[c][kx+K][ky+K][kz+K]
+    std::vector<cplx> F(3 * nf);
+    auto stored = [&](int c, int kx, int ky, int kz) {  // kz >= 0
+        return uh[c * ns + ((size_t)wrap(kx, N) * N + wrap(ky, N)) * Hs + kz];
+    };
+    for (int c = 0; c < 3; ++c)
+#pragma omp parallel for schedule(static)
+        for (int kx = -K; kx <= K; ++kx)
+            for (int ky = -K; ky <= K; ++ky)
+                for (int kz = -K; kz <= K; ++kz) {
+                    cplx v;
+                    if (kz > 0) v = stored(c, kx, ky, kz);
+                    else if (kz < 0) v = std::conj(stored(c, -kx, -ky, -kz));
+                    else v = 0.5 * (stored(c, kx, ky, 0) + std::conj(stored(c, -kx, -ky, 0)));
+                    F[c * nf + ((size_t)(kx + K) * W + (ky + K)) * W + (kz + K)] = v;
+                }
+    static const int pi_[6] = {0, 0, 0, 1, 1, 2}, pj_[6] = {0, 1, 2, 1, 2, 2};
+    static const int sym[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
+    for (int m = 0; m < nmodes; ++m) {
+        const int ix = modes[3 * m], iy = modes[3 * m + 1], iz = modes[3 * m + 2];
+        cplx* out = (cplx*)r_out + 3 * m;
+        out[0] = out[1] = out[2] = cplx(0.0, 0.0);
+        if (nyquist(ix, N) || nyquist(iy, N) || nyquist(iz, N)) continue;
+        const int k[3] = {wavenumber(ix, N), wavenumber(iy, N), iz};
+        if (k[0] == 0 && k[1] == 0 && k[2] == 0) continue;  // reading A8
+        // p ranges over K_N with q = k - p in K_N as well
+        const int lo[3] = {std::max(-K, k[0] - K), std::max(-K, k[1] - K), std::max(-K, k[2] - K)};
+        const int hi[3] = {std::min(K, k[0] + K), std::min(K, k[1] + K), std::min(K, k[2] + K)};
+        long double accr[6] = {0, 0, 0, 0, 0, 0}, acci[6] = {0, 0, 0, 0, 0, 0};
+#pragma omp parallel
+        {
+            long double lr[6] = {0, 0, 0, 0, 0, 0}, li[6] = {0, 0, 0, 0, 0, 0};
+#pragma omp for schedule(static) collapse(2)
+            for (int px = lo[0]; px <= hi[0]; ++px)
+                for (int py = lo[1]; py <= hi[1]; ++py) {
+                    cplx row[6] = {0, 0, 0, 0, 0, 0};
+                    const size_t op = ((size_t)(px + K) * W + (py + K)) * W + K;
+                    const size_t oq = ((size_t)(k[0] - px + K) * W + (k[1] - py + K)) * W + K;
+                    for (int pz = lo[2]; pz <= hi[2]; ++pz) {
+                        cplx up[3], uq[3];
+                        for (int c = 0; c < 3; ++c) {
+                            up[c] = F[c * nf + op + pz];
+                            uq[c] = F[c * nf + oq + (k[2] - pz)];
+                        }
+                        for (int t = 0; t < 6; ++t) row[t] += up[pi_[t]] * uq[pj_[t]];
+                    }
+                    for (int t = 0; t < 6; ++t) { lr[t] += row[t].real(); li[t] += row[t].imag(); }
+                }
+#pragma omp critical(orc_modes_acc)
+            for (int t = 0; t < 6; ++t) { accr[t] += lr[t]; acci[t] += li[t]; }
+        }
+        cplx Bh[6];
+        for (int t = 0; t < 6; ++t) Bh[t] = cplx((double)accr[t], (double)acci[t]);
+        const double kd[3] = {(double)k[0], (double)k[1], (double)k[2]};
+        const double k2 = kd[0] * kd[0] + kd[1] * kd[1] + kd[2] * kd[2];
+        cplx b[3];
+        for (int i = 0; i < 3; ++i) {
+            cplx acc(0.0, 0.0);
+            for (int j = 0; j < 3; ++j) acc += kd[j] * Bh[sym[i][j]];
+            b[i] = cplx(0.0, -1.0) * acc;
+        }
+        const cplx kb = kd[0] * b[0] + kd[1] * b[1] + kd[2] * b[2];
+        const double d = dissipation(prm, N, k2);
+        for (int i = 0; i < 3; ++i) out[i] = b[i] - kd[i] * kb / k2 - d * stored(i, k[0], k[1], k[2]);
+    }
 }
 
 // One SSP-RK3 step (eq. 2.6), dissipation explicit inside R (reading A9).

@@ -28,6 +28,7 @@ def _load():
     lib.orc_dissipation.argtypes = [i, d, d, d, d, d, i, d]
     lib.orc_dissipation.restype = d
     lib.orc_rhs_parts.argtypes = [i, i, d, d, d, d, d, i, p, p, p, p, p]
+    lib.orc_rhs_at_modes.argtypes = [i, d, d, d, d, d, i, p, i, p, p]
     lib.orc_step.argtypes = [i, i, d, d, d, d, d, i, p, d]
     lib.orc_set_initial.argtypes = [i, p, p]
     lib.orc_get_fields.argtypes = [i, p, p]
@@ -108,6 +109,17 @@ def rhs_parts(N, params: Params, u_hat, M=None):
 
 def rhs(N, params: Params, u_hat, M=None):
     return rhs_parts(N, params, u_hat, M)["r"]
+
+
+def rhs_at_modes(N, params: Params, u_hat, modes):
+    """R_hat at the stored indices modes[n] = (ix, iy, iz) by the direct truncated convolution sum; returns [n][3]."""
+    u_hat = _c128(u_hat)
+    assert u_hat.shape == spectral_shape(N)
+    modes = np.ascontiguousarray(modes, dtype=np.int32)
+    assert modes.ndim == 2 and modes.shape[1] == 3
+    out = np.empty((modes.shape[0], 3), dtype=np.complex128)
+    _lib.orc_rhs_at_modes(N, *params.args(), _ptr(u_hat), modes.shape[0], _ptr(modes), _ptr(out))
+    return out
 
 
 def step(N, params: Params, u_hat, dt, M=None):

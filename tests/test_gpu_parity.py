@@ -182,6 +182,96 @@ def test_step_cfl_per_sample_and_t_end(ns, oracle):
     assert np.isnan(s.time(B))
 
 
+# ------------------------------------------------------------- full BASELINE sizes, sampled outputs
+def _sample_modes(N, n, seed):
+    rng = np.random.default_rng(seed)
+    K = N // 2 - 1
+    lowk = np.stack([rng.integers(-4, 5, n // 2) % N, rng.integers(-4, 5, n // 2) % N, rng.integers(0, 5, n // 2)], axis=1)
+    anyk = np.stack([rng.integers(0, N, n - n // 2), rng.integers(0, N, n - n // 2), rng.integers(0, N // 2, n - n // 2)], axis=1)
+    fixed = np.array([(1, 0, 0), (0, 0, 1), (K, K, K), (N - K, 3, K), (5, N - K, 0), (N // 2, 2, 2), (0, 0, 0)])
+    return np.concatenate([lowk, anyk, fixed]).astype(np.int32)
+
+
+@pytest.mark.parametrize("workload", ["N256", "c5_N512"])
+def test_full_size_sampled_rhs_and_step(ns, oracle, workload):
+    """BASELINE.json sizes 256^3 (L = 128 kernels) and 512^3 (L = 256 kernels, configs[4] input), same launch
+    configuration as bench.py: ns_rhs at sampled wavenumbers against the oracle's direct truncated convolution
+    (orc_rhs_at_modes), the invariants P4/P5 on the whole array, and the fused RK3 step against the same step
+    assembled on the host from ns_rhs evaluations (eq. 2.6)."""
+    if workload == "N256":
+        N, nm = 256, 24
+        u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    else:
+        N, nm = 512, 10
+        u = inputs.gaussian_k53(N, seed=5)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    del u
+    uh = s.get_spectral()[0]
+    r = s.rhs()[0]
+    rmax = np.abs(r).max()
+    modes = _sample_modes(N, nm, N)
+    want = oracle.rhs_at_modes(N, oracle.Params(**kw), uh, modes)
+    got = np.stack([r[:, ix, iy, iz] for ix, iy, iz in modes])
+    assert np.abs(want).max() > 1e-3 * rmax
+    assert np.abs(got - want).max() < 1e-12 * rmax, np.abs(got - want).max() / rmax
+    # P5 / masks / P4 on the whole output
+    k = np.fft.fftfreq(N, 1.0 / N)
+    div = k[:, None, None] * r[0] + k[None, :, None] * r[1] + np.arange(N // 2 + 1.0)[None, None, :] * r[2]
+    assert np.abs(div).max() < 1e-12 * rmax * N
+    del div
+    assert np.all(r[:, N // 2] == 0) and np.all(r[:, :, N // 2] == 0) and np.all(r[:, :, :, N // 2] == 0)
+    w = np.full(N // 2 + 1, 2.0)
+    w[0] = 1.0
+    s_nl = ns.Solver(N) if N <= 256 else None      # inviscid RHS for the energy identity (memory: only at 256)
+    if s_nl is not None:
+        s_nl.set_spectral(uh[None])
+        rn = s_nl.rhs()[0]
+        assert abs(np.sum(w * np.real(np.conj(uh) * rn))) < 1e-12 * np.sum(w * np.abs(uh) * np.abs(rn))
+        del rn, s_nl
+    # fused RK3 step == eq. 2.6 assembled from ns_rhs (same kernels in mode 0)
+    dt = 0.2 * (2 * np.pi / N) / s.max_velocity()[0]
+    u1 = uh + dt * r
+    s.set_spectral(u1[None])
+    u2 = 0.75 * uh + 0.25 * u1 + 0.25 * dt * s.rhs()[0]
+    del u1
+    s.set_spectral(u2[None])
+    un = uh / 3.0 + (2.0 / 3.0) * u2 + (2.0 / 3.0) * dt * s.rhs()[0]
+    del u2
+    s.set_spectral(uh[None])
+    dts = s.step_cfl(0.2, 1e9)
+    assert abs(dts[0] - dt) < 1e-13 * dt
+    assert rel(s.get_spectral()[0], un) < 1e-14
+
+
+def test_config4_ensemble_two_samples(ns, oracle):
+    """BASELINE.json configs[3]: 32 x 128^3 shear-layer ensemble in one launch; samples 0 and 31 against the oracle
+    (1 RHS + 1 CFL step, oracle replays the GPU's dt), spectra and structure functions of those samples."""
+    N, B = 128, 32
+    us = inputs.shear_layer_ensemble(N, B, seed0=1000)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, batch=B, **kw)
+    s.set_initial(us)
+    p = oracle.Params(**kw)
+    u0 = s.get_spectral()
+    r0 = s.rhs()
+    dts = s.step_cfl(0.2, 1.0)
+    got = s.get_spectral()
+    E = s.energy_spectrum(N)
+    S = s.structure_function()
+    for i in (0, 31):
+        uh = oracle.set_initial(N, us[i])
+        assert rel(u0[i], uh) < 1e-13
+        assert rel(r0[i], oracle.rhs(N, p, u0[i])) < TOL_RHS_F64
+        assert abs(dts[i] - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, u0[i])) < 1e-12 * dts[i]
+        un = oracle.step(N, p, u0[i], dts[i])
+        assert rel(got[i], un) < TOL_STEPS_F64
+        assert np.abs(E[i] - oracle.energy_spectrum(N, un, N)).max() < 1e-13
+        assert np.abs(S[i] / oracle.structure_function(N, un) - 1).max() < 1e-10
+    assert len(set(np.round(dts, 12))) > 1          # distinct seeds -> distinct steps
+
+
 # ---------------------------------------------------------------------- invariants run on the GPU path
 def test_gpu_invariants(ns):
     N = 32

@@ -346,6 +346,37 @@ def test_p11_hyperviscous_single_mode(oracle, s):
     assert oracle.dissipation(N, oracle.Params(eps=eps, s=s, q_sharp=1), 36.0) == pytest.approx(eps / N ** (2 * s - 1) * kk ** (2 * s), rel=1e-15)
 
 
+# ------------------------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("N", [6, 8])
+def test_p12_rhs_at_modes_vs_direct_convolution(oracle, N):
+    """orc_rhs_at_modes (used for sampled parity at 256^3 / 512^3) against the test's own O(N^6) sum, every mode."""
+    uh = full_state(oracle, N, 40 + N)
+    modes = np.array([(ix, iy, iz) for ix in range(N) for iy in range(N) for iz in range(N // 2 + 1)], dtype=np.int32)
+    got = oracle.rhs_at_modes(N, oracle.Params(), uh, modes)
+    want = direct_convolution_rhs(N, uh)
+    assert rel(got.T.reshape(want.shape), want) < 1e-13
+    nyq = (modes[:, 0] == N // 2) | (modes[:, 1] == N // 2) | (modes[:, 2] == N // 2)
+    assert np.all(got[nyq] == 0) and np.all(got[0] == 0)
+
+
+@pytest.mark.parametrize("N,s", [(12, 1.0), (32, 1.0), (32, 1.5)])
+def test_p12_rhs_at_modes_vs_stepwise_oracle(oracle, N, s):
+    """... and against the step-by-step pseudo-spectral RHS with dissipation, on sampled modes incl. the box corners."""
+    uh = full_state(oracle, N, 60 + N)
+    p = oracle.Params(nu=0.01, eps=0.05, s=s)
+    r = oracle.rhs(N, p, uh)
+    rng = np.random.default_rng(N)
+    K = N // 2 - 1
+    modes = np.concatenate([
+        np.stack([rng.integers(0, N, 40), rng.integers(0, N, 40), rng.integers(0, N // 2 + 1, 40)], axis=1),
+        np.array([(K, K, K), (N - K, N - K, K), (K, N - K, 0), (0, 0, 1), (1, 0, 0), (0, 0, 0), (N // 2, 1, 1), (1, 1, N // 2)]),
+    ]).astype(np.int32)
+    got = oracle.rhs_at_modes(N, p, uh, modes)
+    want = np.stack([r[:, ix, iy, iz] for ix, iy, iz in modes])
+    assert np.abs(got - want).max() < 1e-13 * np.abs(r).max()
+    assert np.linalg.norm(want) > 1e-3
+
+
 def test_max_velocity_and_padding(oracle):
     N = 8
     uh = oracle.set_initial(N, inputs.taylor_green_2d(N))
