@@ -257,20 +257,23 @@ def main():
 
     # ---- roofline of the dominant kernel and of the whole step (fixed model)
     peak, peak_src = measured_peaks()
-    per_step = roofline.pass_bytes_per_step(N, batch, cbytes)
-    fused_z = prof["a4_z_fwd"][1] == 0   # a3 and a4 run as ONE kernel (the M^3 products never reach HBM)
+    per_step = roofline.pass_bytes_per_step(N, batch, cbytes)        # fixed model
+    built = roofline.built_pass_bytes_per_step(N, batch, cbytes)     # what the built kernels must move
+    prof_label = {"a1_col_inv_x": "a1_col_inv_x", "a2_col_inv_y": "a2_col_inv_y", "a3_z_inv_prod": "a3a4_z_fused",
+                  "a5_col_fwd_y": "a5_col_fwd_y", "a6_col_fwd_x": "a6_col_fwd_x", "a7_spectral": "a7_spectral"}
     kernels = {}
-    for name in roofline.PASS_NAMES:
+    for name, label in prof_label.items():
         ms, cnt = prof[name]
         if not cnt:
             continue
-        nbytes, label, extra = per_step[name], name, {}
-        if fused_z and name == "a3_z_inv_prod":
-            # what the fused kernel itself must move: read 3 A2, write 6 A2; the fixed model charges a3 + a4
-            label = "a3a4_z_fused"
-            nbytes = roofline.fused_z_bytes(N, batch, cbytes) * 3
+        nbytes, extra = built[label], {}
+        if label == "a3a4_z_fused":
+            # the fixed model charges a3 + a4 separately (six M^3 products written and read back)
             model = per_step["a3_z_inv_prod"] + per_step["a4_z_fwd"]
-            extra = {"model_bytes_per_launch_a3_plus_a4": model * args.steps / cnt,
+        else:
+            model = per_step[name]
+        if model != nbytes:
+            extra = {"model_bytes_per_launch": model * args.steps / cnt,
                      "model_gbs_equivalent": model * args.steps / (ms * 1e-3) / 1e9}
         gbs = nbytes * args.steps / (ms * 1e-3) / 1e9
         kernels[label] = {"ms_per_launch": ms / cnt, "launches": cnt, "alg_bytes_per_launch": nbytes * args.steps / cnt,
@@ -291,12 +294,12 @@ def main():
                  "frac_of_measured_peak": model_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                  "frac_of_nominal_8TBs": model_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
                  "t_model_ms_at_measured_peak": model_bytes / (peak * 1e9) * 1e3}
-    if fused_z:
-        actual = roofline.actual_step_bytes(N, batch, cbytes)
-        step_roof["actual_bytes_per_step"] = actual
-        step_roof["actual_frac_of_measured_peak"] = actual / (ms_per_step * 1e-3) / 1e9 / peak
-        step_roof["note"] = ("a3+a4 are fused (products never reach HBM): frac_* use the FIXED model bytes of SURVEY.md 8(d); "
-                             "actual_* use the bytes the built pass structure must move")
+    actual = roofline.actual_step_bytes(N, batch, cbytes)
+    step_roof["actual_bytes_per_step"] = actual
+    step_roof["actual_frac_of_measured_peak"] = actual / (ms_per_step * 1e-3) / 1e9 / peak
+    step_roof["note"] = ("a3+a4 are one kernel (products never reach HBM) and 5 trace-free flux components are transformed "
+                         "instead of 6: frac_* use the FIXED model bytes of SURVEY.md 8(d); actual_* use the bytes the "
+                         "built pass structure must move")
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D state, step, D2H state, every step
     e2e = None

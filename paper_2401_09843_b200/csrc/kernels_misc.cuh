@@ -8,14 +8,16 @@
 // public layout is not stored, so rows are 128-byte aligned).
 #pragma once
 #include "cx.cuh"
+#include "ns_internal.h"
 
 namespace ns {
 
 __device__ __forceinline__ int wavenum(int i, int N) { return i < N / 2 ? i : i - N; }
 
 // ------------------------------------------------------------------------------------------------
-// a7.  Bh: [b][6][N][N][H] unnormalised transforms of u_i u_j (order 11 12 13 22 23 33).
-//   b_i = -i k_j Bh_ij * scale;  Nl = b - k (k.b)/|k|^2;  R = Nl - d(|k|^2) * Us
+// a7.  Th: [b][5][N][N][H] unnormalised transforms of the trace-free flux T_ij = u_i u_j - delta_ij u_3^2
+//   (order 11 12 13 22 23, T33 = 0; kernels_z.cuh: the omitted part is a gradient, removed by the projection).
+//   b_i = -i k_j Th_ij * scale;  Nl = b - k (k.b)/|k|^2;  R = Nl - d(|k|^2) * Us
 //   mode 0: out = R
 //   mode 1: out = alpha*Un + beta*Us + gamma*dt_b*R   (Un may be NULL when alpha == 0)
 //           dt_b == 0 marks an inactive sample: out = Un (or Us when Un is NULL), bit exact.
@@ -45,16 +47,16 @@ spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* __restrict__ Us, cons
 #pragma unroll
     for (int c = 0; c < 3; ++c) u[c] = us[c * plane];
     if (!dead) {
-        const cx<T>* bp = Bh + b * 6 * plane + o;
+        const cx<T>* bp = Bh + b * NS_NFLUX * plane + o;
         const cx<T> B11 = ldg(bp), B12 = ldg(bp + plane), B13 = ldg(bp + 2 * plane), B22 = ldg(bp + 3 * plane),
-                    B23 = ldg(bp + 4 * plane), B33 = ldg(bp + 5 * plane);
+                    B23 = ldg(bp + 4 * plane);
         const T kx = (T)kxi, ky = (T)kyi, kz = (T)iz;
         // -i z = (z.y, -z.x)
         cx<T> bb[3];
         {
             const cx<T> z0 = mk<T>(kx * B11.x + ky * B12.x + kz * B13.x, kx * B11.y + ky * B12.y + kz * B13.y);
             const cx<T> z1 = mk<T>(kx * B12.x + ky * B22.x + kz * B23.x, kx * B12.y + ky * B22.y + kz * B23.y);
-            const cx<T> z2 = mk<T>(kx * B13.x + ky * B23.x + kz * B33.x, kx * B13.y + ky * B23.y + kz * B33.y);
+            const cx<T> z2 = mk<T>(kx * B13.x + ky * B23.x, kx * B13.y + ky * B23.y);
             bb[0] = mk<T>(scale * z0.y, -scale * z0.x);
             bb[1] = mk<T>(scale * z1.y, -scale * z1.x);
             bb[2] = mk<T>(scale * z2.y, -scale * z2.x);

@@ -1,8 +1,8 @@
 // kernels_zfused.cuh -- steps a3 + a4 of SURVEY.md section 8(a) in ONE kernel (the "beyond the model"
-// fusion of SURVEY.md section 7 item 5(i)): per (px,py) line, pad + inverse c2r along z, the six
+// fusion of SURVEY.md section 7 item 5(i)): per (px,py) line, pad + inverse c2r along z, the flux
 // products u_i u_j (Algorithm 2 steps 2-3), max|u|^2, forward r2c + truncate
 // (steps 4-5).  The M^3 physical arrays never touch HBM: the kernel reads 3 half
-// spectra lines and writes 6.
+// spectra lines and writes 5.
 //
 // Persistent CTAs; the input lines of the NEXT tile are fetched by the TMA bulk-copy engine
 // (cp.async.bulk, completion on an mbarrier) into shared memory while the current tile is being
@@ -51,7 +51,7 @@ __device__ __forceinline__ cx<T> prune3(cx<T> a, cx<T> c, int q, int n, const Tw
     return cmul(z, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
 }
 
-// in [batch][3][MM][L] complex -> out [batch][6][MM][L] complex (unnormalised transforms of the products)
+// in [batch][3][MM][L] complex -> out [batch][5][MM][L] complex (unnormalised transforms of the flux components)
 template <typename T, int L, int R1, int R2, int LPB, int MINB, bool SEPCMB>
 __global__ void __launch_bounds__(3 * ZP<R1, R2>::value* LPB, MINB)
 z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, long total_tiles,
@@ -178,19 +178,19 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
             for (int o = 16; o > 0; o >>= 1) lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
             if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax2 + b, (double)lmax);
         }
-        // ---------------- forward pairs (11,22) (33,12) (13,23)
-        cx<T>* Op = out + (b * 6 * MM + pp) * L;
+        // ---------------- forward pairs (T11,T22) (T12,T13) (T23,-), see kernels_z.cuh
+        cx<T>* Op = out + (b * 5 * MM + pp) * L;
 #pragma unroll 1
         for (int pair = 0; pair < 3; ++pair) {
-            const int ca = pair == 0 ? 0 : (pair == 1 ? 5 : 2);
-            const int cb = pair == 0 ? 3 : (pair == 1 ? 1 : 4);
+            const int ca = pair == 0 ? 0 : (pair == 1 ? 1 : 4);
+            const int cb = pair == 0 ? 3 : 2;  // unused for pair 2
             if (i < R1) {
                 cx<T> x[R2];
 #pragma unroll
                 for (int r2 = 0; r2 < R2; ++r2) {
                     const cx<T> w = u12[brev<R2>(r2)];
                     const T w3 = u3r[brev<R2>(r2)];
-                    x[r2] = pair == 0 ? mk<T>(w.x * w.x, w.y * w.y) : (pair == 1 ? mk<T>(w3 * w3, w.x * w.y) : mk<T>(w.x * w3, w.y * w3));
+                    x[r2] = pair == 0 ? mk<T>(w.x * w.x - w3 * w3, w.y * w.y - w3 * w3) : (pair == 1 ? mk<T>(w.x * w.y, w.x * w3) : mk<T>(w.y * w3, 0));
                 }
                 fft_reg<R2, -1, T>(x);
                 // pair 0: this thread overwrites the row only it has read in stage B above; later pairs: barrier above
@@ -225,7 +225,7 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
                     const cx<T> An = f0 + S;
                     if (n == 0) {
                         Op[ca * cs] = mk<T>(An.x, 0);
-                        Op[cb * cs] = mk<T>(An.y, 0);
+                        if (pair < 2) Op[cb * cs] = mk<T>(An.y, 0);
                     } else {
                         const cx<T> Cn = mk<T>(f0.x - (T)0.5 * S.x - h3 * D.y, f0.y - (T)0.5 * S.y + h3 * D.x);
                         const int m = L - n;
@@ -234,10 +234,10 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
                         const cx<T> Am = f0m + Sm;
                         const cx<T> Cm = mk<T>(f0m.x - (T)0.5 * Sm.x - h3 * Dm.y, f0m.y - (T)0.5 * Sm.y + h3 * Dm.x);
                         Op[ca * cs + n] = mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y));
-                        Op[cb * cs + n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
+                        if (pair < 2) Op[cb * cs + n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
                         if (m != n) {
                             Op[ca * cs + m] = mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y));
-                            Op[cb * cs + m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
+                            if (pair < 2) Op[cb * cs + m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
                         }
                     }
                 }

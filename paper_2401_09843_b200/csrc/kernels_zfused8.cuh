@@ -1,5 +1,5 @@
 // kernels_zfused8.cuh -- steps a3 + a4 of SURVEY.md section 8(a) in one kernel, warp-synchronous version
-// for the long lines (L = N/2 in {64, 128, 256}): per (px,py) line, pad + inverse c2r along z, the six
+// for the long lines (L = N/2 in {64, 128, 256}): per (px,py) line, pad + inverse c2r along z, the flux
 // products u_i u_j, max|u|^2, forward r2c + truncate (Algorithm 2 steps 1-5).
 // The M^3 physical arrays never touch HBM.
 //
@@ -118,7 +118,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// in [batch][3][MM][L] complex -> out [batch][6][MM][L] complex (unnormalised transforms of the products)
+// in [batch][3][MM][L] complex -> out [batch][5][MM][L] complex (unnormalised transforms of the flux components)
 template <typename T, int L, int LPB, int MINB>
 __global__ void __launch_bounds__(3 * (L / 8) * LPB, MINB)
 z_fused8_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, long total_lines,
@@ -211,17 +211,17 @@ z_fused8_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, 
             for (int o = 16; o > 0; o >>= 1) lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
             if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax2 + b, (double)lmax);
         }
-        // ---------------- forward pairs (11,22) (33,12) (13,23)
-        cx<T>* Op = out + (b * 6 * MM + pp) * L;
+        // ---------------- forward pairs (T11,T22) (T12,T13) (T23,-), see kernels_z.cuh
+        cx<T>* Op = out + (b * 5 * MM + pp) * L;
 #pragma unroll 1
         for (int pair = 0; pair < 3; ++pair) {
-            const int ca = pair == 0 ? 0 : (pair == 1 ? 5 : 2);
-            const int cb = pair == 0 ? 3 : (pair == 1 ? 1 : 4);
+            const int ca = pair == 0 ? 0 : (pair == 1 ? 1 : 4);
+            const int cb = pair == 0 ? 3 : 2;  // unused for pair 2
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
                 const cx<T> w = u12[k];
                 const T w3 = u3r[k];
-                v[k] = pair == 0 ? mk<T>(w.x * w.x, w.y * w.y) : (pair == 1 ? mk<T>(w3 * w3, w.x * w.y) : mk<T>(w.x * w3, w.y * w3));
+                v[k] = pair == 0 ? mk<T>(w.x * w.x - w3 * w3, w.y * w.y - w3 * w3) : (pair == 1 ? mk<T>(w.x * w.y, w.x * w3) : mk<T>(w.y * w3, 0));
             }
             z8_forward<T, L>(v, S, t, tw);
             // F_q[n] W^{-qn} into this sub-transform's region, natural order
@@ -243,7 +243,7 @@ z_fused8_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, 
                     const cx<T> An = f0 + Sm_;
                     if (n == 0) {
                         Op[ca * cs] = mk<T>(An.x, 0);
-                        Op[cb * cs] = mk<T>(An.y, 0);
+                        if (pair < 2) Op[cb * cs] = mk<T>(An.y, 0);
                     } else {
                         const cx<T> Cn = mk<T>(f0.x - (T)0.5 * Sm_.x - h3 * D.y, f0.y - (T)0.5 * Sm_.y + h3 * D.x);
                         const int m = L - n;
@@ -252,10 +252,10 @@ z_fused8_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, 
                         const cx<T> Am = f0m + Sm;
                         const cx<T> Cm = mk<T>(f0m.x - (T)0.5 * Sm.x - h3 * Dm.y, f0m.y - (T)0.5 * Sm.y + h3 * Dm.x);
                         Op[ca * cs + n] = mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y));
-                        Op[cb * cs + n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
+                        if (pair < 2) Op[cb * cs + n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
                         if (m != n) {
                             Op[ca * cs + m] = mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y));
-                            Op[cb * cs + m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
+                            if (pair < 2) Op[cb * cs + m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
                         }
                     }
                 }

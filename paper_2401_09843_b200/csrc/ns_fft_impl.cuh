@@ -25,8 +25,6 @@ template <int L> struct Cfg {
         constexpr int tt = tile_cols<T>() * P;
         return tt >= 128 ? 1 : 128 / tt;
     }
-    // lines per block for the z kernels: aim at 192 threads
-    static constexpr int lpb() { return (3 * P) >= 192 ? 1 : 192 / (3 * P); }
     // lines per block for the fused z kernel: ~96 threads for the long lines (shared memory bound), 192 otherwise
     static constexpr int lpbf() { return L >= 128 ? 2 : 192 / (3 * P); }
     // target CTAs per SM of the fused z kernel (bounds its registers)
@@ -62,33 +60,6 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     if (e != cudaSuccess) return e;
     const long blocks = (g.total_tiles + TPB - 1) / TPB;
     k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, scale, tw);
-    return cudaGetLastError();
-}
-
-template <typename T, int L>
-static cudaError_t z_inv_L(cudaStream_t st, const cx<T>* in, T* phys, long MM, long batch, unsigned long long* umax2,
-                           Twiddles<T> tw) {
-    using C = Cfg<L>;
-    constexpr int LPB = C::lpb();
-    auto k = z_inv_prod_kernel<T, L, C::R1, C::R2, LPB>;
-    const size_t smem = (size_t)2 * LPB * 3 * C::R1 * (C::R2 + 1) * sizeof(cx<T>);
-    cudaError_t e = set_smem(k, smem);
-    if (e != cudaSuccess) return e;
-    const long total = MM * batch;
-    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(in, phys, MM, total, umax2, tw);
-    return cudaGetLastError();
-}
-
-template <typename T, int L>
-static cudaError_t z_fwd_L(cudaStream_t st, const T* phys, cx<T>* out, long MM, long batch, Twiddles<T> tw) {
-    using C = Cfg<L>;
-    constexpr int LPB = C::lpb();
-    auto k = z_fwd_kernel<T, L, C::R1, C::R2, LPB>;
-    const size_t smem = (size_t)LPB * (3 * C::R1 * (C::R2 + 1) + 3 * L) * sizeof(cx<T>);
-    cudaError_t e = set_smem(k, smem);
-    if (e != cudaSuccess) return e;
-    const long total = MM * batch;
-    k<<<(unsigned)((total + LPB - 1) / LPB), 3 * C::P * LPB, smem, st>>>(phys, out, MM, total, tw);
     return cudaGetLastError();
 }
 
@@ -199,21 +170,6 @@ cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
 }
 
 template <typename T>
-cudaError_t launch_z_inv_prod(cudaStream_t st, int L, const cx<T>* in, T* phys, long MM, long batch,
-                              unsigned long long* umax2, Twiddles<T> tw) {
-#define CALL(LL) z_inv_L<T, LL>(st, in, phys, MM, batch, umax2, tw)
-    NS_DISPATCH_L(L, CALL)
-#undef CALL
-}
-
-template <typename T>
-cudaError_t launch_z_fwd(cudaStream_t st, int L, const T* phys, cx<T>* out, long MM, long batch, Twiddles<T> tw) {
-#define CALL(LL) z_fwd_L<T, LL>(st, phys, out, MM, batch, tw)
-    NS_DISPATCH_L(L, CALL)
-#undef CALL
-}
-
-template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw) {
     if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
@@ -229,9 +185,6 @@ cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
                                            long, Twiddles<T>);                                                     \
     template cudaError_t launch_col_fwd<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, T, Twiddles<T>);                                                  \
-    template cudaError_t launch_z_inv_prod<T>(cudaStream_t, int, const cx<T>*, T*, long, long, unsigned long long*, \
-                                              Twiddles<T>);                                                        \
-    template cudaError_t launch_z_fwd<T>(cudaStream_t, int, const T*, cx<T>*, long, long, Twiddles<T>);                \
     template cudaError_t launch_z_fused<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, unsigned long long*,   \
                                            Twiddles<T>);
 

@@ -7,6 +7,9 @@
 
 namespace ns {
 
+// number of flux components carried through a4-a7: the five trace-free combinations of kernels_z.cuh
+constexpr int NS_NFLUX = 5;
+
 // Twiddle tables, laid out so that the lanes of a warp read consecutive entries:
 //   twA[r1 * R2 + n2] = twB[n2 * R1 + r1] = exp(+2 pi i r1 n2 / L)      (inter-stage twiddles, L = R1 R2)
 //   w3a[n] = exp(+2 pi i n / (3L)),  w3b[n] = exp(+2 pi i 2n / (3L)),  n < L   (pruned radix-3 twiddles)
@@ -22,6 +25,9 @@ struct Twiddles {
     const cx<T>* z8B;
     const cx<T>* z8C;
 };
+// number of complex entries of the table block and its host-side construction (long double arguments);
+// make_twiddles() returns the views into a device copy of that block
+inline size_t twiddle_table_len(int L) { return (size_t)7 * L; }
 // register-stage split L = R1 x R2 used by the kernels (needed by the host to build twA / twB)
 void fft_split(int L, int* R1, int* R2);
 
@@ -39,14 +45,8 @@ cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
 template <typename T>
 cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw);
-// z passes.  in/out layouts documented in kernels_z.cuh.  umax2 may be NULL.
-template <typename T>
-cudaError_t launch_z_inv_prod(cudaStream_t st, int L, const cx<T>* in, T* phys, long MM, long batch,
-                              unsigned long long* umax2, Twiddles<T> tw);
-template <typename T>
-cudaError_t launch_z_fwd(cudaStream_t st, int L, const T* phys, cx<T>* out, long MM, long batch, Twiddles<T> tw);
-// fused a3+a4 (kernels_zfused.cuh): in [batch][3][MM][L] -> out [batch][6][MM][L]; persistent grid sized from
-// the SM count and the achievable CTAs per SM.
+// fused a3+a4 (kernels_zfused.cuh, kernels_zfused8.cuh): in [batch][3][MM][L] -> out [batch][NS_NFLUX][MM][L];
+// persistent grid sized from the SM count and the achievable CTAs per SM.  umax2 may be NULL.
 template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw);

@@ -12,6 +12,7 @@
 #include "../../include/ns.h"
 #include "kernels_misc.cuh"
 #include "ns_internal.h"
+#include "twiddles_host.h"
 
 using namespace ns;
 
@@ -110,8 +111,7 @@ public:
     unsigned char* arena = nullptr;
     size_t arena_bytes = 0;
     cx<T>*U = nullptr, *V = nullptr, *X = nullptr, *Y = nullptr, *Z = nullptr;
-    bool z_unfused = false;  // NS_Z_UNFUSED=1: run a3 and a4 as separate kernels (comparison path)
-    cx<T>*twA = nullptr, *twB = nullptr, *w3a = nullptr, *w3b = nullptr, *z8A = nullptr, *z8B = nullptr, *z8C = nullptr;
+    cx<T>* twbase = nullptr;  // twiddle-table block (twiddles_host.h)
     T* dtab = nullptr;
     double *dt_dev = nullptr, *t_dev = nullptr, *scal_dev = nullptr, *red_dev = nullptr;
     unsigned long long* umax2 = nullptr;
@@ -144,7 +144,7 @@ public:
         if (e__ != cudaSuccess) return cuda_fail(e__, name);   \
     } while (0)
 
-    Twiddles<T> tw() const { return Twiddles<T>{twA, twB, w3a, w3b, z8A, z8B, z8C}; }
+    Twiddles<T> tw() const { return make_twiddles<T>(twbase, L); }
     static unsigned blocks_for(long total, int threads) { return (unsigned)((total + threads - 1) / threads); }
 
     int init() {
@@ -152,12 +152,9 @@ public:
         nS = b * 3 * N * N * H;
         // Workspaces shared by all passes: X <- a1 out / a5 out / unpadded-FFT cube / R,
         // Y <- a2 out / a6 out (B_hat) / host staging, Z <- fused-z out.
-        const char* env = std::getenv("NS_Z_UNFUSED");
-        z_unfused = env && env[0] == '1';
-        nX = b * 6 * (size_t)M * N * H;                   // A1b; >= A1u (3 M N H), W (3 N^3), R (3 N^2 H)
-        if (z_unfused) nX = b * 3 * (size_t)M * M * M;    // six M^3 real products = 3 M^3 complex
-        nY = b * 3 * (size_t)M * M * H;                   // A2u; >= Bh (6 N^2 H), public / physical staging
-        nZ = b * 6 * (size_t)M * M * H;                   // A2b
+        nX = b * NS_NFLUX * (size_t)M * N * H;            // A1b; >= A1u (3 M N H), W (3 N^3 = 6 N^2 H), R (3 N^2 H)
+        nY = b * 3 * (size_t)M * M * H;                   // A2u; >= Bh (5 N^2 H), public / physical staging
+        nZ = b * NS_NFLUX * (size_t)M * M * H;            // A2b
         const size_t pub = b * 3 * (size_t)N * N * (H + 1);
         if (nY < pub) nY = pub;
         const size_t ndt = (size_t)3 * L * L + 1;
@@ -167,7 +164,7 @@ public:
         auto take = [&](size_t bytes) { size_t o = off; off += al(bytes); return o; };
         const size_t oU = take(nS * sizeof(cx<T>)), oV = take(nS * sizeof(cx<T>));
         const size_t oX = take(nX * sizeof(cx<T>)), oY = take(nY * sizeof(cx<T>)), oZ = take(nZ * sizeof(cx<T>));
-        const size_t otw = take(((size_t)6 * L + 32) * sizeof(cx<T>));
+        const size_t otw = take(twiddle_table_len(L) * sizeof(cx<T>));
         const size_t oD = take(ndt * sizeof(T));
         const size_t odt = take(b * sizeof(double)), ot = take(b * sizeof(double)), osc = take(b * sizeof(double));
         const size_t oum = take(b * sizeof(unsigned long long));
@@ -186,13 +183,7 @@ public:
         X = (cx<T>*)(arena + oX);
         Y = (cx<T>*)(arena + oY);
         Z = (cx<T>*)(arena + oZ);
-        twA = (cx<T>*)(arena + otw);
-        twB = twA + L;
-        w3a = twB + L;
-        w3b = w3a + L;
-        z8A = w3b + L;
-        z8B = z8A + L;
-        z8C = z8B + L;
+        twbase = (cx<T>*)(arena + otw);
         dtab = (T*)(arena + oD);
         dt_dev = (double*)(arena + odt);
         t_dev = (double*)(arena + ot);
@@ -200,40 +191,10 @@ public:
         umax2 = (unsigned long long*)(arena + oum);
         red_dev = (double*)(arena + ored);
 
-        // twiddle tables, evaluated in long double
-        const long double twopi = 6.283185307179586476925286766559005768L;
-        int R1 = 0, R2 = 0;
-        fft_split(L, &R1, &R2);
-        std::vector<cx<T>> htw((size_t)6 * L + 32);
-        auto root = [&](long num, long den) {
-            const long double a = twopi * (long double)(num % den) / (long double)den;
-            cx<T> w;
-            w.x = (T)cosl(a);
-            w.y = (T)sinl(a);
-            return w;
-        };
-        for (int r1 = 0; r1 < R1; ++r1)
-            for (int n2 = 0; n2 < R2; ++n2) {
-                htw[(size_t)r1 * R2 + n2] = root((long)r1 * n2, L);
-                htw[(size_t)L + (size_t)n2 * R1 + r1] = root((long)r1 * n2, L);
-            }
-        for (int n = 0; n < L; ++n) {
-            htw[(size_t)2 * L + n] = root(n, 3L * L);
-            htw[(size_t)3 * L + n] = root(2L * n, 3L * L);
-        }
-        if (L >= 64) {
-            const int G = L / 8, R3 = G / 8;
-            for (int k = 0; k < 8; ++k)
-                for (int t = 0; t < G; ++t) {
-                    htw[(size_t)4 * L + (size_t)k * G + t] = root((long)k * t, L);
-                    htw[(size_t)5 * L + (size_t)k * G + t] = root((long)(t / R3) * (R3 * k + t % R3), L);
-                }
-            for (int rA = 0; rA < 8; ++rA)
-                for (int tb = 0; tb < R3; ++tb) htw[(size_t)6 * L + (size_t)rA * R3 + tb] = root((long)rA * tb, G);
-        }
+        const std::vector<cx<T>> htw = build_twiddle_block<T>(L);
         std::vector<T> hd(ndt);
         for (size_t k2 = 0; k2 < ndt; ++k2) hd[k2] = (T)dissipation_rate(prm, N, (double)k2);
-        NS_CK(cudaMemcpyAsync(twA, htw.data(), htw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
+        NS_CK(cudaMemcpyAsync(twbase, htw.data(), htw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemcpyAsync(dtab, hd.data(), hd.size() * sizeof(T), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemsetAsync(t_dev, 0, b * sizeof(double), st));
         NS_CK(cudaMemsetAsync(dt_dev, 0, b * sizeof(double), st));
@@ -244,7 +205,7 @@ public:
     long long device_bytes() const override { return (long long)arena_bytes; }
 
     // ---------------------------------------------------------------- RHS transform pipeline a1..a6
-    // Uin (internal layout) -> Y = Bh [b][6][N][N][H] (unnormalised)
+    // Uin (internal layout) -> Y = Th [b][5][N][N][H] (unnormalised transforms of the trace-free flux)
     int transform(const cx<T>* Uin, bool want_umax, int upto = 6) {
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
@@ -257,27 +218,16 @@ public:
         if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
         ++launches;
         prof.tick(2, st);
-        if (!z_unfused) {
-            e = launch_z_fused<T>(st, L, Y, Z, (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
-            if (e != cudaSuccess) return cuda_fail(e, "a3+a4 z_fused");
-            ++launches;
-            if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
-        } else {
-            e = launch_z_inv_prod<T>(st, L, Y, reinterpret_cast<T*>(X), (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
-            if (e != cudaSuccess) return cuda_fail(e, "a3 z_inv_prod");
-            ++launches;
-            if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
-            prof.tick(3, st);
-            e = launch_z_fwd<T>(st, L, reinterpret_cast<const T*>(X), Z, (long)M * M, batch, tw());
-            if (e != cudaSuccess) return cuda_fail(e, "a4 z_fwd");
-            ++launches;
-        }
+        e = launch_z_fused<T>(st, L, Y, Z, (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
+        if (e != cudaSuccess) return cuda_fail(e, "a3+a4 z_fused");
+        ++launches;
+        if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
         prof.tick(4, st);
-        e = launch_col_fwd<T>(st, L, Z, X, H, (long)batch * 6 * M, H, H, MH, NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, L, Z, X, H, (long)batch * NS_NFLUX * M, H, H, MH, NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a5 col_fwd y");
         ++launches;
         prof.tick(5, st);
-        e = launch_col_fwd<T>(st, L, X, Y, NH, (long)batch * 6, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, L, X, Y, NH, (long)batch * NS_NFLUX, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a6 col_fwd x");
         ++launches;
         prof.tick(7, st);

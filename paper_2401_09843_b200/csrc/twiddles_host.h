@@ -1,0 +1,62 @@
+// twiddles_host.h -- host-side construction of the twiddle-table block described in ns_internal.h.
+// All roots are evaluated in long double from exactly reduced arguments and rounded once to T.
+#pragma once
+#include <cmath>
+#include <vector>
+
+#include "ns_internal.h"
+
+namespace ns {
+
+// Block layout (complex entries): twA [0,L) twB [L,2L) w3a [2L,3L) w3b [3L,4L) z8A [4L,5L) z8B [5L,6L)
+// z8C [6L,7L).
+template <typename T>
+inline std::vector<cx<T>> build_twiddle_block(int L) {
+    const long double twopi = 6.283185307179586476925286766559005768L;
+    int R1 = 0, R2 = 0;
+    fft_split(L, &R1, &R2);
+    std::vector<cx<T>> h(twiddle_table_len(L));
+    for (auto& e : h) { e.x = 0; e.y = 0; }
+    auto root = [&](long num, long den) {
+        const long double a = twopi * (long double)(num % den) / (long double)den;
+        cx<T> w;
+        w.x = (T)cosl(a);
+        w.y = (T)sinl(a);
+        return w;
+    };
+    for (int r1 = 0; r1 < R1; ++r1)
+        for (int n2 = 0; n2 < R2; ++n2) {
+            h[(size_t)r1 * R2 + n2] = root((long)r1 * n2, L);
+            h[(size_t)L + (size_t)n2 * R1 + r1] = root((long)r1 * n2, L);
+        }
+    for (int n = 0; n < L; ++n) {
+        h[(size_t)2 * L + n] = root(n, 3L * L);
+        h[(size_t)3 * L + n] = root(2L * n, 3L * L);
+    }
+    if (L >= 64) {
+        const int G = L / 8, R3 = G / 8;
+        for (int k = 0; k < 8; ++k)
+            for (int t = 0; t < G; ++t) {
+                h[(size_t)4 * L + (size_t)k * G + t] = root((long)k * t, L);
+                h[(size_t)5 * L + (size_t)k * G + t] = root((long)(t / R3) * (R3 * k + t % R3), L);
+            }
+        for (int rA = 0; rA < 8; ++rA)
+            for (int tb = 0; tb < R3; ++tb) h[(size_t)6 * L + (size_t)rA * R3 + tb] = root((long)rA * tb, G);
+    }
+    return h;
+}
+
+template <typename T>
+inline Twiddles<T> make_twiddles(const cx<T>* base, int L) {
+    Twiddles<T> t;
+    t.twA = base;
+    t.twB = base + L;
+    t.w3a = base + 2 * (size_t)L;
+    t.w3b = base + 3 * (size_t)L;
+    t.z8A = base + 4 * (size_t)L;
+    t.z8B = base + 5 * (size_t)L;
+    t.z8C = base + 6 * (size_t)L;
+    return t;
+}
+
+}  // namespace ns

@@ -48,16 +48,39 @@ def pass_bytes_per_step(N: int, batch: int = 1, complex_bytes: int = 16) -> dict
     return out
 
 
-def fused_z_bytes(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
-    """Bytes the fused a3+a4 kernel must move per RHS: read 3 A2 (u_hat lines), write 6 A2 (B_hat lines)."""
-    _, _, A2, _ = sizes(N, complex_bytes)
-    return 9 * A2 * batch
+NFLUX = 5  # flux components carried through a4-a7 by the built path (trace-free combinations, csrc/kernels_z.cuh)
+
+BUILT_PASS_NAMES = ["a1_col_inv_x", "a2_col_inv_y", "a3a4_z_fused", "a5_col_fwd_y", "a6_col_fwd_x", "a7_spectral"]
+
+
+def built_pass_bytes(N: int, batch: int = 1, complex_bytes: int = 16, stage: int = 1) -> dict:
+    """Bytes each kernel of the pass structure actually built must move for ONE RHS evaluation + stage update:
+    a3 and a4 are one kernel (the M^3 physical arrays never reach HBM) and only
+    the NFLUX = 5 trace-free flux components are transformed forward (item 5(iii)).  Spectral rows are stored
+    with H = N/2 entries (the zero kz = N/2 column is not stored), which the S term below ignores (< 0.4 %)."""
+    S, A1, A2, _ = sizes(N, complex_bytes)
+    b = {
+        "a1_col_inv_x": 3 * (S + A1),
+        "a2_col_inv_y": 3 * (A1 + A2),
+        "a3a4_z_fused": (3 + NFLUX) * A2,
+        "a5_col_fwd_y": NFLUX * (A2 + A1),
+        "a6_col_fwd_x": NFLUX * (A1 + S),
+        "a7_spectral": (NFLUX + 3 + 3 + (0 if stage == 1 else 3)) * S,
+    }
+    return {k: v * batch for k, v in b.items()}
+
+
+def built_pass_bytes_per_step(N: int, batch: int = 1, complex_bytes: int = 16) -> dict:
+    out = {k: 0 for k in BUILT_PASS_NAMES}
+    for stage in (1, 2, 3):
+        for k, v in built_pass_bytes(N, batch, complex_bytes, stage).items():
+            out[k] += v
+    return out
 
 
 def actual_step_bytes(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
-    """Bytes per RK3 step of the pass structure actually built (a3+a4 fused)."""
-    per = pass_bytes_per_step(N, batch, complex_bytes)
-    return sum(per.values()) - per["a3_z_inv_prod"] - per["a4_z_fwd"] + 3 * fused_z_bytes(N, batch, complex_bytes)
+    """Bytes per RK3 step of the pass structure actually built."""
+    return sum(built_pass_bytes_per_step(N, batch, complex_bytes).values())
 
 
 def step_bytes(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
