@@ -20,6 +20,7 @@
 #pragma once
 #include "cx.cuh"
 #include "ns_internal.h"
+#include "tmem.cuh"
 
 namespace ns {
 
@@ -189,6 +190,115 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
         }
         buf ^= 1;
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// forward, long lines (R1 = 16): same transform as col_fwd_kernel, but the partial results that have to
+// survive from one sub-transform q to the next (F_0 and G_1 = W^{-n} F_1, 16 complex per thread each) are
+// parked in tensor memory (tmem.cuh) instead of registers / shared memory.  That removes 64 registers per
+// thread and a third of the shared memory, which is what bounded the kernel at two CTAs (8 warps) per SM.
+// One tile per CTA; CTAs of 4 (fp64) or 8 (fp32) warps; warp w uses TMEM lanes 32 (w % 4), columns of set w / 4.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int L, int R2, int TC, int MINB>
+__global__ void __launch_bounds__(TC * 16, MINB)
+col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale, Twiddles<T> tw) {
+    constexpr int R1 = 16;
+    static_assert(R1 * R2 == L && R2 >= 2 && R2 <= 16, "two register stages, first of 16");
+    constexpr uint32_t C16 = tmem_cols16<T>();
+    constexpr uint32_t NCOLS = 128;   // (F0.x F0.y G1.x G1.y) x C16 columns per warp set, TC*16/128 warp sets
+    static_assert(4 * C16 * ((TC * 16 + 127) / 128) <= NCOLS, "TMEM columns");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* E = reinterpret_cast<cx<T>*>(smem_raw);  // [2][L][TC] exchange
+    __shared__ uint32_t tslot;
+
+    const int c = threadIdx.x % TC, i = threadIdx.x / TC;
+    const int warp = threadIdx.x / 32;
+    const long tile = blockIdx.x;
+    const long slab = tile / g.tiles_per_slab;
+    const int col0 = (int)(tile % g.tiles_per_slab) * TC;
+    const cx<T>* ip = in + slab * g.in_slab + col0 + c;
+    cx<T>* op = out + slab * g.out_slab + col0 + c;
+    constexpr size_t EBUF = (size_t)L * TC;
+
+    if (warp == 0) tmem_alloc(&tslot, NCOLS);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tb = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * 4 * C16;
+    const uint32_t tF0 = tb, tG1 = tb + 2 * C16;   // 16 complex each
+
+    int buf = 0;
+    cx<T> x[R2];
+#pragma unroll
+    for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(i + R1 * r2) * g.istride);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        {
+            fft_reg<R2, -1, T>(x);
+#pragma unroll
+            for (int n2 = 0; n2 < R2; ++n2) {
+                cx<T> v = x[brev<R2>(n2)];
+                if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
+                E[buf * EBUF + (size_t)(i * R2 + n2) * TC + c] = v;
+            }
+        }
+        // rows of the next sub-transform are fetched while this one goes through its second stage
+        if (q < 2) {
+#pragma unroll
+            for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)((q + 1) * L + i + R1 * r2) * g.istride);
+        }
+        __syncthreads();
+        cx<T> y[R1];
+        const int ii = i < R2 ? i : 0;   // threads beyond R2 (L = 128) redo column 0 and discard it
+#pragma unroll
+        for (int r1 = 0; r1 < R1; ++r1) y[r1] = E[buf * EBUF + (size_t)(r1 * R2 + ii) * TC + c];
+        fft_reg<R1, -1, T>(y);
+        constexpr int CH = tmem_cx_chunk<T>();   // complex values per TMEM access
+        if (q < 2) {
+            const uint32_t dst = q == 0 ? tF0 : tG1;
+#pragma unroll
+            for (int ch = 0; ch < 16 / CH; ++ch) {
+                T px[CH], py[CH];
+#pragma unroll
+                for (int k = 0; k < CH; ++k) {
+                    const int n1 = ch * CH + k;
+                    cx<T> v = y[brev<R1>(n1)];
+                    if (q == 1) v = cmulc(v, ldg(tw.w3a + R2 * n1 + ii));
+                    px[k] = v.x;
+                    py[k] = v.y;
+                }
+                tmem_store_cx(dst + 16 * ch, px, py);
+            }
+        } else {
+            tmem_wait_st();
+#pragma unroll
+            for (int ch = 0; ch < 16 / CH; ++ch) {
+                T fx[CH], fy[CH], gx[CH], gy[CH];
+                tmem_load_cx(tF0 + 16 * ch, fx, fy);
+                tmem_load_cx(tG1 + 16 * ch, gx, gy);
+                if (i < R2) {
+#pragma unroll
+                    for (int k = 0; k < CH; ++k) {
+                        const int n1 = ch * CH + k;
+                        const int n = R2 * n1 + i;
+                        const cx<T> g2 = cmulc(y[brev<R1>(n1)], ldg(tw.w3b + n));
+                        const cx<T> f0 = mk<T>(fx[k], fy[k]), g1 = mk<T>(gx[k], gy[k]);
+                        const cx<T> S = g1 + g2, D = g1 - g2;
+                        constexpr T h3 = (T)0.86602540378443864676L;
+                        const cx<T> A = f0 + S;
+                        // C = F0 - S/2 + i (sqrt3/2) D
+                        const cx<T> C = mk<T>(f0.x - (T)0.5 * S.x - h3 * D.y, f0.y - (T)0.5 * S.y + h3 * D.x);
+                        op[(long)n * g.ostride] = scale * A;
+                        op[(long)(L + n) * g.ostride] = (n == 0) ? mk<T>(0, 0) : scale * C;
+                    }
+                }
+            }
+        }
+        buf ^= 1;
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tslot, NCOLS);
 }
 
 }  // namespace ns

@@ -4,6 +4,10 @@
 #include "kernels_z.cuh"
 #include "kernels_zfused.cuh"
 #include "kernels_zfused8.cuh"
+#include "kernels_zfused16.cuh"
+#include "kernels_zfused16t.cuh"
+#include <cstdlib>
+#include <cstring>
 #include "ns_internal.h"
 
 namespace ns {
@@ -60,6 +64,19 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     if (e != cudaSuccess) return e;
     const long blocks = (g.total_tiles + TPB - 1) / TPB;
     k<<<(unsigned)blocks, TC * C::P * TPB, smem, st>>>(in, out, g, scale, tw);
+    return cudaGetLastError();
+}
+
+// long lines (L = 128, 256): forward pass with F_0 / G_1 parked in tensor memory
+template <typename T, int L>
+static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
+    constexpr int TC = tile_cols<T>(), R2 = L / 16;
+    constexpr int MINB = sizeof(T) == 8 ? 2 : 1;
+    auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB>;
+    const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    k<<<(unsigned)g.total_tiles, TC * 16, smem, st>>>(in, out, g, scale, tw);
     return cudaGetLastError();
 }
 
@@ -126,6 +143,70 @@ static cudaError_t z_fused8_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long
     return cudaGetLastError();
 }
 
+// 16-values-per-lane fused z kernel for L >= 128
+template <typename T, int L, bool STASH3>
+static cudaError_t z_fused16_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+                               Twiddles<T> tw) {
+    using Geo = Z16Geo<L>;
+    constexpr int UPB = 1, LPB = Geo::UL * UPB;
+    constexpr int MINB = STASH3 ? (sizeof(T) == 8 ? 3 : 5) : 2;
+    auto k = z_fused16_kernel<T, L, UPB, MINB, STASH3>;
+    const size_t smem = (size_t)LPB * 3 * (L + Geo::SZ) * sizeof(cx<T>) + (STASH3 ? (size_t)LPB * 3 * L * sizeof(T) : 0) +
+                        (size_t)LPB * 8 + 8;
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
+    const long lines = MM * batch;
+    static int num_sms = 0;
+    if (num_sms == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 96 * UPB, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    long grid = (long)num_sms * occ;
+    if (grid > lines / LPB) grid = lines / LPB;
+    k<<<(unsigned)grid, 96 * UPB, smem, st>>>(in, out, MM, lines, umax2, tw);
+    return cudaGetLastError();
+}
+
+// 16-values-per-lane fused z kernel with the physical fields parked in tensor memory, L >= 128
+template <typename T, int L>
+static cudaError_t z_fused16t_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+                                Twiddles<T> tw) {
+    using Geo = Z16Geo<L>;
+    constexpr int LPB = Geo::UL;
+    constexpr int MINB = sizeof(T) == 8 ? 4 : 6;
+    constexpr int TMEM_COLS = 3 * 16 * sizeof(T) / 4 <= 64 ? 64 : 128;
+    auto k = z_fused16t_kernel<T, L, MINB>;
+    const size_t smem = (size_t)LPB * 3 * (L + Geo::SZ) * sizeof(cx<T>) + (size_t)LPB * 8 + 16;
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
+    const long lines = MM * batch;
+    static int num_sms = 0;
+    if (num_sms == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    // The occupancy API reports 1 CTA/SM for a kernel that allocates tensor memory; the real limits are the
+    // launch bound (registers), shared memory (227 KB per SM, 1 KB reserved per CTA) and 512 TMEM columns.
+    int occ = MINB;
+    const int by_smem = (int)((227 * 1024) / (smem + 1024));
+    if (occ > by_smem) occ = by_smem;
+    if (occ > 512 / TMEM_COLS) occ = 512 / TMEM_COLS;
+    if (occ < 1) occ = 1;
+    if (const char* oc = getenv("NS_ZOCC")) { int o = atoi(oc); if (o >= 1 && o < occ) occ = o; }
+    long grid = (long)num_sms * occ;
+    if (grid > lines / LPB) grid = lines / LPB;
+    k<<<(unsigned)grid, 96, smem, st>>>(in, out, MM, lines, umax2, tw);
+    return cudaGetLastError();
+}
+
 #define NS_DISPATCH_L(L, CALL)                                   \
     switch (L) {                                                 \
         case 8: return CALL(8);                                  \
@@ -164,6 +245,13 @@ cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
+    static int variant = -1;  // 1: tensor-memory variant for the long lines (default), 0: register / shared-memory variant
+    if (variant < 0) {
+        const char* v = getenv("NS_COLVARIANT");
+        variant = (v != nullptr && strcmp(v, "reg") == 0) ? 0 : 1;
+    }
+    if (variant == 1 && L == 128) return col_fwd_tmem_L<T, 128>(st, in, out, g, scale, tw);
+    if (variant == 1 && L == 256) return col_fwd_tmem_L<T, 256>(st, in, out, g, scale, tw);
 #define CALL(LL) col_fwd_L<T, LL>(st, in, out, g, scale, tw)
     NS_DISPATCH_L(L, CALL)
 #undef CALL
@@ -173,6 +261,22 @@ template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw) {
     if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
+    static int variant = -1;  // 0: 8 values per lane, 1: 16 per lane + u3 in shared memory, 2: 16 per lane, all registers
+    if (variant < 0) {
+        const char* v = getenv("NS_ZVARIANT");
+        variant = v == nullptr ? 3 : (strcmp(v, "8") == 0 ? 0 : (strcmp(v, "16r") == 0 ? 2 : (strcmp(v, "16s") == 0 ? 1 : 3)));
+    }
+    if (variant == 3) {
+        if (L == 128) return z_fused16t_L<T, 128>(st, in, out, MM, batch, umax2, tw);
+        if (L == 256) return z_fused16t_L<T, 256>(st, in, out, MM, batch, umax2, tw);
+    }
+    if (variant == 1) {
+        if (L == 128) return z_fused16_L<T, 128, true>(st, in, out, MM, batch, umax2, tw);
+        if (L == 256) return z_fused16_L<T, 256, true>(st, in, out, MM, batch, umax2, tw);
+    } else if (variant == 2) {
+        if (L == 128) return z_fused16_L<T, 128, false>(st, in, out, MM, batch, umax2, tw);
+        if (L == 256) return z_fused16_L<T, 256, false>(st, in, out, MM, batch, umax2, tw);
+    }
     if (L == 128) return z_fused8_L<T, 128>(st, in, out, MM, batch, umax2, tw);
     if (L == 256) return z_fused8_L<T, 256>(st, in, out, MM, batch, umax2, tw);
 #define CALL(LL) z_fused_L<T, LL>(st, in, out, MM, batch, umax2, tw)

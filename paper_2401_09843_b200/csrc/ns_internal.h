@@ -24,10 +24,13 @@ struct Twiddles {
     const cx<T>* z8A;
     const cx<T>* z8B;
     const cx<T>* z8C;
+    // table of the 16-values-per-lane z kernel (kernels_zfused16.cuh), G = L/16 (L >= 128 only):
+    //   z16[r1*G + t] = w_L^{r1 t},  r1 < 16, t < G
+    const cx<T>* z16;
 };
 // number of complex entries of the table block and its host-side construction (long double arguments);
 // make_twiddles() returns the views into a device copy of that block
-inline size_t twiddle_table_len(int L) { return (size_t)7 * L; }
+inline size_t twiddle_table_len(int L) { return (size_t)8 * L; }
 // register-stage split L = R1 x R2 used by the kernels (needed by the host to build twA / twB)
 void fft_split(int L, int* R1, int* R2);
 
