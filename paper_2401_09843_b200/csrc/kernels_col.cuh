@@ -142,19 +142,32 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
     cx<T>* G1 = E + 2 * EBUF + (size_t)tl * L * TC;
 
     cx<T> F0[R1];
+    cx<T> x[R2];
     int buf = 0;
-#pragma unroll 1
+    if (i < R1) {
+#pragma unroll
+        for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(i + R1 * r2) * g.istride);
+    }
+    // PF: rows of the next sub-transform are fetched while this one goes through its second stage
+    // (more bytes in flight per SM; only where the registers allow it)
+    constexpr bool PF = R1 * R2 <= 64;
+#pragma unroll
     for (int q = 0; q < 3; ++q) {
         if (i < R1) {
-            cx<T> x[R2];
+            if (!PF && q > 0) {
 #pragma unroll
-            for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(q * L + i + R1 * r2) * g.istride);
+                for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(q * L + i + R1 * r2) * g.istride);
+            }
             fft_reg<R2, -1, T>(x);
 #pragma unroll
             for (int n2 = 0; n2 < R2; ++n2) {
                 cx<T> v = x[brev<R2>(n2)];
                 if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
                 Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c] = v;
+            }
+            if (PF && q < 2) {
+#pragma unroll
+                for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)((q + 1) * L + i + R1 * r2) * g.istride);
             }
         }
         __syncthreads();

@@ -29,4 +29,47 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, doub
     atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
+// 3 -> 2 radix-3 combine + Hermitian split of one forward pair (see kernels_z.cuh):
+// reads F_q[n] W^{-qn} of the three sub-transforms from Sl (regions SZ apart), writes B_a^[n], B_b^[n] for
+// n and L - n.  One call covers n = tl, tl + TPL, ... <= L/2 with all loads issued first.
+template <typename T, int L, int SZ, int TPL>
+__device__ __forceinline__ void z_combine_store(const cx<T>* __restrict__ Sl, cx<T>* __restrict__ Oa, cx<T>* __restrict__ Ob,
+                                                bool two, int tl) {
+    constexpr int NIT = (L / 2 + TPL) / TPL;  // iterations covering n in [0, L/2]
+    constexpr T h3 = (T)0.86602540378443864676L;
+    cx<T> f0[NIT], g1[NIT], g2[NIT], f0m[NIT], g1m[NIT], g2m[NIT];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        int n = tl + it * TPL;
+        if (n > L / 2) n = L / 2;             // clamped duplicate, not stored
+        const int m = n == 0 ? 0 : L - n;
+        f0[it] = Sl[n]; g1[it] = Sl[SZ + n]; g2[it] = Sl[2 * SZ + n];
+        f0m[it] = Sl[m]; g1m[it] = Sl[SZ + m]; g2m[it] = Sl[2 * SZ + m];
+    }
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        const int n = tl + it * TPL;
+        const cx<T> Sn = g1[it] + g2[it], Dn = g1[it] - g2[it];
+        const cx<T> An = f0[it] + Sn;
+        const cx<T> Cn = mk<T>(f0[it].x - (T)0.5 * Sn.x - h3 * Dn.y, f0[it].y - (T)0.5 * Sn.y + h3 * Dn.x);
+        const cx<T> Sm = g1m[it] + g2m[it], Dm = g1m[it] - g2m[it];
+        const cx<T> Am = f0m[it] + Sm;
+        const cx<T> Cm = mk<T>(f0m[it].x - (T)0.5 * Sm.x - h3 * Dm.y, f0m[it].y - (T)0.5 * Sm.y + h3 * Dm.x);
+        if (n <= L / 2) {
+            if (n == 0) {
+                Oa[0] = mk<T>(An.x, 0);
+                if (two) Ob[0] = mk<T>(An.y, 0);
+            } else {
+                const int m = L - n;
+                Oa[n] = mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y));
+                if (two) Ob[n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
+                if (m != n) {
+                    Oa[m] = mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y));
+                    if (two) Ob[m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
+                }
+            }
+        }
+    }
+}
+
 }  // namespace ns

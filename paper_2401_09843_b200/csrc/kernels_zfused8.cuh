@@ -235,31 +235,7 @@ z_fused8_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, 
             named_bar_sync(bar_id, UT);
             // the line's inputs were consumed long ago by all three warps: prefetch the next line
             if (pair == 0 && tl == 0 && line + groups < total_lines) issue(line + groups);
-            {
-                constexpr T h3 = (T)0.86602540378443864676L;
-                for (int n = tl; n <= L / 2; n += TPL) {
-                    const cx<T> f0 = Sl[n], g1 = Sl[SZ + n], g2 = Sl[2 * SZ + n];
-                    const cx<T> Sm_ = g1 + g2, D = g1 - g2;
-                    const cx<T> An = f0 + Sm_;
-                    if (n == 0) {
-                        Op[ca * cs] = mk<T>(An.x, 0);
-                        if (pair < 2) Op[cb * cs] = mk<T>(An.y, 0);
-                    } else {
-                        const cx<T> Cn = mk<T>(f0.x - (T)0.5 * Sm_.x - h3 * D.y, f0.y - (T)0.5 * Sm_.y + h3 * D.x);
-                        const int m = L - n;
-                        const cx<T> f0m = Sl[m], g1m = Sl[SZ + m], g2m = Sl[2 * SZ + m];
-                        const cx<T> Sm = g1m + g2m, Dm = g1m - g2m;
-                        const cx<T> Am = f0m + Sm;
-                        const cx<T> Cm = mk<T>(f0m.x - (T)0.5 * Sm.x - h3 * Dm.y, f0m.y - (T)0.5 * Sm.y + h3 * Dm.x);
-                        Op[ca * cs + n] = mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y));
-                        if (pair < 2) Op[cb * cs + n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
-                        if (m != n) {
-                            Op[ca * cs + m] = mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y));
-                            if (pair < 2) Op[cb * cs + m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
-                        }
-                    }
-                }
-            }
+            z_combine_store<T, L, SZ, TPL>(Sl, Op + ca * cs, Op + cb * cs, pair < 2, tl);
             named_bar_sync(bar_id, UT);  // combine reads done before the regions are reused
         }
     }

@@ -71,7 +71,7 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
 template <typename T, int L>
 static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
     constexpr int TC = tile_cols<T>(), R2 = L / 16;
-    constexpr int MINB = sizeof(T) == 8 ? 2 : 1;
+    constexpr int MINB = 2;
     auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB>;
     const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
@@ -143,36 +143,6 @@ static cudaError_t z_fused8_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long
     return cudaGetLastError();
 }
 
-// 16-values-per-lane fused z kernel for L >= 128
-template <typename T, int L, bool STASH3>
-static cudaError_t z_fused16_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
-                               Twiddles<T> tw) {
-    using Geo = Z16Geo<L>;
-    constexpr int UPB = 1, LPB = Geo::UL * UPB;
-    constexpr int MINB = STASH3 ? (sizeof(T) == 8 ? 3 : 5) : 2;
-    auto k = z_fused16_kernel<T, L, UPB, MINB, STASH3>;
-    const size_t smem = (size_t)LPB * 3 * (L + Geo::SZ) * sizeof(cx<T>) + (STASH3 ? (size_t)LPB * 3 * L * sizeof(T) : 0) +
-                        (size_t)LPB * 8 + 8;
-    cudaError_t e = set_smem(k, smem);
-    if (e != cudaSuccess) return e;
-    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
-    const long lines = MM * batch;
-    static int num_sms = 0;
-    if (num_sms == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-    }
-    int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 96 * UPB, smem);
-    if (e != cudaSuccess) return e;
-    if (occ < 1) occ = 1;
-    long grid = (long)num_sms * occ;
-    if (grid > lines / LPB) grid = lines / LPB;
-    k<<<(unsigned)grid, 96 * UPB, smem, st>>>(in, out, MM, lines, umax2, tw);
-    return cudaGetLastError();
-}
-
 // 16-values-per-lane fused z kernel with the physical fields parked in tensor memory, L >= 128
 template <typename T, int L>
 static cudaError_t z_fused16t_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
@@ -200,7 +170,6 @@ static cudaError_t z_fused16t_L(cudaStream_t st, const cx<T>* in, cx<T>* out, lo
     if (occ > by_smem) occ = by_smem;
     if (occ > 512 / TMEM_COLS) occ = 512 / TMEM_COLS;
     if (occ < 1) occ = 1;
-    if (const char* oc = getenv("NS_ZOCC")) { int o = atoi(oc); if (o >= 1 && o < occ) occ = o; }
     long grid = (long)num_sms * occ;
     if (grid > lines / LPB) grid = lines / LPB;
     k<<<(unsigned)grid, 96, smem, st>>>(in, out, MM, lines, umax2, tw);
@@ -260,23 +229,17 @@ cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
 template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw) {
-    if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
-    static int variant = -1;  // 0: 8 values per lane, 1: 16 per lane + u3 in shared memory, 2: 16 per lane, all registers
+    // NS_ZVARIANT=8 selects the 8-values-per-lane kernel for L >= 128 as well (A/B comparison, profiles/)
+    static int variant = -1;
     if (variant < 0) {
         const char* v = getenv("NS_ZVARIANT");
-        variant = v == nullptr ? 3 : (strcmp(v, "8") == 0 ? 0 : (strcmp(v, "16r") == 0 ? 2 : (strcmp(v, "16s") == 0 ? 1 : 3)));
+        variant = (v != nullptr && strcmp(v, "8") == 0) ? 0 : 1;
     }
-    if (variant == 3) {
+    if (variant == 1) {
         if (L == 128) return z_fused16t_L<T, 128>(st, in, out, MM, batch, umax2, tw);
         if (L == 256) return z_fused16t_L<T, 256>(st, in, out, MM, batch, umax2, tw);
     }
-    if (variant == 1) {
-        if (L == 128) return z_fused16_L<T, 128, true>(st, in, out, MM, batch, umax2, tw);
-        if (L == 256) return z_fused16_L<T, 256, true>(st, in, out, MM, batch, umax2, tw);
-    } else if (variant == 2) {
-        if (L == 128) return z_fused16_L<T, 128, false>(st, in, out, MM, batch, umax2, tw);
-        if (L == 256) return z_fused16_L<T, 256, false>(st, in, out, MM, batch, umax2, tw);
-    }
+    if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
     if (L == 128) return z_fused8_L<T, 128>(st, in, out, MM, batch, umax2, tw);
     if (L == 256) return z_fused8_L<T, 256>(st, in, out, MM, batch, umax2, tw);
 #define CALL(LL) z_fused_L<T, LL>(st, in, out, MM, batch, umax2, tw)

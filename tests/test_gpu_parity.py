@@ -325,6 +325,47 @@ def test_fp32_parity(ns, oracle, N):
     assert rel(s.get_fields()[0], oracle.get_fields(N, uh)) < 1e-4
 
 
+def test_fp32_rhs_parity_128(ns, oracle):
+    """fp32 RHS at 128^3 (L = 64 kernels) against the full fp64 oracle."""
+    N = 128
+    u = field(N, 428)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, dtype="f32", **kw)
+    uh = oracle.set_initial(N, u)
+    s.set_spectral(uh[None].astype(np.complex64))
+    assert rel(s.rhs()[0], oracle.rhs(N, oracle.Params(**kw), uh)) < TOL_RHS_F32
+
+
+@pytest.mark.parametrize("N", [256, 512])
+def test_fp32_full_size_sampled(ns, oracle, N):
+    """fp32 at the sizes that run the long-line kernels (L = 128, 256: 16 values per lane, tensor-memory parking):
+    ns_rhs at sampled wavenumbers against the oracle's direct truncated convolution, the whole array against the
+    fp64 CUDA result (itself checked against the oracle in test_full_size_sampled_rhs_and_step), and one RK3 step."""
+    u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5) if N == 256 else inputs.gaussian_k53(N, seed=5)
+    kw = dict(eps=0.05, s=1.0)
+    s64 = ns.Solver(N, **kw)
+    s64.set_initial(u[None])
+    del u
+    uh = s64.get_spectral()[0]
+    r64 = s64.rhs()[0]
+    dt = 0.2 * (2 * np.pi / N) / s64.max_velocity()[0]
+    s64.step(dt)
+    u64 = s64.get_spectral()[0]
+    del s64
+    s = ns.Solver(N, dtype="f32", **kw)
+    s.set_spectral(uh[None].astype(np.complex64))
+    r = s.rhs()[0]
+    assert rel(r, r64) < TOL_RHS_F32
+    rmax = np.abs(r64).max()
+    modes = _sample_modes(N, 10, N + 1)
+    want = oracle.rhs_at_modes(N, oracle.Params(**kw), uh, modes)
+    got = np.stack([r[:, ix, iy, iz] for ix, iy, iz in modes])
+    assert np.abs(got - want).max() < 2e-5 * rmax, np.abs(got - want).max() / rmax
+    assert abs(s.max_velocity()[0] * dt / (0.2 * (2 * np.pi / N)) - 1.0) < 1e-5
+    s.step(dt)
+    assert rel(s.get_spectral()[0], u64) < TOL_RHS_F32
+
+
 # ---------------------------------------------------------------------------------- errors / device buffers
 def test_errors_and_device_buffers(ns):
     import torch
