@@ -314,4 +314,110 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
     if (warp == 0) tmem_dealloc(tslot, NCOLS);
 }
 
+// ------------------------------------------------------------------------------------------------
+// inverse, long lines (R1 = 16): same transform as col_inv_kernel with the per-thread inputs
+// t1 = a - c/2, t2 = (sqrt3/2) c (needed again for q = 1, 2) parked in tensor memory, so that a third CTA
+// fits on the SM (the register-resident version needs 254 registers; ncu: 1.9 warps per scheduler, stalls
+// dominated by the global loads).  Thread layout and TMEM window as in col_fwd_tmem_kernel.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int L, int R2, int TC, int MINB>
+__global__ void __launch_bounds__(TC * 16, MINB)
+col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, Twiddles<T> tw) {
+    constexpr int R1 = 16;
+    static_assert(R1 * R2 == L && R2 >= 2 && R2 <= 16, "two register stages, first of 16");
+    constexpr uint32_t C16 = tmem_cols16<T>();
+    constexpr uint32_t NCOLS = 128;
+    static_assert(4 * C16 * ((TC * 16 + 127) / 128) <= NCOLS, "TMEM columns");
+    constexpr int CH = tmem_cx_chunk<T>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* E = reinterpret_cast<cx<T>*>(smem_raw);  // [2][L][TC] exchange
+    __shared__ uint32_t tslot;
+
+    const int c = threadIdx.x % TC, i = threadIdx.x / TC;
+    const int warp = threadIdx.x / 32;
+    const long tile = blockIdx.x;
+    const long slab = tile / g.tiles_per_slab;
+    const int col0 = (int)(tile % g.tiles_per_slab) * TC;
+    const cx<T>* ip = in + slab * g.in_slab + col0 + c;
+    cx<T>* op = out + slab * g.out_slab + col0 + c;
+    constexpr size_t EBUF = (size_t)L * TC;
+    const int ii = i < R2 ? i : 0;   // threads beyond R2 (L = 128) redo column 0 of the first stage and discard it
+
+    // the loads are issued before the TMEM allocation so that their latency overlaps it
+    cx<T> s[R1], cc[R1];
+#pragma unroll
+    for (int n1 = 0; n1 < R1; ++n1) s[n1] = ldg(ip + (long)(R2 * n1 + ii) * g.istride);
+#pragma unroll
+    for (int n1 = 0; n1 < R1; ++n1) {
+        const int n = R2 * n1 + ii;
+        cc[n1] = (n == 0) ? mk<T>(0, 0) : ldg(ip + (long)(L + n) * g.istride);
+    }
+    if (warp == 0) tmem_alloc(&tslot, NCOLS);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tb = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * 4 * C16;
+    const uint32_t tT1 = tb, tT2 = tb + 2 * C16;   // 16 complex each
+
+    // q = 0: s = a + c; park t1 = a - c/2, t2 = (sqrt3/2) c
+#pragma unroll
+    for (int ch = 0; ch < 16 / CH; ++ch) {
+        T ax[CH], ay[CH], bx[CH], by[CH];
+#pragma unroll
+        for (int k = 0; k < CH; ++k) {
+            const int n1 = ch * CH + k;
+            ax[k] = s[n1].x - (T)0.5 * cc[n1].x;
+            ay[k] = s[n1].y - (T)0.5 * cc[n1].y;
+            bx[k] = (T)0.86602540378443864676L * cc[n1].x;
+            by[k] = (T)0.86602540378443864676L * cc[n1].y;
+            s[n1] = s[n1] + cc[n1];
+        }
+        tmem_store_cx(tT1 + 16 * ch, ax, ay);
+        tmem_store_cx(tT2 + 16 * ch, bx, by);
+    }
+    int buf = 0;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        if (q > 0) {
+            if (q == 1) tmem_wait_st();
+#pragma unroll
+            for (int ch = 0; ch < 16 / CH; ++ch) {
+                T ax[CH], ay[CH], bx[CH], by[CH];
+                tmem_load_cx(tT1 + 16 * ch, ax, ay);
+                tmem_load_cx(tT2 + 16 * ch, bx, by);
+#pragma unroll
+                for (int k = 0; k < CH; ++k) {
+                    const int n1 = ch * CH + k;
+                    const int n = R2 * n1 + ii;
+                    // a + c w3^{-q}:  q=1: t1 - i t2,  q=2: t1 + i t2
+                    const cx<T> z = (q == 1) ? mk<T>(ax[k] + by[k], ay[k] - bx[k]) : mk<T>(ax[k] - by[k], ay[k] + bx[k]);
+                    s[n1] = cmul(z, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
+                }
+            }
+        }
+        if (i < R2) {
+            fft_reg<R1, +1, T>(s);
+#pragma unroll
+            for (int r1 = 0; r1 < R1; ++r1) {
+                cx<T> v = s[brev<R1>(r1)];
+                if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
+                E[buf * EBUF + (size_t)(r1 * R2 + i) * TC + c] = v;
+            }
+        }
+        __syncthreads();
+        {
+            cx<T> y[R2];
+#pragma unroll
+            for (int n2 = 0; n2 < R2; ++n2) y[n2] = E[buf * EBUF + (size_t)(i * R2 + n2) * TC + c];
+            fft_reg<R2, +1, T>(y);
+#pragma unroll
+            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[brev<R2>(r2)];
+        }
+        buf ^= 1;
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tslot, NCOLS);
+}
+
 }  // namespace ns

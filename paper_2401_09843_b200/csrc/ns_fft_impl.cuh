@@ -67,11 +67,24 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     return cudaGetLastError();
 }
 
+// long lines (L = 128, 256): inverse pass with its inputs parked in tensor memory
+template <typename T, int L>
+static cudaError_t col_inv_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, Twiddles<T> tw) {
+    constexpr int TC = tile_cols<T>(), R2 = L / 16;
+    constexpr int MINB = sizeof(T) == 8 ? 3 : 2;
+    auto k = col_inv_tmem_kernel<T, L, R2, TC, MINB>;
+    const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    k<<<(unsigned)g.total_tiles, TC * 16, smem, st>>>(in, out, g, tw);
+    return cudaGetLastError();
+}
+
 // long lines (L = 128, 256): forward pass with F_0 / G_1 parked in tensor memory
 template <typename T, int L>
 static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
     constexpr int TC = tile_cols<T>(), R2 = L / 16;
-    constexpr int MINB = 2;
+    constexpr int MINB = sizeof(T) == 8 ? 3 : 2;
     auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB>;
     const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
@@ -187,6 +200,16 @@ static cudaError_t z_fused16t_L(cudaStream_t st, const cx<T>* in, cx<T>* out, lo
         default: return cudaErrorInvalidValue;                   \
     }
 
+// NS_COLVARIANT=reg selects the register / shared-memory column kernels for the long lines too (A/B comparison)
+static int col_variant() {
+    static int variant = -1;
+    if (variant < 0) {
+        const char* v = getenv("NS_COLVARIANT");
+        variant = (v != nullptr && strcmp(v, "reg") == 0) ? 0 : 1;
+    }
+    return variant;
+}
+
 template <typename T>
 static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab) {
     ColArgs g;
@@ -204,6 +227,8 @@ cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
                            long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
+    // measured (profiles/): parking pays at L = 128 (0.264 -> 0.216 ms at 256^3); at L = 256 the register kernel is faster
+    if (col_variant() == 1 && L == 128) return col_inv_tmem_L<T, 128>(st, in, out, g, tw);
 #define CALL(LL) col_inv_L<T, LL>(st, in, out, g, tw)
     NS_DISPATCH_L(L, CALL)
 #undef CALL
@@ -214,13 +239,8 @@ cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
-    static int variant = -1;  // 1: tensor-memory variant for the long lines (default), 0: register / shared-memory variant
-    if (variant < 0) {
-        const char* v = getenv("NS_COLVARIANT");
-        variant = (v != nullptr && strcmp(v, "reg") == 0) ? 0 : 1;
-    }
-    if (variant == 1 && L == 128) return col_fwd_tmem_L<T, 128>(st, in, out, g, scale, tw);
-    if (variant == 1 && L == 256) return col_fwd_tmem_L<T, 256>(st, in, out, g, scale, tw);
+    if (col_variant() == 1 && L == 128) return col_fwd_tmem_L<T, 128>(st, in, out, g, scale, tw);
+    if (col_variant() == 1 && L == 256) return col_fwd_tmem_L<T, 256>(st, in, out, g, scale, tw);
 #define CALL(LL) col_fwd_L<T, LL>(st, in, out, g, scale, tw)
     NS_DISPATCH_L(L, CALL)
 #undef CALL
