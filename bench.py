@@ -290,6 +290,11 @@ def main():
     roof = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
             "frac": kernels[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
             "alg_bytes_per_launch": kernels[dom]["alg_bytes_per_launch"], "ms_per_launch": kernels[dom]["ms_per_launch"]}
+    if dom == "a3a4_z_fused":
+        roof["note"] = ("fused a3+a4: by bytes HBM is the roofline (DRAM traffic = algorithmic 8*A2), but ncu shows a latency / "
+                        "fp64-issue limited kernel (c5: fp64 pipe 44 %, l1tex 63 %, DRAM 23 % busy; profiles/r01b_tmem.md); the "
+                        "unfused a3 + a4 of the fixed model would need model_bytes_per_launch / peak = "
+                        f"{kernels[dom]['model_bytes_per_launch'] / (peak * 1e9) * 1e3:.2f} ms at the measured peak")
     step_roof = {"model_bytes_per_step": model_bytes, "achieved_gbs": model_bytes / (ms_per_step * 1e-3) / 1e9,
                  "frac_of_measured_peak": model_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                  "frac_of_nominal_8TBs": model_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
