@@ -108,6 +108,10 @@ int ns_get_fields(ns_solver* h, void* u_phys_out, ns_memspace ms);
  *   E_out[b][K] = 1/2 sum_{K-1/2 <= |k| < K+1/2} |u_hat_k|^2 over the full spectrum, K = 0..nbins-1,
  * host array [batch][nbins] of double; sum_K E = 1/2 <|u|^2> when nbins covers all modes. */
 int ns_energy_spectrum(ns_solver* h, double* E_out, int nbins);
+/* Shell enstrophy spectrum (the "enstrophy spectrum" writer; reading A20): with omega_hat = i k x u_hat,
+ *   Z_out[b][K] = 1/2 sum_{K-1/2 <= |k| < K+1/2} |omega_hat_k|^2, same shells, weights, layout and errors as
+ * ns_energy_spectrum; sum_K Z = 1/2 <|curl u|^2>. */
+int ns_enstrophy_spectrum(ns_solver* h, double* Z_out, int nbins);
 /* Second-order longitudinal+transverse structure function on the N grid (reading A15):
  *   S_out[b][l-1] = (1/3) sum_d < |u(x + l dx e_d) - u(x)|^2 >_x,  l = 1..nl (nl <= N/2), host [batch][nl]. */
 int ns_structure_function(ns_solver* h, double* S_out, int nl);

@@ -464,6 +464,30 @@ void orc_energy_spectrum(int N, const double* u_hat, int nbins, double* E) {
             }
 }
 
+// Enstrophy spectrum (PAPER.md:L163 names the writer only; reading A20): with the vorticity
+// omega_hat_k = i k x u_hat_k,  Z(K) = 1/2 sum_{K-1/2 <= |k| < K+1/2} |omega_hat_k|^2 over the FULL spectrum
+// (same shells and weights as orc_energy_spectrum), so that sum_K Z = 1/2 <|curl u|^2>.
+void orc_enstrophy_spectrum(int N, const double* u_hat, int nbins, double* Z) {
+    const int Hs = N / 2 + 1;
+    const size_t ns = (size_t)N * N * Hs;
+    const cplx* uh = (const cplx*)u_hat;
+    const cplx I(0.0, 1.0);
+    for (int b = 0; b < nbins; ++b) Z[b] = 0.0;
+    for (int ix = 0; ix < N; ++ix)
+        for (int iy = 0; iy < N; ++iy)
+            for (int iz = 0; iz < Hs; ++iz) {
+                if (nyquist(ix, N) || nyquist(iy, N) || nyquist(iz, N)) continue;
+                const double kx = wavenumber(ix, N), ky = wavenumber(iy, N), kz = iz;
+                const int bin = (int)std::floor(std::sqrt(kx * kx + ky * ky + kz * kz) + 0.5);
+                if (bin >= nbins) continue;
+                const size_t o = ((size_t)ix * N + iy) * Hs + iz;
+                const cplx u1 = uh[o], u2 = uh[ns + o], u3 = uh[2 * ns + o];
+                const cplx w1 = I * (ky * u3 - kz * u2), w2 = I * (kz * u1 - kx * u3), w3 = I * (kx * u2 - ky * u1);
+                const double w = iz == 0 ? 1.0 : 2.0;
+                Z[bin] += 0.5 * w * (std::norm(w1) + std::norm(w2) + std::norm(w3));
+            }
+}
+
 // Second-order structure function (reading A15), computed in PHYSICAL space on the N grid:
 // S2(l) = (1/3) sum_{d=1..3} < |u(x + l dx e_d) - u(x)|^2 >_x,  l = 1..nl.
 void orc_structure_function(int N, const double* u_hat, int nl, double* S2) {

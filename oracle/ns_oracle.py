@@ -35,6 +35,7 @@ def _load():
     lib.orc_max_velocity.argtypes = [i, i, p]
     lib.orc_max_velocity.restype = d
     lib.orc_energy_spectrum.argtypes = [i, p, i, p]
+    lib.orc_enstrophy_spectrum.argtypes = [i, p, i, p]
     lib.orc_structure_function.argtypes = [i, p, i, p]
     return lib
 
@@ -156,6 +157,13 @@ def energy_spectrum(N, u_hat, nbins):
     E = np.empty(nbins, dtype=np.float64)
     _lib.orc_energy_spectrum(N, _ptr(u_hat), nbins, _ptr(E))
     return E
+
+
+def enstrophy_spectrum(N, u_hat, nbins):
+    u_hat = _c128(u_hat)
+    Z = np.empty(nbins, dtype=np.float64)
+    _lib.orc_enstrophy_spectrum(N, _ptr(u_hat), nbins, _ptr(Z))
+    return Z
 
 
 def structure_function(N, u_hat, nl=None):

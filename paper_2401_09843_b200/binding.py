@@ -21,7 +21,7 @@ NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE = 0, -1, -2, -3
 
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
-    "ns_step_cfl", "ns_step_dts", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum",
+    "ns_step_cfl", "ns_step_dts", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
     "ns_structure_function", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
 
@@ -61,6 +61,7 @@ def lib():
         L.ns_max_velocity.argtypes = [vp, vp]
         L.ns_get_fields.argtypes = [vp, vp, i]
         L.ns_energy_spectrum.argtypes = [vp, vp, i]
+        L.ns_enstrophy_spectrum.argtypes = [vp, vp, i]
         L.ns_structure_function.argtypes = [vp, vp, i]
         L.ns_profile.argtypes = [vp, i]
         L.ns_profile_read.argtypes = [vp, vp, vp]
@@ -208,6 +209,11 @@ class Solver:
         E = np.empty((self.batch, int(nbins)), dtype=np.float64)
         self._check(lib().ns_energy_spectrum(self._h, ctypes.c_void_p(E.ctypes.data), int(nbins)))
         return E
+
+    def enstrophy_spectrum(self, nbins):
+        Z = np.empty((self.batch, int(nbins)), dtype=np.float64)
+        self._check(lib().ns_enstrophy_spectrum(self._h, ctypes.c_void_p(Z.ctypes.data), int(nbins)))
+        return Z
 
     def structure_function(self, nl=None):
         nl = self.N // 2 if nl is None else int(nl)

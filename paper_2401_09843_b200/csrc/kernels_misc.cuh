@@ -150,9 +150,10 @@ __global__ void to_public_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict
 
 // ------------------------------------------------------------------------------------------------
 // energy spectrum: E[b][K] += w/2 |u_hat|^2, K = floor(|k| + 1/2)
+// ENS: enstrophy spectrum, |u_hat|^2 replaced by |k x u_hat|^2 (vorticity omega_hat = i k x u_hat)
 // grid = (chunks, batch); dynamic smem nbins doubles
 // ------------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, bool ENS>
 __global__ void energy_spectrum_kernel(const cx<T>* __restrict__ U, double* __restrict__ E, int N, int nbins) {
     extern __shared__ double bins[];
     for (int i = threadIdx.x; i < nbins; i += blockDim.x) bins[i] = 0.0;
@@ -168,10 +169,20 @@ __global__ void energy_spectrum_kernel(const cx<T>* __restrict__ U, double* __re
         const int bin = (int)floor(sqrt(kx * kx + ky * ky + kz * kz) + 0.5);
         if (bin >= nbins) continue;
         double e = 0.0;
+        if constexpr (ENS) {
+            const cx<T> a = u[idx], b2 = u[plane + idx], c3 = u[2 * plane + idx];
+            const double ax = a.x, ay = a.y, bx = b2.x, by = b2.y, cxr = c3.x, cyi = c3.y;
+            // k x u, real and imaginary parts separately (the factor i does not change the modulus)
+            const double w1r = ky * cxr - kz * bx, w1i = ky * cyi - kz * by;
+            const double w2r = kz * ax - kx * cxr, w2i = kz * ay - kx * cyi;
+            const double w3r = kx * bx - ky * ax, w3i = kx * by - ky * ay;
+            e = w1r * w1r + w1i * w1i + w2r * w2r + w2i * w2i + w3r * w3r + w3i * w3i;
+        } else {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const cx<T> v = u[c * plane + idx];
-            e += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+            for (int c = 0; c < 3; ++c) {
+                const cx<T> v = u[c * plane + idx];
+                e += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+            }
         }
         atomicAdd(&bins[bin], (iz == 0 ? 0.5 : 1.0) * e);
     }

@@ -29,7 +29,7 @@ struct ns_solver {
     virtual int step_dts(const double* dt) = 0;
     virtual int max_velocity(double* out) = 0;
     virtual int get_fields(void* out, ns_memspace ms) = 0;
-    virtual int energy_spectrum(double* E, int nbins) = 0;
+    virtual int energy_spectrum(double* E, int nbins, bool enstrophy) = 0;
     virtual int structure_function(double* S, int nl) = 0;
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
@@ -409,14 +409,17 @@ public:
         return NS_OK;
     }
 
-    int energy_spectrum(double* E, int nbins) override {
+    int energy_spectrum(double* E, int nbins, bool enstrophy) override {
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
         if (!E || nbins < 1 || nbins > 4096) return fail(NS_ERR_INVALID_ARG, "E is NULL or nbins not in [1, 4096]");
         NS_CK(cudaMemsetAsync(red_dev, 0, (size_t)batch * nbins * sizeof(double), st));
         const long plane = (long)N * N * H;
         unsigned chunks = blocks_for(plane, 256 * 16);
         if (chunks > 1024) chunks = 1024;
-        energy_spectrum_kernel<T><<<dim3(chunks, batch), 256, (size_t)nbins * sizeof(double), st>>>(U, red_dev, N, nbins);
+        if (enstrophy)
+            energy_spectrum_kernel<T, true><<<dim3(chunks, batch), 256, (size_t)nbins * sizeof(double), st>>>(U, red_dev, N, nbins);
+        else
+            energy_spectrum_kernel<T, false><<<dim3(chunks, batch), 256, (size_t)nbins * sizeof(double), st>>>(U, red_dev, N, nbins);
         NS_LAUNCHED("energy_spectrum");
         NS_CK(cudaMemcpyAsync(E, red_dev, (size_t)batch * nbins * sizeof(double), cudaMemcpyDeviceToHost, st));
         NS_CK(cudaStreamSynchronize(st));
@@ -530,7 +533,8 @@ int ns_step_cfl(ns_solver* h, double cfl, double t_end, double* dt_out) { NS_H(h
 int ns_step_dts(ns_solver* h, const double* dt) { NS_H(h); return h->step_dts(dt); }
 int ns_max_velocity(ns_solver* h, double* out) { NS_H(h); return h->max_velocity(out); }
 int ns_get_fields(ns_solver* h, void* out, ns_memspace ms) { NS_H(h); return h->get_fields(out, ms); }
-int ns_energy_spectrum(ns_solver* h, double* E, int nbins) { NS_H(h); return h->energy_spectrum(E, nbins); }
+int ns_energy_spectrum(ns_solver* h, double* E, int nbins) { NS_H(h); return h->energy_spectrum(E, nbins, false); }
+int ns_enstrophy_spectrum(ns_solver* h, double* Z, int nbins) { NS_H(h); return h->energy_spectrum(Z, nbins, true); }
 int ns_structure_function(ns_solver* h, double* S, int nl) { NS_H(h); return h->structure_function(S, nl); }
 double ns_time(const ns_solver* h, int sample) {
     if (!h) return std::numeric_limits<double>::quiet_NaN();

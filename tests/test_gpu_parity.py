@@ -101,6 +101,9 @@ def test_config1_20_steps_fp64(ns, oracle):
     assert abs(s.time(0) - 20 * dt) < 1e-15
     E = s.energy_spectrum(N)[0]
     assert np.abs(E - oracle.energy_spectrum(N, uh, N)).max() < 1e-14
+    Z = s.enstrophy_spectrum(N)[0]
+    Zo = oracle.enstrophy_spectrum(N, uh, N)
+    assert np.abs(Z - Zo).max() < 1e-13 * Zo.max()
     S = s.structure_function()[0]
     assert np.abs(S / oracle.structure_function(N, uh) - 1).max() < 1e-11
 
@@ -259,6 +262,7 @@ def test_config4_ensemble_two_samples(ns, oracle):
     dts = s.step_cfl(0.2, 1.0)
     got = s.get_spectral()
     E = s.energy_spectrum(N)
+    Zs = s.enstrophy_spectrum(N)
     S = s.structure_function()
     for i in (0, 31):
         uh = oracle.set_initial(N, us[i])
@@ -268,6 +272,8 @@ def test_config4_ensemble_two_samples(ns, oracle):
         un = oracle.step(N, p, u0[i], dts[i])
         assert rel(got[i], un) < TOL_STEPS_F64
         assert np.abs(E[i] - oracle.energy_spectrum(N, un, N)).max() < 1e-13
+        Zo = oracle.enstrophy_spectrum(N, un, N)
+        assert np.abs(Zs[i] - Zo).max() < 1e-10 * Zo.max()
         assert np.abs(S[i] / oracle.structure_function(N, un) - 1).max() < 1e-10
     assert len(set(np.round(dts, 12))) > 1          # distinct seeds -> distinct steps
 

@@ -288,6 +288,45 @@ def test_p8_energy_spectrum(oracle):
     assert abs(E[3] - 0.2) < 1e-14 and abs(E.sum() - E[3]) < 1e-15
 
 
+def test_p8b_enstrophy_spectrum(oracle):
+    """Reading A20 (PAPER.md:L163 names the writer only).  Pins: Taylor-Green has omega = (0, 0, 2 sin x sin y), so
+    1/2 <|omega|^2> = 1/2 lands in bin 1; a Beltrami (ABC) field has curl u = u, so Z = E bin by bin; a gradient
+    field has no vorticity (this separates |k x u|^2 from the solenoidal shortcut |k|^2 |u|^2); and sum_K Z equals
+    1/2 <|curl u|^2> with the curl taken by centred spectral differences written here with numpy.fft."""
+    N = 16
+    tg = oracle.set_initial(N, inputs.taylor_green_2d(N))
+    Z = oracle.enstrophy_spectrum(N, tg, 8)
+    want = np.zeros(8)
+    want[1] = 0.5
+    assert np.abs(Z - want).max() < 1e-15
+    x = 2 * np.pi * np.arange(N) / N
+    X, Y, Zc = np.meshgrid(x, x, x, indexing="ij")
+    A, B, C = 0.7, -0.4, 1.1
+    abc = np.stack([A * np.sin(Zc) + C * np.cos(Y), B * np.sin(X) + A * np.cos(Zc), C * np.sin(Y) + B * np.cos(X)])
+    ua = oracle.set_initial(N, abc)
+    assert np.abs(oracle.enstrophy_spectrum(N, ua, N) - oracle.energy_spectrum(N, ua, N)).max() < 1e-14
+    # gradient field: u = grad(phi), written straight into the spectral state (set_initial would project it away)
+    rng = np.random.default_rng(82)
+    phi = rng.standard_normal((N, N, N))
+    ph = np.fft.rfftn(phi) / N ** 3
+    k = np.fft.fftfreq(N, 1.0 / N)
+    kz = np.arange(N // 2 + 1.0)
+    g = np.stack([1j * k[:, None, None] * ph, 1j * k[None, :, None] * ph, 1j * kz[None, None, :] * ph])
+    g[:, N // 2] = 0; g[:, :, N // 2] = 0; g[:, :, :, N // 2] = 0
+    assert oracle.energy_spectrum(N, g, N).sum() > 1e-3
+    assert oracle.enstrophy_spectrum(N, g, N).max() < 1e-28
+    # Parseval against a curl evaluated with numpy.fft on the physical field
+    u = inputs.gaussian_field(N, 83, lambda kk: np.where(kk <= 5, kk ** 2, 0.0), e_tot=0.37)
+    uh = oracle.set_initial(N, u)
+    U = np.fft.fftn(u, axes=(1, 2, 3))
+    KX, KY, KZ = np.meshgrid(k, k, k, indexing="ij")
+    for K in (KX, KY, KZ):
+        K[np.abs(K) == N // 2] = 0.0   # the oracle state carries no Nyquist planes
+    W = np.stack([KY * U[2] - KZ * U[1], KZ * U[0] - KX * U[2], KX * U[1] - KY * U[0]]) * 1j
+    w = np.real(np.fft.ifftn(W, axes=(1, 2, 3)))
+    assert abs(oracle.enstrophy_spectrum(N, uh, N).sum() - 0.5 * np.mean(np.sum(w * w, axis=0))) < 1e-12
+
+
 # ------------------------------------------------------------------------------------------- P9
 def test_p9_structure_function_identity(oracle):
     N = 12
