@@ -37,6 +37,9 @@ WORKLOADS = {
     "c2": dict(cfg=1, N=128, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[1]: 128^3 Gaussian k^4 exp, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=64),
     "c3": dict(cfg=2, N=256, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[2]: 256^3 perturbed shear layer, hyperviscosity, CFL 0.2", cpuN=64),
     "c4": dict(cfg=3, N=128, batch=32, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[3]: 32 x 128^3 shear-layer ensemble in one launch, CFL 0.2", cpuN=64),
+    # the paper's own experiments, hyperviscosity order s = 1.5
+    "tg3d": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.1-6.3: 256^3 perturbed 3-D Taylor-Green, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=64),
+    "cyl": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.4-6.6: 256^3 cylindrical shear flow rho=0.05, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=64),
     "c5": dict(cfg=4, N=512, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[4]: 512^3 Gaussian k^-5/3, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=64),
 }
 
@@ -53,6 +56,10 @@ def make_input(name: str, N: int, batch: int) -> np.ndarray:
         return inputs.shear_layer_ensemble(N, batch, seed0=1000)
     if name == "c5":
         return inputs.gaussian_k53(N, seed=5)[None]
+    if name == "tg3d":
+        return inputs.taylor_green_3d_perturbed(N, seed=6)[None]
+    if name == "cyl":
+        return inputs.cylindrical_shear(N, seed=7, rho=0.05)[None]
     raise KeyError(name)
 
 

@@ -12,6 +12,9 @@ Workload recipes (they stand in for the paper's workloads, 
   config 3  shear_layer              N=256  doubly periodic perturbed shear layer
   config 4  shear_layer ensemble     32 x N=128, seed 1000+i per sample
   config 5  gaussian_field k^-5/3    N=512  E(k) ~ k^-5/3 on 1 <= k <= N/3, E_tot = 0.5
+The paper's own experiments (NEXT-2 of SURVEY.md 8(f), hyperviscosity order s = 1.5):
+  tg3d      taylor_green_3d_perturbed   eq. (6.1)-(6.3)
+  cyl       cylindrical_shear           eq. (6.4)-(6.6)
 """
 from __future__ import annotations
 
@@ -160,6 +163,46 @@ def shear_layer(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmod
 def shear_layer_ensemble(N: int = 128, batch: int = 32, seed0: int = 1000) -> np.ndarray:
     """Config 4: `batch` shear-layer samples, sample i uses seed seed0 + i.  [batch][3][N][N][N]."""
     return np.stack([shear_layer(N, seed0 + i) for i in range(batch)])
+
+
+def taylor_green_3d_perturbed(N: int, seed: int, delta: float = 0.025) -> np.ndarray:
+    """The paper's perturbed 3-D Taylor-Green vortex, eq. (6.1)-(6.3) with A = 1, B = -1, C = 0,
+    on [0,2pi)^3 (the paper's 2 pi x is our x):
+      u = cos x sin y sin z + e_0,  v = -sin x cos y sin z + e_1,  w = e_2,
+      e_d = (1/8) sum_{(i,j,k) in {0,1}^3} d_{d,i,j,k} a_i(2x) a_j(2y) a_k(2z),  a_0 = sin, a_1 = cos,
+      d_{d,i,j,k} ~ U[-delta, delta] i.i.d. (24 numbers per sample).  The perturbation is not solenoidal as written;
+    `set_initial` projects it."""
+    X, Y, Z = grid(N)
+    d = (2.0 * uniform01(seed, 200, 24) - 1.0) * delta
+    u = np.zeros((3, N, N, N))
+    u[0] = np.cos(X) * np.sin(Y) * np.sin(Z)
+    u[1] = -np.sin(X) * np.cos(Y) * np.sin(Z)
+    a = lambda i, t: np.sin(t) if i == 0 else np.cos(t)
+    for c in range(3):
+        for i in range(2):
+            for j in range(2):
+                for k in range(2):
+                    u[c] += 0.125 * d[((c * 2 + i) * 2 + j) * 2 + k] * a(i, 2 * X) * a(j, 2 * Y) * a(k, 2 * Z)
+    return u
+
+
+def cylindrical_shear(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmodes: int = 10) -> np.ndarray:
+    """The paper's cylindrical shear flow, eq. (6.4)-(6.6), in unit coordinates X = x/2pi etc.:
+      u = tanh(2 pi (r - 0.25)/rho)  (rho = 0: the sign function of eq. 6.6),  v = w = 0,
+      r^2 = (Y - 0.5 + s_y(X))^2 + (Z - 0.5 + s_z(X))^2,  s(X) = delta sum_{k=1..p} a_k sin(2 pi k X - b_k),
+      a_k ~ U[0,1], b_k ~ U[0,2pi] i.i.d., p = 10, delta = 0.025."""
+    xs = np.arange(N) / N
+    a = uniform01(seed, 210, 2 * nmodes)
+    b = uniform01(seed, 211, 2 * nmodes) * 2.0 * np.pi
+    k = np.arange(1, nmodes + 1)
+    sy = delta * np.sum(a[:nmodes, None] * np.sin(2.0 * np.pi * k[:, None] * xs[None, :] - b[:nmodes, None]), axis=0)
+    sz = delta * np.sum(a[nmodes:, None] * np.sin(2.0 * np.pi * k[:, None] * xs[None, :] - b[nmodes:, None]), axis=0)
+    Y = xs[None, :, None]
+    Z = xs[None, None, :]
+    r = np.sqrt((Y - 0.5 + sy[:, None, None]) ** 2 + (Z - 0.5 + sz[:, None, None]) ** 2)
+    u = np.zeros((3, N, N, N))
+    u[0] = np.where(r <= 0.25, -1.0, 1.0) if rho == 0 else np.tanh(2.0 * np.pi * (r - 0.25) / rho)
+    return u
 
 
 def checksum(a: np.ndarray) -> str:

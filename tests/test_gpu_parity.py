@@ -136,6 +136,29 @@ def test_fractional_order(ns, oracle):
     assert rel(s.rhs()[0], oracle.rhs(N, oracle.Params(**kw), uh)) < TOL_RHS_F64
 
 
+@pytest.mark.parametrize("name,N", [("tg3d", 64), ("cyl", 64), ("tg3d", 128)])
+def test_paper_experiments_s15(ns, oracle, name, N):
+    """NEXT-2 of SURVEY.md 8(f): the paper's own workloads, perturbed 3-D Taylor-Green (eq. 6.1-6.3) and cylindrical
+    shear flow (eq. 6.4-6.6), with its fractional hyperviscosity order s = 1.5: set_initial,
+    one RHS and CFL-0.2 steps against the oracle, which replays the GPU's dt."""
+    u = inputs.taylor_green_3d_perturbed(N, 11) if name == "tg3d" else inputs.cylindrical_shear(N, 12, rho=0.05)
+    kw = dict(eps=0.05, s=1.5)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    s.set_spectral(uh[None])
+    p = oracle.Params(**kw)
+    assert rel(s.rhs()[0], oracle.rhs(N, p, uh)) < TOL_RHS_F64
+    for _ in range(4 if N == 64 else 2):
+        dts = s.step_cfl(0.2, 1e9)
+        assert abs(dts[0] - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, uh)) < 1e-12 * dts[0]
+        uh = oracle.step(N, p, uh, dts[0])
+    assert rel(s.get_spectral()[0], uh) < TOL_STEPS_F64
+    Zo = oracle.enstrophy_spectrum(N, uh, N)
+    assert np.abs(s.enstrophy_spectrum(N)[0] - Zo).max() < 1e-10 * Zo.max()
+
+
 def test_batch_is_bitwise_independent(ns):
     """Reading A18: a batched launch gives bit for bit the per-sample result of batch = 1."""
     N, B = 32, 5
