@@ -115,6 +115,17 @@ int ns_enstrophy_spectrum(ns_solver* h, double* Z_out, int nbins);
 /* Second-order longitudinal+transverse structure function on the N grid (reading A15):
  *   S_out[b][l-1] = (1/3) sum_d < |u(x + l dx e_d) - u(x)|^2 >_x,  l = 1..nl (nl <= N/2), host [batch][nl]. */
 int ns_structure_function(ns_solver* h, double* S_out, int nl);
+/* Structure function of order p > 0 (the statistics the paper's ensembles are evaluated with, PAPER.md:L164, L309;
+ * reading A15 extended): S_out[b][l-1] = (1/3) sum_d < |u(x + l dx e_d) - u(x)|^p >_x with the Euclidean norm of the
+ * vector increment, evaluated in physical space on the N grid, l = 1..nl (nl <= N/2), host [batch][nl].
+ * NS_ERR_INVALID_ARG for p <= 0, NULL or nl out of range.  Overwrites the library's workspaces, not the state. */
+int ns_structure_function_p(ns_solver* h, double p, double* S_out, int nl);
+/* Pointwise ensemble moments of the empirical measure (Algorithm 1; the mean and variance fields of
+ * its Fig. 9-10): over the batch samples b = 0..batch-1 on the N grid,
+ *   mean_out[c][x] = (1/batch) sum_b u_b,c(x),   var_out[c][x] = (1/batch) sum_b (u_b,c(x) - mean[c][x])^2,
+ * each [3][N][N][N] reals of the solver dtype in caller memory `ms`; either pointer may be NULL (not both).
+ * Overwrites the library's workspaces, not the state. */
+int ns_ensemble_moments(ns_solver* h, void* mean_out, void* var_out, ns_memspace ms);
 
 /* Simulation time of one sample; NaN if `sample` is out of range. */
 double ns_time(const ns_solver* h, int sample);

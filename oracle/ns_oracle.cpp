@@ -513,4 +513,32 @@ void orc_structure_function(int N, const double* u_hat, int nl, double* S2) {
     }
 }
 
+// Structure function of order p (PAPER.md:L164 names the writer only; reading A15 extended to p != 2):
+// S_p(l) = (1/3) sum_{d=1..3} < |u(x + l dx e_d) - u(x)|^p >_x with the Euclidean norm of the vector increment,
+// in PHYSICAL space on the N grid, l = 1..nl.  p = 2 is orc_structure_function.
+void orc_structure_function_p(int N, const double* u_hat, double p, int nl, double* Sp) {
+    const size_t np = (size_t)N * N * N;
+    std::vector<double> u(3 * np);
+    orc_get_fields(N, u_hat, u.data());
+    for (int l = 1; l <= nl; ++l) {
+        double acc = 0.0;
+        for (int ix = 0; ix < N; ++ix)
+            for (int iy = 0; iy < N; ++iy)
+                for (int iz = 0; iz < N; ++iz) {
+                    const size_t o = ((size_t)ix * N + iy) * N + iz;
+                    const size_t od[3] = {((size_t)((ix + l) % N) * N + iy) * N + iz, ((size_t)ix * N + (iy + l) % N) * N + iz,
+                                          ((size_t)ix * N + iy) * N + (iz + l) % N};
+                    for (int d = 0; d < 3; ++d) {
+                        double r2 = 0.0;
+                        for (int c = 0; c < 3; ++c) {
+                            const double du = u[c * np + od[d]] - u[c * np + o];
+                            r2 += du * du;
+                        }
+                        acc += std::pow(r2, 0.5 * p);
+                    }
+                }
+        Sp[l - 1] = acc / (3.0 * (double)np);
+    }
+}
+
 }  // extern "C"

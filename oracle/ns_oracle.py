@@ -37,6 +37,7 @@ def _load():
     lib.orc_energy_spectrum.argtypes = [i, p, i, p]
     lib.orc_enstrophy_spectrum.argtypes = [i, p, i, p]
     lib.orc_structure_function.argtypes = [i, p, i, p]
+    lib.orc_structure_function_p.argtypes = [i, p, ctypes.c_double, i, p]
     return lib
 
 
@@ -171,4 +172,12 @@ def structure_function(N, u_hat, nl=None):
     u_hat = _c128(u_hat)
     S = np.empty(nl, dtype=np.float64)
     _lib.orc_structure_function(N, _ptr(u_hat), nl, _ptr(S))
+    return S
+
+
+def structure_function_p(N, u_hat, p, nl=None):
+    nl = N // 2 if nl is None else nl
+    u_hat = _c128(u_hat)
+    S = np.empty(nl, dtype=np.float64)
+    _lib.orc_structure_function_p(N, _ptr(u_hat), float(p), nl, _ptr(S))
     return S

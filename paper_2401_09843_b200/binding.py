@@ -22,7 +22,7 @@ NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE = 0, -1, -2, -3
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
     "ns_step_cfl", "ns_step_dts", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
-    "ns_structure_function", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
+    "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
 
 
@@ -63,6 +63,8 @@ def lib():
         L.ns_energy_spectrum.argtypes = [vp, vp, i]
         L.ns_enstrophy_spectrum.argtypes = [vp, vp, i]
         L.ns_structure_function.argtypes = [vp, vp, i]
+        L.ns_structure_function_p.argtypes = [vp, d, vp, i]
+        L.ns_ensemble_moments.argtypes = [vp, vp, vp, i]
         L.ns_profile.argtypes = [vp, i]
         L.ns_profile_read.argtypes = [vp, vp, vp]
         L.ns_time.argtypes = [vp, i]
@@ -209,6 +211,20 @@ class Solver:
         E = np.empty((self.batch, int(nbins)), dtype=np.float64)
         self._check(lib().ns_energy_spectrum(self._h, ctypes.c_void_p(E.ctypes.data), int(nbins)))
         return E
+
+    def structure_function_p(self, p, nl=None):
+        nl = self.N // 2 if nl is None else int(nl)
+        S = np.empty((self.batch, nl), dtype=np.float64)
+        self._check(lib().ns_structure_function_p(self._h, float(p), ctypes.c_void_p(S.ctypes.data), nl))
+        return S
+
+    def ensemble_moments(self):
+        """(mean, var) over the batch, each [3][N][N][N] of the solver dtype (host arrays)."""
+        shape = self.physical_shape[1:]
+        mean = np.empty(shape, dtype=self.real)
+        var = np.empty(shape, dtype=self.real)
+        self._check(lib().ns_ensemble_moments(self._h, ctypes.c_void_p(mean.ctypes.data), ctypes.c_void_p(var.ctypes.data), NS_HOST))
+        return mean, var
 
     def enstrophy_spectrum(self, nbins):
         Z = np.empty((self.batch, int(nbins)), dtype=np.float64)

@@ -375,4 +375,65 @@ __global__ void expand_hermitian_kernel(const cx<T>* __restrict__ U, cx<T>* __re
     W[idx] = v;
 }
 
+// ------------------------------------------------------------------------------------------------
+// structure function of order p in physical space: S[b][l-1] += sum_x sum_d |u(x + l e_d) - u(x)|^p
+// u: [batch][3][N][N][N] reals; grid = (chunks, nl, batch); one shift l per blockIdx.y
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void sf_p_kernel(const T* __restrict__ u, double* __restrict__ S, int N, int nl, double p) {
+    const long np = (long)N * N * N;
+    const int l = blockIdx.y + 1;
+    const long b = blockIdx.z;
+    const T* ub = u + b * 3 * np;
+    const double hp = 0.5 * p;
+    double acc = 0.0;
+    for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < np; idx += (long)gridDim.x * blockDim.x) {
+        const int iz = (int)(idx % N), iy = (int)((idx / N) % N), ix = (int)(idx / ((long)N * N));
+        const long ox = ((long)((ix + l) % N) * N + iy) * N + iz;
+        const long oy = ((long)ix * N + (iy + l) % N) * N + iz;
+        const long oz = ((long)ix * N + iy) * N + (iz + l) % N;
+        double rx = 0.0, ry = 0.0, rz = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double a = (double)ub[c * np + idx];
+            const double dx = (double)ub[c * np + ox] - a, dy = (double)ub[c * np + oy] - a, dz = (double)ub[c * np + oz] - a;
+            rx += dx * dx; ry += dy * dy; rz += dz * dz;
+        }
+        acc += (p == 2.0) ? rx + ry + rz : pow(rx, hp) + pow(ry, hp) + pow(rz, hp);
+    }
+    __shared__ double red[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) atomicAdd(&S[b * nl + (l - 1)], v);
+    }
+}
+
+__global__ void scale_kernel(double* __restrict__ a, double s, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] *= s;
+}
+
+// pointwise mean and (population) variance over the batch: u [batch][n] -> mean [n], var [n]
+template <typename T>
+__global__ void ensemble_moments_kernel(const T* __restrict__ u, T* __restrict__ mean, T* __restrict__ var, long n, int batch) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double m = 0.0;
+    for (int b = 0; b < batch; ++b) m += (double)u[(long)b * n + i];
+    m /= (double)batch;
+    double v = 0.0;
+    for (int b = 0; b < batch; ++b) {
+        const double d = (double)u[(long)b * n + i] - m;
+        v += d * d;
+    }
+    mean[i] = (T)m;
+    var[i] = (T)(v / (double)batch);
+}
+
 }  // namespace ns

@@ -31,6 +31,8 @@ struct ns_solver {
     virtual int get_fields(void* out, ns_memspace ms) = 0;
     virtual int energy_spectrum(double* E, int nbins, bool enstrophy) = 0;
     virtual int structure_function(double* S, int nl) = 0;
+    virtual int structure_function_p(double p, double* S, int nl) = 0;
+    virtual int ensemble_moments(void* mean, void* var, ns_memspace ms) = 0;
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
     virtual int profile(int enable) = 0;
@@ -443,6 +445,56 @@ public:
         return NS_OK;
     }
 
+    int structure_function_p(double p, double* S, int nl) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!S || nl < 1 || nl > N / 2 || !(p > 0.0) || std::isinf(p)) return fail(NS_ERR_INVALID_ARG, "S is NULL, nl not in [1, N/2] or p not positive and finite");
+        // physical fields on the N grid, as in get_fields: Hermitian expansion -> unpadded inverse FFT -> reals in Y
+        const long cubes = (long)batch * 3;
+        const long total = cubes * N * N * N;
+        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        NS_LAUNCHED("expand_hermitian");
+        int rc = generic_fft3(X, cubes, +1);
+        if (rc != NS_OK) return rc;
+        T* phys = reinterpret_cast<T*>(Y);
+        complex_to_real_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(X, phys, total);
+        NS_LAUNCHED("complex_to_real");
+        NS_CK(cudaMemsetAsync(red_dev, 0, (size_t)batch * nl * sizeof(double), st));
+        const long np = (long)N * N * N;
+        unsigned chunks = blocks_for(np, 256 * 8);
+        if (chunks > 592) chunks = 592;
+        sf_p_kernel<T><<<dim3(chunks, nl, batch), 256, 0, st>>>(phys, red_dev, N, nl, p);
+        NS_LAUNCHED("sf_p");
+        scale_kernel<<<blocks_for((long)batch * nl, 128), 128, 0, st>>>(red_dev, 1.0 / (3.0 * (double)np), batch * nl);
+        NS_LAUNCHED("scale");
+        NS_CK(cudaMemcpyAsync(S, red_dev, (size_t)batch * nl * sizeof(double), cudaMemcpyDeviceToHost, st));
+        NS_CK(cudaStreamSynchronize(st));
+        return NS_OK;
+    }
+
+    int ensemble_moments(void* mean, void* var, ns_memspace ms) override {
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        if (!mean && !var) return fail(NS_ERR_INVALID_ARG, "both output pointers are NULL");
+        const long cubes = (long)batch * 3;
+        const long total = cubes * N * N * N;
+        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        NS_LAUNCHED("expand_hermitian");
+        int rc = generic_fft3(X, cubes, +1);
+        if (rc != NS_OK) return rc;
+        T* phys = reinterpret_cast<T*>(Y);
+        complex_to_real_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(X, phys, total);
+        NS_LAUNCHED("complex_to_real");
+        const long n = 3L * N * N * N;                 // X is free again: mean | var staged there
+        T* dmean = reinterpret_cast<T*>(X);
+        T* dvar = dmean + n;
+        ensemble_moments_kernel<T><<<blocks_for(n, 256), 256, 0, st>>>(phys, dmean, dvar, n, batch);
+        NS_LAUNCHED("ensemble_moments");
+        const cudaMemcpyKind kind = ms == NS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+        if (mean) NS_CK(cudaMemcpyAsync(mean, dmean, (size_t)n * sizeof(T), kind, st));
+        if (var) NS_CK(cudaMemcpyAsync(var, dvar, (size_t)n * sizeof(T), kind, st));
+        if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));
+        return NS_OK;
+    }
+
     int profile(int enable) override {
         NS_CK(cudaStreamSynchronize(st));
         prof.reset();
@@ -536,6 +588,8 @@ int ns_get_fields(ns_solver* h, void* out, ns_memspace ms) { NS_H(h); return h->
 int ns_energy_spectrum(ns_solver* h, double* E, int nbins) { NS_H(h); return h->energy_spectrum(E, nbins, false); }
 int ns_enstrophy_spectrum(ns_solver* h, double* Z, int nbins) { NS_H(h); return h->energy_spectrum(Z, nbins, true); }
 int ns_structure_function(ns_solver* h, double* S, int nl) { NS_H(h); return h->structure_function(S, nl); }
+int ns_ensemble_moments(ns_solver* h, void* mean, void* var, ns_memspace ms) { NS_H(h); return h->ensemble_moments(mean, var, ms); }
+int ns_structure_function_p(ns_solver* h, double p, double* S, int nl) { NS_H(h); return h->structure_function_p(p, S, nl); }
 double ns_time(const ns_solver* h, int sample) {
     if (!h) return std::numeric_limits<double>::quiet_NaN();
     return const_cast<ns_solver*>(h)->time(sample);

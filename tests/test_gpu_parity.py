@@ -159,6 +159,39 @@ def test_paper_experiments_s15(ns, oracle, name, N):
     assert np.abs(s.enstrophy_spectrum(N)[0] - Zo).max() < 1e-10 * Zo.max()
 
 
+@pytest.mark.parametrize("N,dtype", [(32, "f64"), (64, "f64"), (32, "f32")])
+def test_structure_function_order_p(ns, oracle, N, dtype):
+    """ns_structure_function_p (physical-space kernel) against the oracle for p = 1, 3, 4 and, for p = 2, also against
+    ns_structure_function (the spectral-identity path); two samples in one launch."""
+    us = np.stack([field(N, 500 + N), inputs.taylor_green_3d_perturbed(N, 13)])
+    s = ns.Solver(N, batch=2, dtype=dtype)
+    s.set_initial(us)
+    tol = 1e-11 if dtype == "f64" else 2e-5
+    for b in range(2):
+        uh = oracle.set_initial(N, us[b])
+        for p in (1.0, 3.0, 4.0):
+            assert np.abs(s.structure_function_p(p)[b] / oracle.structure_function_p(N, uh, p) - 1).max() < tol
+    assert np.abs(s.structure_function_p(2.0, nl=5) / s.structure_function(nl=5) - 1).max() < tol
+    with pytest.raises(ns.NSError):
+        s.structure_function_p(0.0)
+
+
+def test_ensemble_moments(ns, oracle):
+    """Pointwise mean and variance of the empirical measure over the batch (Algorithm 1) against the
+    same moments of the oracle's physical fields; a batch of identical samples has zero variance to round-off."""
+    N, B = 32, 5
+    us = np.stack([inputs.cylindrical_shear(N, 40 + i, rho=0.3) for i in range(B)])
+    s = ns.Solver(N, batch=B)
+    s.set_initial(us)
+    mean, var = s.ensemble_moments()
+    f = np.stack([oracle.get_fields(N, oracle.set_initial(N, u)) for u in us])
+    assert np.abs(mean - f.mean(axis=0)).max() < 1e-13
+    assert np.abs(var - f.var(axis=0)).max() < 1e-13 and var.max() > 1e-3
+    s.set_initial(np.stack([us[0]] * B))
+    mean, var = s.ensemble_moments()
+    assert var.max() < 1e-28 and np.abs(mean - f[0]).max() < 1e-13
+
+
 def test_batch_is_bitwise_independent(ns):
     """Reading A18: a batched launch gives bit for bit the per-sample result of batch = 1."""
     N, B = 32, 5

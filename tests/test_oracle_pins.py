@@ -340,6 +340,29 @@ def test_p9_structure_function_identity(oracle):
     assert np.abs(S / want - 1).max() < 1e-12
 
 
+def test_p9b_structure_function_order_p(oracle):
+    """S_p (reading A15 extended to p != 2): p = 2 is S2; a single shear mode u = (0, a sin(kx), 0) has
+    S_p(l) = (1/3) (2a |sin(k l dx / 2)|)^p <cos^p> with <cos^4> = 3/8, <cos^6> = 5/16 (exact on the grid);
+    odd and fractional orders against increments taken with numpy.roll."""
+    N = 16
+    uh = full_state(oracle, N, 91)
+    assert np.abs(oracle.structure_function_p(N, uh, 2.0) / oracle.structure_function(N, uh) - 1).max() < 1e-13
+    a, k = 0.8, 2
+    x = 2 * np.pi * np.arange(N) / N
+    u = np.zeros((3, N, N, N))
+    u[1] = a * np.sin(k * x)[:, None, None]
+    um = oracle.set_initial(N, u)
+    l = np.arange(1, N // 2 + 1)
+    for p, c in ((4.0, 3.0 / 8.0), (6.0, 5.0 / 16.0)):
+        want = (2 * a * np.abs(np.sin(k * l * (2 * np.pi / N) / 2))) ** p * c / 3.0
+        assert np.abs(oracle.structure_function_p(N, um, p) - want).max() < 1e-13
+    phys = oracle.get_fields(N, uh)
+    for p in (1.0, 3.0, 2.5):
+        want = np.array([sum(np.mean(np.sum((np.roll(phys, -ll, axis=d + 1) - phys) ** 2, axis=0) ** (p / 2)) for d in range(3)) / 3.0
+                         for ll in l])
+        assert np.abs(oracle.structure_function_p(N, uh, p) / want - 1).max() < 1e-12
+
+
 # ------------------------------------------------------------------------------------------- P10
 def test_p10_third_order_in_time(oracle):
     N = 8
