@@ -286,13 +286,14 @@ def main():
         kernels[label] = {"ms_per_launch": ms / cnt, "launches": cnt, "alg_bytes_per_launch": nbytes * args.steps / cnt,
                           "gbs": gbs, "frac": gbs / peak, "share_of_step": ms / (ms_per_step * args.steps), **extra}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_launch"] * kernels[k]["launches"])
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # dram bytes per launch from the committed ncu --set full captures
+    # dram bytes per launch from the committed ncu --set full captures (profiles/traffic.csv), attached to every kernel
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
         for ln in open(tpath).read().splitlines()[1:]:
             f = ln.split(",", 3)
-            if len(f) >= 3 and f[0] == f"{args.workload}_{args.dtype}" and f[1] == dom:
-                traffic = float(f[2])
+            if len(f) >= 3 and f[0] == f"{args.workload}_{args.dtype}" and f[1] in kernels:
+                kernels[f[1]]["traffic"] = float(f[2])
+    traffic = kernels[dom].get("traffic")
     model_bytes = roofline.step_bytes(N, batch, cbytes)
     roof = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
             "frac": kernels[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
