@@ -78,3 +78,32 @@ def test_product_does_not_import_oracle():
                 assert "ns_oracle" not in text and "from oracle" not in text and "import oracle" not in text, f
     otext = open(os.path.join(ROOT, "oracle", "ns_oracle.py")).read() + open(os.path.join(ROOT, "oracle", "ns_oracle.cpp")).read()
     assert "paper_2401_09843_b200" not in otext.replace("paper_2401_09843_b200/csrc/", "")
+
+
+def test_sass_is_blackwell_native():
+    """The built library carries the sm_100a paths the design names (B200_PROFILING.md 'What proves a Blackwell-native
+    kernel'): TMA bulk copies (UBLKCP) in every fused z kernel, tensor-memory parking (STTM / LDTM after a
+    tcgen05.alloc) in the long-line kernels, and no cuFFT / cuBLAS dependency.  Static check with cuobjdump / ldd."""
+    import shutil
+    import subprocess
+    from paper_2401_09843_b200 import binding
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    assert "sm_100a" in sass
+    per_fn, name = {}, None
+    for line in sass.splitlines():
+        if "Function :" in line:
+            name = line.split("Function :")[1].strip()
+            per_fn[name] = set()
+        elif name is not None:
+            for m in ("UBLKCP", "LDTM", "STTM", "UTCATOMSWS", "DFMA"):
+                if m in line:
+                    per_fn[name].add(m)
+    z = {k: v for k, v in per_fn.items() if "z_fused" in k}
+    assert z and all("UBLKCP" in v for v in z.values())
+    tm = {k: v for k, v in per_fn.items() if "z_fused16t" in k or "_tmem_kernel" in k}
+    assert len(tm) >= 6 and all({"LDTM", "STTM", "UTCATOMSWS"} <= v for v in tm.values())
+    ldd = subprocess.run(["ldd", binding.LIB_PATH], capture_output=True, text=True).stdout
+    assert "cufft" not in ldd.lower() and "cublas" not in ldd.lower()
