@@ -1,13 +1,12 @@
-// kernels_zfused16t.cuh -- the 16-values-per-lane fused z kernel (steps a3 + a4, see kernels_zfused16.cuh)
+// kernels_zfused16t.cuh -- steps a3 + a4 of SURVEY.md section 8(a) in one kernel for the longest lines
+// (L = N/2 in {128, 256}): per (px,py) line, pad + inverse c2r along z, the trace-free flux products, max|u|^2,
+// forward r2c + truncate (Algorithm 2 steps 1-5).  16 values per lane (kernels_zfused16.cuh)
 // with the physical-space fields parked in TENSOR MEMORY instead of registers / shared memory.
 //
-// ncu on kernels_zfused16.cuh (profiles/) shows a latency-bound kernel: 9 warps per SM (shared memory and
-// registers both bind), 0.4 eligible warps per scheduler.  Here u1, u2 and u3 on the padded line (48 words per
-// thread in fp64) live in TMEM (tmem.cuh), which costs neither of the two: 128 (fp64) / 64 (fp32) columns per
-// CTA, four CTAs per SM.  Registers then hold only the transform being worked on, and shared memory only the
-// TMA input lines and the exchange / combine regions.
-// The 3 -> 2 combine loop is unrolled with its loads hoisted so that the shared-memory latency of its
-// iterations overlaps.
+// The kernel is latency bound and scales with the number of resident warps (profiles/r01b_tmem.md); registers and
+// shared memory both cap it.  u1, u2 and u3 on the padded line (48 words per thread in fp64) live in TMEM
+// (tmem.cuh), which costs neither: 128 (fp64) / 64 (fp32) columns per CTA, four CTAs per SM.  Registers then hold only
+// the transform being worked on, and shared memory only the TMA input lines and the exchange / combine regions.
 #pragma once
 #include <cstdint>
 

@@ -262,9 +262,13 @@ cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
     if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
     if (L == 128) return z_fused8_L<T, 128>(st, in, out, MM, batch, umax2, tw);
     if (L == 256) return z_fused8_L<T, 256>(st, in, out, MM, batch, umax2, tw);
-#define CALL(LL) z_fused_L<T, LL>(st, in, out, MM, batch, umax2, tw)
-    NS_DISPATCH_L(L, CALL)
-#undef CALL
+    // short lines: block-synchronous kernel
+    switch (L) {
+        case 8: return z_fused_L<T, 8>(st, in, out, MM, batch, umax2, tw);
+        case 16: return z_fused_L<T, 16>(st, in, out, MM, batch, umax2, tw);
+        case 32: return z_fused_L<T, 32>(st, in, out, MM, batch, umax2, tw);
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 #define NS_INSTANTIATE_FFT(T)                                                                                      \
