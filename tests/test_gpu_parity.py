@@ -192,6 +192,33 @@ def test_ensemble_moments(ns, oracle):
     assert var.max() < 1e-28 and np.abs(mean - f[0]).max() < 1e-13
 
 
+def test_two_handles_on_two_streams(ns):
+    """Handles are independent (include/ns.h): two solvers stepping concurrently on two streams -- their tensor-memory
+    kernels share the SMs' 512 TMEM columns -- give bit for bit what each gives alone."""
+    import torch
+    N = 256
+    ua = inputs.taylor_green_3d_perturbed(N, 21)[None]
+    ub = inputs.cylindrical_shear(N, 22, rho=0.1)[None]
+    kw = dict(eps=0.05, s=1.0)
+    ref = []
+    for u in (ua, ub):
+        s = ns.Solver(N, **kw)
+        s.set_initial(u)
+        for _ in range(3):
+            s.step(1e-3)
+        ref.append(s.get_spectral())
+        del s
+    st = [torch.cuda.Stream(), torch.cuda.Stream()]
+    sol = [ns.Solver(N, stream=st[i].cuda_stream, **kw) for i in range(2)]
+    sol[0].set_initial(ua)
+    sol[1].set_initial(ub)
+    for _ in range(3):
+        for s in sol:
+            s.step(1e-3)          # asynchronous launches on the handle's stream
+    got = [s.get_spectral() for s in sol]
+    assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1])
+
+
 def test_batch_is_bitwise_independent(ns):
     """Reading A18: a batched launch gives bit for bit the per-sample result of batch = 1."""
     N, B = 32, 5
