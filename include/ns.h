@@ -99,6 +99,12 @@ int ns_step_cfl(ns_solver* h, double cfl, double t_end, double* dt_out);
 /* One SSP-RK3 step with caller-given per-sample steps dt[batch] (host array); dt_b == 0 leaves
  * sample b untouched.  Used to replay a recorded CFL sequence. */
 int ns_step_dts(ns_solver* h, const double* dt);
+/* Integrate every sample to t_end (Algorithm 1 line "evolve the sample"; BASELINE configs[3]:
+ * "integrated to t=1 at CFL 0.2"): repeated ns_step_cfl(cfl, t_end) without a host round trip per step; the host
+ * reads the sample times every fourth step and stops when all have reached t_end or after max_steps steps.
+ * *steps_done (may be NULL) = RK3 steps launched; steps issued after a sample has finished leave it untouched.
+ * NS_ERR_INVALID_ARG for cfl <= 0 or max_steps < 0. */
+int ns_advance(ns_solver* h, double cfl, double t_end, int max_steps, int* steps_done);
 
 /* umax_out[batch] (host): max over the padded M^3 grid of the Euclidean |u| of the current state. */
 int ns_max_velocity(ns_solver* h, double* umax_out);

@@ -21,7 +21,7 @@ NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE = 0, -1, -2, -3
 
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
-    "ns_step_cfl", "ns_step_dts", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
+    "ns_step_cfl", "ns_step_dts", "ns_advance", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
     "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
 
@@ -58,6 +58,7 @@ def lib():
         L.ns_step.argtypes = [vp, d]
         L.ns_step_cfl.argtypes = [vp, d, d, vp]
         L.ns_step_dts.argtypes = [vp, vp]
+        L.ns_advance.argtypes = [vp, d, d, i, ctypes.POINTER(ctypes.c_int)]
         L.ns_max_velocity.argtypes = [vp, vp]
         L.ns_get_fields.argtypes = [vp, vp, i]
         L.ns_energy_spectrum.argtypes = [vp, vp, i]
@@ -211,6 +212,12 @@ class Solver:
         E = np.empty((self.batch, int(nbins)), dtype=np.float64)
         self._check(lib().ns_energy_spectrum(self._h, ctypes.c_void_p(E.ctypes.data), int(nbins)))
         return E
+
+    def advance(self, cfl, t_end, max_steps=1 << 30):
+        """Integrate every sample to t_end at the given CFL number; returns the number of RK3 steps launched."""
+        n = ctypes.c_int(0)
+        self._check(lib().ns_advance(self._h, float(cfl), float(t_end), int(max_steps), ctypes.byref(n)))
+        return n.value
 
     def structure_function_p(self, p, nl=None):
         nl = self.N // 2 if nl is None else int(nl)

@@ -27,6 +27,7 @@ struct ns_solver {
     virtual int step_uniform(double dt) = 0;
     virtual int step_cfl(double cfl, double t_end, double* dt_out) = 0;
     virtual int step_dts(const double* dt) = 0;
+    virtual int advance(double cfl, double t_end, int max_steps, int* steps_done) = 0;
     virtual int max_velocity(double* out) = 0;
     virtual int get_fields(void* out, ns_memspace ms) = 0;
     virtual int energy_spectrum(double* E, int nbins, bool enstrophy) = 0;
@@ -296,6 +297,28 @@ public:
             NS_CK(cudaMemcpyAsync(dt_out, dt_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
             NS_CK(cudaStreamSynchronize(st));
         }
+        return NS_OK;
+    }
+
+    int advance(double cfl, double t_end, int max_steps, int* steps_done) override {
+        if (!(cfl > 0.0) || max_steps < 0 || !(t_end == t_end)) return fail(NS_ERR_INVALID_ARG, "need cfl > 0, max_steps >= 0, finite t_end");
+        if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
+        std::vector<double> th((size_t)batch);
+        int n = 0;
+        while (n < max_steps) {
+            NS_CK(cudaMemcpyAsync(th.data(), t_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
+            NS_CK(cudaStreamSynchronize(st));
+            bool done = true;
+            for (double tb : th) done = done && !(tb < t_end);
+            if (done) break;
+            const int burst = max_steps - n < 4 ? max_steps - n : 4;
+            for (int i = 0; i < burst; ++i) {
+                int rc = rk3(DT_CFL, 0, nullptr, cfl, t_end);
+                if (rc != NS_OK) return rc;
+            }
+            n += burst;
+        }
+        if (steps_done) *steps_done = n;
         return NS_OK;
     }
 
@@ -583,6 +606,7 @@ int ns_rhs(ns_solver* h, void* out, ns_memspace ms) { NS_H(h); return h->rhs(out
 int ns_step(ns_solver* h, double dt) { NS_H(h); return h->step_uniform(dt); }
 int ns_step_cfl(ns_solver* h, double cfl, double t_end, double* dt_out) { NS_H(h); return h->step_cfl(cfl, t_end, dt_out); }
 int ns_step_dts(ns_solver* h, const double* dt) { NS_H(h); return h->step_dts(dt); }
+int ns_advance(ns_solver* h, double cfl, double t_end, int max_steps, int* steps_done) { NS_H(h); return h->advance(cfl, t_end, max_steps, steps_done); }
 int ns_max_velocity(ns_solver* h, double* out) { NS_H(h); return h->max_velocity(out); }
 int ns_get_fields(ns_solver* h, void* out, ns_memspace ms) { NS_H(h); return h->get_fields(out, ms); }
 int ns_energy_spectrum(ns_solver* h, double* E, int nbins) { NS_H(h); return h->energy_spectrum(E, nbins, false); }

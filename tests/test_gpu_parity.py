@@ -219,6 +219,29 @@ def test_two_handles_on_two_streams(ns):
     assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1])
 
 
+def test_advance_to_t_end(ns):
+    """ns_advance == the host loop over ns_step_cfl it replaces, bit for bit, with every sample ending at t_end."""
+    N, B, t_end = 32, 3, 0.05
+    us = np.stack([field(N, 600 + i) * (1.0 + i) for i in range(B)])
+    kw = dict(eps=0.05, s=1.5)
+    a = ns.Solver(N, batch=B, **kw)
+    a.set_initial(us)
+    steps = 0
+    while min(a.time(b) for b in range(B)) < t_end:
+        a.step_cfl(0.2, t_end, return_dt=False)
+        steps += 1
+    b_ = ns.Solver(N, batch=B, **kw)
+    b_.set_initial(us)
+    n = b_.advance(0.2, t_end)
+    assert steps <= n <= steps + 3 and steps > 5
+    assert all(abs(b_.time(i) - t_end) < 1e-15 for i in range(B))
+    assert np.array_equal(a.get_spectral(), b_.get_spectral())
+    assert b_.advance(0.2, t_end) == 0                       # already there
+    c = ns.Solver(N, batch=B, **kw)
+    c.set_initial(us)
+    assert c.advance(0.2, t_end, max_steps=2) == 2 and c.time(0) < t_end
+
+
 def test_batch_is_bitwise_independent(ns):
     """Reading A18: a batched launch gives bit for bit the per-sample result of batch = 1."""
     N, B = 32, 5
