@@ -384,6 +384,35 @@ def test_config4_ensemble_two_samples(ns, oracle):
     assert len(set(np.round(dts, 12))) > 1          # distinct seeds -> distinct steps
 
 
+def test_config4_ensemble_to_t1(ns):
+    """BASELINE.json configs[3] at full length: the 32 x 128^3 shear-layer ensemble integrated to t = 1 at CFL 0.2 in one
+    batched run (ns_advance).  The oracle needs hours for this horizon (its parity over the first step is
+    test_config4_ensemble_two_samples), so this checks what must hold at any length: every sample ends at t = 1,
+    sample 7 of the batch equals bit for bit the same sample integrated alone (reading A18), the energy of every sample
+    has not grown, the ensemble statistics are finite, and the two independent routes to S_2 (spectral identity and
+    physical-space increments) agree."""
+    N, B = 128, 32
+    us = inputs.shear_layer_ensemble(N, B, seed0=1000)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, batch=B, **kw)
+    s.set_initial(us)
+    E0 = s.energy_spectrum(N).sum(axis=1)
+    n = s.advance(0.2, 1.0)
+    assert 20 < n < 2000 and all(abs(s.time(b) - 1.0) < 1e-14 for b in range(B))
+    E = s.energy_spectrum(N)
+    assert np.isfinite(E).all() and np.all(E.sum(axis=1) <= E0 * (1 + 1e-12)) and np.all(E.sum(axis=1) > 0.5 * E0)
+    S2 = s.structure_function(nl=16)
+    assert np.abs(s.structure_function_p(2.0, nl=16) / S2 - 1).max() < 1e-10
+    mean, var = s.ensemble_moments()
+    assert np.isfinite(mean).all() and var.max() > 1e-4          # distinct seeds decorrelate the samples
+    Emean = E.mean(axis=0)                                       # the reported ensemble-mean spectrum
+    assert Emean[1:4].sum() > 0.5 * Emean.sum()                  # the shear layer keeps its energy at the largest scales
+    one = ns.Solver(N, batch=1, **kw)
+    one.set_initial(us[7:8])
+    one.advance(0.2, 1.0)
+    assert np.array_equal(one.get_spectral()[0], s.get_spectral()[7])
+
+
 # ---------------------------------------------------------------------- invariants run on the GPU path
 def test_gpu_invariants(ns):
     N = 32
