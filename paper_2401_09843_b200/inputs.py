@@ -133,7 +133,7 @@ def gaussian_k53(N: int = 512, seed: int = 5) -> np.ndarray:
     """Config 5: E(k) ~ k^(-5/3) on 1 <= k <= N/3, zero elsewhere, total energy 0.5."""
     def spec(k):
         with np.errstate(divide="ignore"):
-            return np.where((k >= 1.0) & (k <= N / 3.0), np.power(np.maximum(k, 1e-300), -5.0 / 3.0), 0.0)
+            return np.where((k >= 1.0) & (k <= N / 3.0), np.power(np.maximum(k, 1.0), -5.0 / 3.0), 0.0)
     return gaussian_field(N, seed, spec, e_tot=0.5)
 
 
