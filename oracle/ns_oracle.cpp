@@ -11,7 +11,7 @@
 //     eq. (2.5)        PAPER.md:L122-126  Leray-projected spectral time derivative
 //     Algorithm 2      PAPER.md:L128-136  pad -> iFFT -> u(x)u -> FFT -> dealias -> d/dt u_hat
 //     eq. (2.6)        PAPER.md:L146-153  third-order SSP Runge-Kutta
-// Readings of points where the paper is silent (A1..A18) are listed in DESIGN.md section 3.
+// Readings of points where the paper is silent (A1..A20) are listed in DESIGN.md section 3.
 //
 // Deliberately naive: every 3-D transform is a FULL complex transform on the padded M^3 grid
 // (no r2c tricks, no pruning, no fusion), 1-D transforms are a textbook recursive
@@ -22,7 +22,9 @@
 // convolution; P2 Taylor-Green / ABC project to zero; P3 RK3 decay closed form; P4 energy identity;
 // P5 div-free; P6 Galilean shift; P7 padding independence; P8 spectrum/Parseval; P9 structure
 // function identity; P10 temporal order 3; P11 hyperviscous single mode; P12 orc_rhs_at_modes (direct
-// truncated convolution at sampled wavenumbers) vs the step-by-step RHS and vs the test's own O(N^6) sum.
+// truncated convolution at sampled wavenumbers) vs the step-by-step RHS and vs the test's own O(N^6) sum;
+// P13 orc_max_velocity / rhs_parts' umax: constant field (Euclidean norm of all three components), a cosine whose
+// maximum lies on the padded grid only, and a zero-padded numpy.fft.irfftn of a random state.
 // "parity unpinned" against the authors' code (the paper gives no formula): the readings A3
 // (Nyquist planes zero), A5 (form of Q_k), A6 (constants), A10 (CFL formula), A14 (energy-spectrum
 // binning), A15 (structure function) -- they are pinned for self-consistency only.

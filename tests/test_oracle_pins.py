@@ -445,3 +445,70 @@ def test_max_velocity_and_padding(oracle):
     # |u|^2 = sin^2 x cos^2 y + cos^2 x sin^2 y <= 1, attained at x = pi/2, y = 0 (on the 12-point padded grid too)
     assert abs(oracle.max_velocity(N, uh) - 1.0) < 1e-14
     assert abs(oracle.rhs_parts(N, oracle.Params(), uh)["umax"] - 1.0) < 1e-14
+
+
+def _both_umax(oracle, N, uh):
+    a = oracle.max_velocity(N, uh)
+    b = oracle.rhs_parts(N, oracle.Params(), uh)["umax"]
+    assert a == b          # the two entry points evaluate the same definition
+    return a
+
+
+def test_p13_max_velocity_is_euclidean_norm_of_all_three_components(oracle):
+    """Pin of reading A10 / SURVEY.md 8(c) item 10, part (i): a constant field U has umax = |U|_2 exactly.  Fails for a
+    dropped component (0.3, -0.7 only -> 0.7616), for the max-component norm (0.7) and for the 1-norm (1.45)."""
+    N = 8
+    U = np.array([0.3, -0.7, 0.45])
+    uh = np.zeros(oracle.spectral_shape(N), dtype=np.complex128)
+    uh[:, 0, 0, 0] = U
+    assert abs(_both_umax(oracle, N, uh) - np.sqrt(0.09 + 0.49 + 0.2025)) < 1e-15
+    # and with the third component alone (a field whose u1 = u2 = 0)
+    uh[:2] = 0
+    assert abs(_both_umax(oracle, N, uh) - 0.45) < 1e-15
+
+
+def test_p13_max_velocity_is_taken_on_the_padded_grid(oracle):
+    """Part (ii): u = (0, 0, cos(x - 2 pi/12)) at N = 8.  Its maximum 1 is attained at x = 2 pi/12, a point of the 12-point
+    padded grid that is NOT on the 8-point grid, where the maximum is cos(pi/12) = 0.96593 (at x = 0 and x = 2 pi/8).
+    Fails when the maximum is taken over the N grid instead of the M = 3N/2 grid."""
+    N = 8
+    x = 2 * np.pi * np.arange(N) / N
+    u = np.zeros((3, N, N, N))
+    u[2] = np.cos(x - 2 * np.pi / 12)[:, None, None]
+    assert abs(np.abs(u[2]).max() - np.cos(np.pi / 12)) < 1e-15
+    uh = oracle.set_initial(N, u)               # a z-directed shear depending on x only is solenoidal: unchanged
+    assert abs(_both_umax(oracle, N, uh) - 1.0) < 1e-14
+    # the same along y and z (u1 depending on y, u2 depending on z) -- catches an axis handled on the wrong grid
+    u = np.zeros((3, N, N, N))
+    u[0] = np.cos(x - 2 * np.pi / 12)[None, :, None]
+    assert abs(_both_umax(oracle, N, oracle.set_initial(N, u)) - 1.0) < 1e-14
+    u = np.zeros((3, N, N, N))
+    u[1] = np.cos(x - 2 * np.pi / 12)[None, None, :]
+    assert abs(_both_umax(oracle, N, oracle.set_initial(N, u)) - 1.0) < 1e-14
+
+
+@pytest.mark.parametrize("N", [8, 12, 16])
+def test_p13_max_velocity_vs_zero_padded_numpy_irfftn(oracle, N):
+    """Part (iii): a random solenoidal state exciting every active mode, evaluated on the M = 3N/2 grid by a zero-padded
+    numpy.fft.irfftn written here (library routine as a second witness), Euclidean norm, maximum over the grid."""
+    uh = full_state(oracle, N, 900 + N)
+    M = 3 * N // 2
+    pad = np.zeros((3, M, M, M // 2 + 1), dtype=np.complex128)
+    K = N // 2 - 1
+    for ix in range(N):
+        kx = ix if ix < N // 2 else ix - N
+        if abs(kx) > K:
+            continue
+        for iy in range(N):
+            ky = iy if iy < N // 2 else iy - N
+            if abs(ky) > K:
+                continue
+            pad[:, kx % M, ky % M, :K + 1] = uh[:, ix, iy, :K + 1]
+    phys = np.fft.irfftn(pad, s=(M, M, M), axes=(1, 2, 3)) * M ** 3    # unnormalised synthesis sum_k u_hat e^{ikx}
+    want = np.sqrt((phys ** 2).sum(axis=0)).max()
+    got = _both_umax(oracle, N, uh)
+    assert abs(got - want) < 1e-13 * want
+    # the maximum over the N grid differs (so the pin discriminates) and so do the other norms
+    coarse = np.sqrt((oracle.get_fields(N, uh) ** 2).sum(axis=0)).max()
+    assert abs(coarse - want) > 1e-6 * want
+    assert abs(np.abs(phys).max() - want) > 1e-6 * want
