@@ -34,32 +34,34 @@ from paper_2401_09843_b200 import inputs, roofline  # noqa: E402
 WORKLOADS = {
     # name: (BASELINE.json configs index, N, batch, params, cfl, description, cpu sample N)
     "c1": dict(cfg=0, N=32, batch=1, params=dict(nu=0.01), dt=1e-3, desc="configs[0]: 32^3 Taylor-Green + 1e-3 noise, nu=0.01, dt=1e-3", cpuN=32),
-    "c2": dict(cfg=1, N=128, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[1]: 128^3 Gaussian k^4 exp, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=64),
-    "c3": dict(cfg=2, N=256, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[2]: 256^3 perturbed shear layer, hyperviscosity, CFL 0.2", cpuN=64),
-    "c4": dict(cfg=3, N=128, batch=32, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[3]: 32 x 128^3 shear-layer ensemble in one launch, CFL 0.2", cpuN=64),
+    "c2": dict(cfg=1, N=128, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[1]: 128^3 Gaussian k^4 exp, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=128),
+    "c3": dict(cfg=2, N=256, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[2]: 256^3 perturbed shear layer, hyperviscosity, CFL 0.2", cpuN=128),
+    "c4": dict(cfg=3, N=128, batch=32, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[3]: 32 x 128^3 shear-layer ensemble in one launch, CFL 0.2", cpuN=128),
     # the paper's own experiments, hyperviscosity order s = 1.5
-    "tg3d": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.1-6.3: 256^3 perturbed 3-D Taylor-Green, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=64),
-    "cyl": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.4-6.6: 256^3 cylindrical shear flow rho=0.05, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=64),
-    "c5": dict(cfg=4, N=512, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[4]: 512^3 Gaussian k^-5/3, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=64),
+    "tg3d": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.1-6.3: 256^3 perturbed 3-D Taylor-Green, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=128),
+    "cyl": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.4-6.6: 256^3 cylindrical shear flow rho=0.05, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=128),
+    "c5": dict(cfg=4, N=512, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[4]: 512^3 Gaussian k^-5/3, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=128),
 }
 
 
-def make_input(name: str, N: int, batch: int) -> np.ndarray:
-    """Physical-space samples [batch][3][N][N][N] of the workload recipe at grid size N."""
+def make_input(name: str, N: int, batch: int, rank: int = 0) -> np.ndarray:
+    """Physical-space samples [batch][3][N][N][N] of the workload recipe at grid size N.  Under torchrun every rank draws
+    its own Monte-Carlo samples (Algorithm 1): the seeds are offset by 10007 * rank."""
+    o = 10007 * rank
     if name == "c1":
-        return inputs.taylor_green_perturbed(N, seed=1)[None]
+        return inputs.taylor_green_perturbed(N, seed=1 + o)[None]
     if name == "c2":
-        return inputs.gaussian_k4(N, seed=2)[None]
+        return inputs.gaussian_k4(N, seed=2 + o)[None]
     if name == "c3":
-        return inputs.shear_layer(N, seed=3)[None]
+        return inputs.shear_layer(N, seed=3 + o)[None]
     if name == "c4":
-        return inputs.shear_layer_ensemble(N, batch, seed0=1000)
+        return inputs.shear_layer_ensemble(N, batch, seed0=1000 + o)
     if name == "c5":
-        return inputs.gaussian_k53(N, seed=5)[None]
+        return inputs.gaussian_k53(N, seed=5 + o)[None]
     if name == "tg3d":
-        return inputs.taylor_green_3d_perturbed(N, seed=6)[None]
+        return inputs.taylor_green_3d_perturbed(N, seed=6 + o)[None]
     if name == "cyl":
-        return inputs.cylindrical_shear(N, seed=7, rho=0.05)[None]
+        return inputs.cylindrical_shear(N, seed=7 + o, rho=0.05)[None]
     raise KeyError(name)
 
 
@@ -70,8 +72,30 @@ def dist_env():
     return rank, world, local
 
 
+def init_dist(world: int):
+    """Process group for the N > 1 plumbing (barrier + max / sum of two host scalars; no data-path collective).  With GPUs:
+    NCCL for CUDA tensors and gloo for the host scalars in ONE group; without (the CPU test): gloo only.  The same
+    function is used by bench.py under torchrun and by tests/test_bench_host.py."""
+    if world == 1:
+        return None
+    import torch
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    backend = "cpu:gloo,cuda:nccl" if torch.cuda.is_available() else "gloo"
+    if not dist.is_initialized():
+        dist.init_process_group(backend)
+    return dist
+
+
+def host_barrier(dist):
+    """Barrier over the host (gloo) side of the group: an all-reduce of a CPU scalar."""
+    if dist is not None:
+        import torch
+        dist.all_reduce(torch.zeros(1, dtype=torch.float64))
+
+
 def aggregate(local_ms_total: float, local_units: float, world: int, dist=None):
-    """Max-over-ranks time and summed units (host logic; covered by a gloo world_size-2 CPU test)."""
+    """Max-over-ranks time and summed units; CPU tensors, i.e. the gloo side of the group."""
     if world == 1 or dist is None:
         return local_ms_total, local_units
     import torch
@@ -136,7 +160,9 @@ class ClockSampler:
 
 
 def cpu_oracle_run(name: str, steps: int, warmup: int = 0):
-    """Time the oracle, as it stands, on a bounded sample of the workload: RK3 steps at a reduced grid."""
+    """Time the oracle, as it stands, on a bounded sample of the workload: RK3 steps of ONE sample of the same recipe on
+    a grid of at most 128^3 (a 512^3 oracle step needs ~28 GB and a quarter of an hour; its cost per grid point grows only
+    with log N).  A reported baseline for context -- a deliberately naive program -- never a speed-up denominator."""
     from oracle import ns_oracle
     w = WORKLOADS[name]
     Ns = w["cpuN"]
@@ -151,7 +177,8 @@ def cpu_oracle_run(name: str, steps: int, warmup: int = 0):
         uh = ns_oracle.step(Ns, p, uh, dt)
     el = time.perf_counter() - t0
     value = roofline.grid_point_stages(Ns, 1, steps) / el
-    sample = f"{steps} RK3 step(s) of the {name} recipe on a {Ns}^3 grid (1 sample), fp64, naive radix-2/3 FFT, OpenMP"
+    sample = (f"{steps} RK3 step(s) of one sample of the {name} recipe on a {Ns}^3 grid (workload grid {w['N']}^3 x {w['batch']}), "
+              "fp64, full-complex padded transforms with a naive recursive radix-2/3 FFT, OpenMP over lines")
     return dict(value=value, unit="grid-point-stages/s", cores=ns_oracle.num_threads(), kind="oracle", sample=sample,
                 seconds=el, steps_per_s=steps / el), el / steps * 1e3
 
@@ -175,45 +202,28 @@ def run_reference(args):
     return 0
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
-    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=3)
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-    if args.warmup < 3:
-        args.warmup = 3  # timing rule: at least 3 warm-up steps
+PROF_LABEL = {"a1_col_inv_x": "a1_col_inv_x", "a2_col_inv_y": "a2_col_inv_y", "a3_z_inv_prod": "a3a4_z_fused",
+              "a5_col_fwd_y": "a5_col_fwd_y", "a6_col_fwd_x": "a6_col_fwd_x", "a7_spectral": "a7_spectral"}
 
-    import torch
-    rank, world, local = dist_env()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist  # plumbing only: barrier + max/sum of two scalars
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl")
-    from paper_2401_09843_b200 import binding
 
-    w = WORKLOADS[args.workload]
+def run_workload(binding, torch, name, dtype, steps, warmup, dist, world, rank, local, state=None, split_steps=None):
+    """Time `steps` RK3 steps of one workload with the state resident in HBM (CUDA events on the solver's stream, per-pass
+    profiler OFF), then a second short run with the per-pass event profiler ON for the split.  Returns (record, solver,
+    extras); the caller owns the solver."""
+    w = WORKLOADS[name]
     N, batch = w["N"], w["batch"]
-    cbytes = 16 if args.dtype == "f64" else 8
+    cbytes = 16 if dtype == "f64" else 8
     t_gen = time.perf_counter()
-    u0 = make_input(args.workload, N, batch)
+    s = binding.Solver(N, batch=batch, dtype=dtype, **w["params"])
+    if state is None:
+        u0 = make_input(name, N, batch, rank)
+        chk = inputs.checksum(u0[0, 0, :2])
+        s.set_initial(u0)
+        del u0
+    else:
+        s.set_spectral(state.astype(s.cplx))
+        chk = "state of the f64 run of the same workload"
     t_gen = time.perf_counter() - t_gen
-    s = binding.Solver(N, batch=batch, dtype=args.dtype, **w["params"])
-    s.set_initial(u0)
-    chk = inputs.checksum(u0[0, 0, :2])
-    del u0
 
     def one_step():
         if "dt" in w:
@@ -227,17 +237,15 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
+        host_barrier(dist)
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         one_step()
     barrier()
-    s.profile(True)
     launches0 = s.kernel_launches()
     sampler = ClockSampler(local)
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps if flush else 1)]
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps if flush else 1)]
     barrier()
     if flush:
         for a, b in evs:
@@ -247,75 +255,120 @@ def main():
             b.record()
     else:
         evs[0][0].record()
-        for _ in range(args.steps):
+        for _ in range(steps):
             one_step()
         evs[0][1].record()
     barrier()
     total_ms = sum(a.elapsed_time(b) for a, b in evs)
     clocks = sampler.stop()
     launches = s.kernel_launches() - launches0
+    # per-pass split: a second, short run with one event record between the kernels (not part of the timed value)
+    nsplit = split_steps or min(steps, 5)
+    s.profile(True)
+    for _ in range(nsplit):
+        if flush:
+            flush_buf.fill_(1)
+        one_step()
     prof = s.profile_read()
     s.profile(False)
-    finite = bool(np.isfinite(s.max_velocity()).all())
+    E = s.energy_spectrum(min(N, 4096))
+    finite = bool(np.isfinite(E).all() and (E.sum(axis=1) > 0).all())   # finiteness of the STATE itself
 
-    total_ms, units = aggregate(total_ms, roofline.grid_point_stages(N, batch, args.steps), world, dist)
-    ms_per_step = total_ms / args.steps
+    total_ms, units = aggregate(total_ms, roofline.grid_point_stages(N, batch, steps), world, dist)
+    ms_per_step = total_ms / steps
     value = units / (total_ms * 1e-3)
 
-    # ---- roofline of the dominant kernel and of the whole step (fixed model)
     peak, peak_src = measured_peaks()
     per_step = roofline.pass_bytes_per_step(N, batch, cbytes)        # fixed model
     built = roofline.built_pass_bytes_per_step(N, batch, cbytes)     # what the built kernels must move
-    prof_label = {"a1_col_inv_x": "a1_col_inv_x", "a2_col_inv_y": "a2_col_inv_y", "a3_z_inv_prod": "a3a4_z_fused",
-                  "a5_col_fwd_y": "a5_col_fwd_y", "a6_col_fwd_x": "a6_col_fwd_x", "a7_spectral": "a7_spectral"}
+    split_ms = sum(prof[k][0] for k in PROF_LABEL) / nsplit
     kernels = {}
-    for name, label in prof_label.items():
-        ms, cnt = prof[name]
+    for pname, label in PROF_LABEL.items():
+        ms, cnt = prof[pname]
         if not cnt:
             continue
         nbytes, extra = built[label], {}
-        if label == "a3a4_z_fused":
-            # the fixed model charges a3 + a4 separately (six M^3 products written and read back)
-            model = per_step["a3_z_inv_prod"] + per_step["a4_z_fwd"]
-        else:
-            model = per_step[name]
+        model = per_step["a3_z_inv_prod"] + per_step["a4_z_fwd"] if label == "a3a4_z_fused" else per_step[pname]
         if model != nbytes:
-            extra = {"model_bytes_per_launch": model * args.steps / cnt,
-                     "model_gbs_equivalent": model * args.steps / (ms * 1e-3) / 1e9}
-        gbs = nbytes * args.steps / (ms * 1e-3) / 1e9
-        kernels[label] = {"ms_per_launch": ms / cnt, "launches": cnt, "alg_bytes_per_launch": nbytes * args.steps / cnt,
-                          "gbs": gbs, "frac": gbs / peak, "share_of_step": ms / (ms_per_step * args.steps), **extra}
+            extra = {"fixed_model_bytes_per_launch": model * nsplit / cnt}
+        gbs = nbytes * nsplit / (ms * 1e-3) / 1e9
+        kernels[label] = {"ms_per_launch": ms / cnt, "launches": cnt, "alg_bytes_per_launch": nbytes * nsplit / cnt,
+                          "gbs": gbs, "frac": gbs / peak, "share_of_step": ms / nsplit / split_ms, **extra}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_launch"] * kernels[k]["launches"])
-    # dram bytes per launch from the committed ncu --set full captures (profiles/traffic.csv), attached to every kernel
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
         for ln in open(tpath).read().splitlines()[1:]:
             f = ln.split(",", 3)
-            if len(f) >= 3 and f[0] == f"{args.workload}_{args.dtype}" and f[1] in kernels:
+            if len(f) >= 3 and f[0] == f"{name}_{dtype}" and f[1] in kernels:
                 kernels[f[1]]["traffic"] = float(f[2])
-    traffic = kernels[dom].get("traffic")
-    model_bytes = roofline.step_bytes(N, batch, cbytes)
     roof = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-            "frac": kernels[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+            "frac": kernels[dom]["frac"], "traffic": kernels[dom].get("traffic"), "peak_source": peak_src,
             "alg_bytes_per_launch": kernels[dom]["alg_bytes_per_launch"], "ms_per_launch": kernels[dom]["ms_per_launch"]}
     if dom == "a3a4_z_fused":
-        roof["note"] = ("fused a3+a4: by bytes HBM is the roofline (DRAM traffic = algorithmic 8*A2), but ncu shows a latency / "
-                        "fp64-issue limited kernel (c5: fp64 pipe 44 %, l1tex 63 %, DRAM 23 % busy; profiles/r01b_tmem.md); the "
-                        "unfused a3 + a4 of the fixed model would need model_bytes_per_launch / peak = "
-                        f"{kernels[dom]['model_bytes_per_launch'] / (peak * 1e9) * 1e3:.2f} ms at the measured peak")
-    step_roof = {"model_bytes_per_step": model_bytes, "achieved_gbs": model_bytes / (ms_per_step * 1e-3) / 1e9,
-                 "frac_of_measured_peak": model_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
-                 "frac_of_nominal_8TBs": model_bytes / (ms_per_step * 1e-3) / 1e9 / 8000.0,
-                 "t_model_ms_at_measured_peak": model_bytes / (peak * 1e9) * 1e3}
+        roof["note"] = ("fused a3+a4: by bytes HBM is the roofline (DRAM traffic = algorithmic 8*A2), but the kernel is bound by "
+                        "fp64 issue / latency, not by HBM (profiles/); frac is bytes the kernel must move / time / measured peak")
     actual = roofline.actual_step_bytes(N, batch, cbytes)
-    step_roof["actual_bytes_per_step"] = actual
-    step_roof["actual_frac_of_measured_peak"] = actual / (ms_per_step * 1e-3) / 1e9 / peak
-    step_roof["note"] = ("a3+a4 are one kernel (products never reach HBM) and 5 trace-free flux components are transformed "
-                         "instead of 6: frac_* use the FIXED model bytes of SURVEY.md 8(d); actual_* use the bytes the "
-                         "built pass structure must move")
+    model_bytes = roofline.step_bytes(N, batch, cbytes)
+    step_roof = {
+        "bound": "hbm", "bytes_per_step": actual, "achieved_gbs": actual / (ms_per_step * 1e-3) / 1e9, "peak": peak,
+        "frac": actual / (ms_per_step * 1e-3) / 1e9 / peak,
+        "frac_of_nominal_8TBs": actual / (ms_per_step * 1e-3) / 1e9 / 8000.0,
+        "note": "frac = bytes the BUILT pass structure must move per RK3 step (a3+a4 fused: products never reach HBM; 5 trace-free "
+                "flux components) / measured time / measured HBM peak -- the HBM utilisation of the step",
+        "fixed_model": {
+            "bytes_per_step": model_bytes, "t_model_ms_at_measured_peak": model_bytes / (peak * 1e9) * 1e3,
+            "speed_ratio_vs_model_at_measured_peak": model_bytes / (peak * 1e9) * 1e3 / ms_per_step,
+            "speed_ratio_vs_model_at_nominal_8TBs": model_bytes / 8e12 * 1e3 / ms_per_step,
+            "note": "SURVEY.md 8(d) fixed reference model (unfused a3 / a4, six products): T_model / T_measured, a SPEED ratio against "
+                    "a pass structure that moves more bytes than this one -- it can exceed 1 and is not an HBM utilisation"},
+    }
+    rec = {"workload": name, "dtype": dtype, "ms_per_step": ms_per_step, "value": value, "unit": "grid-point-stages/s",
+           "steps": steps, "steps_per_s": 1e3 / ms_per_step * world, "step_roofline": step_roof, "roofline": roof,
+           "kernels": kernels, "clocks": clocks, "gpu_launches": launches, "state_finite": finite,
+           "l2": "L2 flushed (256 MiB write) between timed steps" if flush else "inputs exceed L2 (126 MB): no flush needed",
+           "input_checksum": chk, "setup_s": round(t_gen, 1), "device_bytes": s.device_bytes(),
+           "profiler": f"timed region: per-pass profiler off; split from {nsplit} further step(s) with one event record per kernel"}
+    return rec, s, one_step
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the sub-records of the other north-star targets")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+
+    import torch
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = init_dist(world)   # plumbing only: barrier + max/sum of two scalars
+    if dist is not None:      # one NCCL collective so that a broken NVLink / NCCL setup fails here, not silently
+        x = torch.ones(1, device="cuda")
+        dist.all_reduce(x)
+        assert int(x.item()) == world
+    from paper_2401_09843_b200 import binding
+
+    w = WORKLOADS[args.workload]
+    N, batch = w["N"], w["batch"]
+    cbytes = 16 if args.dtype == "f64" else 8
+    rec, s, one_step = run_workload(binding, torch, args.workload, args.dtype, args.steps, args.warmup, dist, world, rank, local)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D state, step, D2H state, every step
     e2e = None
+    state64 = None
     if not args.no_e2e:
         shape = s.spectral_shape
         ct = torch.complex128 if args.dtype == "f64" else torch.complex64
@@ -325,7 +378,8 @@ def main():
         s.get_spectral(a_in)
         for _ in range(1):
             s.set_spectral(a_in); one_step(); s.get_spectral(a_out)
-        barrier()
+        torch.cuda.synchronize()
+        host_barrier(dist)
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):
             s.set_spectral(a_in)
@@ -339,29 +393,45 @@ def main():
         e2e = {"value": eunits / (el * 1e-3), "unit": "grid-point-stages/s", "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "ms_per_step": el / args.e2e_steps, "steps": args.e2e_steps,
                "api": "ns_set_spectral(NS_HOST) + ns_step_cfl + ns_get_spectral(NS_HOST), pinned host buffers"}
+        del h_in, h_out, a_in, a_out
+
+    # ---- the other north-star targets in the same invocation (BASELINE.json: "the 512^3 single-sample and the 32 x 128^3
+    #      ensemble"; configs[4]: "plus the same run in fp32"), 10 steps each, as sub-records
+    also = {}
+    if args.workload == "c5" and args.dtype == "f64" and not args.no_also:
+        state64 = s.get_spectral()
+        del s
+        r32, s32, _ = run_workload(binding, torch, "c5", "f32", 10, 3, dist, world, rank, local, state=state64)
+        del s32, state64
+        also["c5_f32"] = r32
+        r4, s4, _ = run_workload(binding, torch, "c4", "f64", 10, 3, dist, world, rank, local)
+        del s4
+        also["c4_f64"] = r4
+    else:
+        del s
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        nst = 20 if args.workload == "c1" else 12   # about 10 s on the GPU box's 16 cores, 30 s on 8
+        nst = 20 if args.workload == "c1" else 3   # 128^3: about 6 s per step on the GPU box's 16 cores
         cpu, _ = cpu_oracle_run(args.workload, nst)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "seconds")}
 
     if rank == 0:
         line = {
-            "metric": "grid_point_stages_per_s", "value": value, "unit": "grid-point-stages/s",
-            "steps_per_s": 1e3 / ms_per_step * world, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "metric": "grid_point_stages_per_s", "value": rec["value"], "unit": "grid-point-stages/s",
+            "steps_per_s": rec["steps_per_s"], "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": rec["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": w["desc"], "N": N, "batch_per_gpu": batch, "padded": 3 * N // 2,
-                       "l2": "L2 flushed (256 MiB write) between timed steps" if flush else "inputs exceed L2 (126 MB): no flush needed",
-                       "parallelism": "replicas only (independent samples per GPU)" if world > 1 else "single GPU",
-                       "input_checksum": chk, "input_gen_s": round(t_gen, 1), "state_finite": finite},
-            "roofline": roof, "step_roofline": step_roof, "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e,
-            "gpu_launches": launches, "clocks": clocks, "device_bytes": s.device_bytes(),
+            "config": {"workload": w["desc"], "N": N, "batch_per_gpu": batch, "padded": 3 * N // 2, "l2": rec["l2"],
+                       "parallelism": "replicas only (independent Monte-Carlo samples per GPU, seeds offset by rank)" if world > 1 else "single GPU",
+                       "input_checksum": rec["input_checksum"], "setup_s": rec["setup_s"], "state_finite": rec["state_finite"],
+                       "profiler": rec["profiler"]},
+            "roofline": rec["roofline"], "step_roofline": rec["step_roofline"], "kernels": rec["kernels"], "cpu_baseline": cpu,
+            "e2e": e2e, "also": also, "gpu_launches": rec["gpu_launches"], "clocks": rec["clocks"], "device_bytes": rec["device_bytes"],
         }
         print(json.dumps(line))
     if dist is not None:
-        dist.barrier()
+        host_barrier(dist)
         dist.destroy_process_group()
     return 0
 

@@ -12,7 +12,7 @@
  *                      here they are the leading `batch` index of every array and launch
  *   outputs            "writers" of PAPER.md:L157-167: full field, energy spectrum
  * Readings of points the paper leaves open (Nyquist planes, form of Q_k, CFL formula, ...) are
- * listed in DESIGN.md section 3 (A1..A18).
+ * listed in DESIGN.md section 3 (A1..A20).
  *
  * Conventions
  *   N         grid points per axis, a power of two, 16 <= N <= 512 (fp32: 32 <= N).  Padded grid M = 3N/2.
@@ -34,6 +34,12 @@
  *             available from ns_last_error(h) until the next call on h.  On error the state is
  *             unchanged unless stated.  There is no CPU fallback: without a usable CUDA device
  *             ns_create fails with NS_ERR_CUDA.
+ *   non-finite states   every step evaluates max|u| over the padded grid on the device (a by-product
+ *             of the first stage).  A sample whose field contains NaN or inf is marked, frozen
+ *             (dt_b = 0: it is never advanced again) and reported as NS_ERR_NONFINITE with its index
+ *             by the next call that synchronises anyway: ns_step_cfl with dt_out, ns_step_dts,
+ *             ns_advance (which stops instead of running to max_steps) and ns_max_velocity (which
+ *             still fills umax_out, +inf or NaN for that sample).  Setting a new state clears the mark.
  *   threads   no global state; handles are independent; one handle must not be used concurrently.
  */
 #ifndef NS_H_
@@ -53,7 +59,8 @@ typedef enum {
   NS_ERR_INVALID_ARG = -1, /* bad N / batch / dtype / NULL pointer / nbins < 1 / bad params */
   NS_ERR_OOM = -2,         /* device allocation failed */
   NS_ERR_CUDA = -3,        /* CUDA runtime error; text in ns_last_error */
-  NS_ERR_STATE = -4        /* ns_rhs / ns_step / getters called before an initial state was set */
+  NS_ERR_STATE = -4,       /* ns_rhs / ns_step / getters called before an initial state was set */
+  NS_ERR_NONFINITE = -5    /* a sample's velocity field contains NaN or inf; ns_last_error names the sample */
 } ns_status;
 
 /* Dissipation operator of eq. (2.1)-(2.4), applied explicitly inside the RHS:
@@ -69,8 +76,9 @@ typedef struct {
 } ns_params;
 
 /* Create a solver for `batch` independent samples on an N^3 grid.  `p` may be NULL (inviscid).
- * Allocates one device arena of about 20 * batch * N^3 * sizeof(complex) bytes (state, stage
- * state and two ping-pong workspaces shared by all passes, cf. "Workspaces").
+ * Allocates one device arena of about 15.7 * batch * N^3 * sizeof(complex) bytes (state, stage
+ * state and three workspaces aliased across the passes, cf. "Workspaces", PAPER.md:L207-213;
+ * ns_device_bytes returns the exact figure).
  * cuda_stream: a cudaStream_t cast to void* (NULL = default stream). */
 int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream);
 int ns_destroy(ns_solver* h);

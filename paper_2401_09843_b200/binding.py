@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libns.so")
 
 NS_F64, NS_F32 = 0, 1
 NS_HOST, NS_DEVICE = 0, 1
-NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE = 0, -1, -2, -3, -4
+NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE, NS_ERR_NONFINITE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",

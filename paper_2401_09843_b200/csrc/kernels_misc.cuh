@@ -7,6 +7,8 @@
 // Internal spectral layout: [batch][comp][N][N][H], H = N/2 (the identically-zero kz = N/2 column of the
 // public layout is not stored, so rows are 128-byte aligned).
 #pragma once
+#include <math_constants.h>
+
 #include "cx.cuh"
 #include "ns_internal.h"
 
@@ -21,11 +23,12 @@ __device__ __forceinline__ int wavenum(int i, int N) { return i < N / 2 ? i : i 
 //   mode 0: out = R
 //   mode 1: out = alpha*Un + beta*Us + gamma*dt_b*R   (Un may be NULL when alpha == 0)
 //           dt_b == 0 marks an inactive sample: out = Un (or Us when Un is NULL), bit exact.
+//   IN-PLACE CONTRACT: out may alias Us or Un (RK stages 2 and 3 update V and U in place), so these three pointers are
+//   not __restrict__; every thread reads its own entries of Us / Un before it writes the same entries of out.
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(256)
-spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* __restrict__ Us, const cx<T>* __restrict__ Un,
-                cx<T>* __restrict__ out, int N, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
+spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
                 T gamma, const double* __restrict__ dt, int mode) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
@@ -94,33 +97,50 @@ spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* __restrict__ Us, cons
 // ------------------------------------------------------------------------------------------------
 // time-step bookkeeping (device resident: no host sync inside a step)
 // ------------------------------------------------------------------------------------------------
-__global__ void set_dt_uniform_kernel(double* dt, double* t, double value, int batch) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < batch) { dt[b] = value; t[b] += value; }
+// umax2[b] holds the bits of max |u|^2 over the padded grid at the start of the step (by-product of a3 in stage 1; a
+// non-finite field gives +inf or NaN there, kernels_z.cuh).  A sample whose maximum is not finite is marked in bad[b]
+// and frozen (dt_b = 0): the host reports NS_ERR_NONFINITE at its next synchronising call.
+__device__ __forceinline__ bool nonfinite_sq(unsigned long long bits) {
+    const double um2 = __longlong_as_double((long long)bits);
+    return !(um2 < CUDART_INF);
 }
-__global__ void set_dt_array_kernel(double* dt, double* t, const double* src, int batch) {
+__global__ void set_dt_uniform_kernel(double* dt, double* t, double value, const unsigned long long* umax2, int* bad, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < batch) { dt[b] = src[b]; t[b] += src[b]; }
+    if (b >= batch) return;
+    if (nonfinite_sq(umax2[b])) { bad[b] = 1; value = 0.0; }
+    dt[b] = value;
+    t[b] += value;
 }
-// dt_b = min(cfl * dx / umax_b, t_end - t_b); 0 for finished samples.  umax2 holds the bits of max |u|^2.
-__global__ void cfl_finalize_kernel(double* dt, double* t, const unsigned long long* umax2, double cfl, double dx,
+__global__ void set_dt_array_kernel(double* dt, double* t, const double* src, const unsigned long long* umax2, int* bad, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    double value = src[b];
+    if (nonfinite_sq(umax2[b])) { bad[b] = 1; value = 0.0; }
+    dt[b] = value;
+    t[b] += value;
+}
+// dt_b = min(cfl * dx / umax_b, t_end - t_b); 0 for finished samples.
+__global__ void cfl_finalize_kernel(double* dt, double* t, const unsigned long long* umax2, int* bad, double cfl, double dx,
                                     double t_end, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
     const double remaining = t_end - t[b];
     double v = 0.0;
-    if (remaining > 0.0) {
+    if (nonfinite_sq(umax2[b])) {
+        bad[b] = 1;
+    } else if (remaining > 0.0) {
         const double um = sqrt(__longlong_as_double((long long)umax2[b]));
         v = um > 0.0 ? cfl * dx / um : remaining;
         if (!(v < remaining)) v = remaining;
-        if (!isfinite(v)) v = 0.0;
     }
     dt[b] = v;
     t[b] += v;
 }
-__global__ void umax_read_kernel(double* out, const unsigned long long* umax2, int batch) {
+__global__ void umax_read_kernel(double* out, const unsigned long long* umax2, int* bad, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < batch) out[b] = sqrt(__longlong_as_double((long long)umax2[b]));
+    if (b >= batch) return;
+    if (nonfinite_sq(umax2[b])) bad[b] = 1;
+    out[b] = sqrt(__longlong_as_double((long long)umax2[b]));   // +inf / NaN for a non-finite field
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -25,8 +25,22 @@ namespace ns {
 
 template <int R1, int R2> struct ZP { static constexpr int value = R1 > R2 ? R1 : R2; };
 
-__device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v) {
-    atomicMax(addr, (unsigned long long)__double_as_longlong(v));
+// Running maximum of |u|^2 that PROPAGATES non-finite values (fmax would drop a NaN): for x >= +0 the IEEE bit patterns
+// order like the values, +inf sorts above every finite value and every NaN above +inf, so an unsigned integer maximum of
+// the bits keeps them.  umax2[b] holds the bits of a double; cfl_finalize / umax_read turn a non-finite maximum into a
+// failed sample (NS_ERR_NONFINITE) instead of a silent dt.
+__device__ __forceinline__ unsigned long long sq_bits(double v) { return (unsigned long long)__double_as_longlong(v); }
+__device__ __forceinline__ unsigned int sq_bits(float v) { return __float_as_uint(v); }
+template <typename U> __device__ __forceinline__ U umax_bits(U a, U b) { return a > b ? a : b; }
+__device__ __forceinline__ unsigned long long warp_max_bits(unsigned long long m) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = umax_bits(m, __shfl_xor_sync(0xffffffffu, m, o));
+    return m;
+}
+__device__ __forceinline__ unsigned int warp_max_bits(unsigned int m) { return __reduce_max_sync(0xffffffffu, m); }
+__device__ __forceinline__ void atomic_max_sq(unsigned long long* addr, unsigned long long m) { atomicMax(addr, m); }
+__device__ __forceinline__ void atomic_max_sq(unsigned long long* addr, unsigned int m) {
+    atomicMax(addr, (unsigned long long)__double_as_longlong((double)__uint_as_float(m)));   // float -> double keeps inf / NaN
 }
 
 // 3 -> 2 radix-3 combine + Hermitian split of one forward pair (see kernels_z.cuh):

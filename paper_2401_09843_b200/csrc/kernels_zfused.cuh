@@ -169,14 +169,13 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
             fft_reg<R2, +1, T>(u12);  // u12[j] holds r2 = brev(j)
         }
         if (umax2 != nullptr) {
-            T lmax = 0;
+            auto lmax = sq_bits((T)0);
             if (i < R1) {
 #pragma unroll
-                for (int j = 0; j < R2; ++j) lmax = fmax(lmax, u12[j].x * u12[j].x + u12[j].y * u12[j].y + u3r[j] * u3r[j]);
+                for (int j = 0; j < R2; ++j) lmax = umax_bits(lmax, sq_bits(u12[j].x * u12[j].x + u12[j].y * u12[j].y + u3r[j] * u3r[j]));
             }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
-            if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax2 + b, (double)lmax);
+            lmax = warp_max_bits(lmax);
+            if ((threadIdx.x & 31) == 0) atomic_max_sq(umax2 + b, lmax);
         }
         // ---------------- forward pairs (T11,T22) (T12,T13) (T23,-), see kernels_z.cuh
         cx<T>* Op = out + (b * 5 * MM + pp) * L;

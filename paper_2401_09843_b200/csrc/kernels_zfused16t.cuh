@@ -130,18 +130,17 @@ z_fused16t_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM
                 tmem_load16(tZ, w3);
                 if (pair == 0) {
                     // v still holds u1 + i u2
-                    T lmax = 0;
+                    auto lmax = sq_bits((T)0);
 #pragma unroll
                     for (int k = 0; k < 16; ++k) {
                         const T x2 = v[k].x * v[k].x, y2 = v[k].y * v[k].y, z2 = w3[k] * w3[k];
-                        lmax = fmax(lmax, x2 + y2 + z2);
+                        lmax = umax_bits(lmax, sq_bits(x2 + y2 + z2));
                         v[k] = mk<T>(x2 - z2, y2 - z2);
                     }
                     if (umax2 != nullptr) {
                         // lanes of a warp belong to neighbouring lines of the same sample (LPB | MM)
-#pragma unroll
-                        for (int o = 16; o > 0; o >>= 1) lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
-                        if (lane == 0) atomic_max_nonneg(umax2 + b, (double)lmax);
+                        lmax = warp_max_bits(lmax);
+                        if (lane == 0) atomic_max_sq(umax2 + b, lmax);
                     }
                 } else if (pair == 1) {
                     T wx[16], wy[16];

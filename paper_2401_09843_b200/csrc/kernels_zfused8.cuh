@@ -203,13 +203,12 @@ z_fused8_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, 
         }
         z8_inverse<T, L>(u12, S, t, tw);
         if (umax2 != nullptr) {
-            T lmax = 0;
+            auto lmax = sq_bits((T)0);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) lmax = fmax(lmax, u12[k].x * u12[k].x + u12[k].y * u12[k].y + u3r[k] * u3r[k]);
+            for (int k = 0; k < 8; ++k) lmax = umax_bits(lmax, sq_bits(u12[k].x * u12[k].x + u12[k].y * u12[k].y + u3r[k] * u3r[k]));
             // lanes of a warp may belong to different lines, but (LPB | MM) to the same sample
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
-            if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax2 + b, (double)lmax);
+            lmax = warp_max_bits(lmax);
+            if ((threadIdx.x & 31) == 0) atomic_max_sq(umax2 + b, lmax);
         }
         // ---------------- forward pairs (T11,T22) (T12,T13) (T23,-), see kernels_z.cuh
         cx<T>* Op = out + (b * 5 * MM + pp) * L;

@@ -78,6 +78,14 @@ struct PassProfiler {
         used = 0;
         for (int i = 0; i < NPASS; ++i) { ms[i] = 0; cnt[i] = 0; }
     }
+    void reserve(size_t n) {   // events are created when profiling is switched on, not inside a timed loop
+        while (ev.size() < n) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return;
+            ev.push_back(e);
+            tag.push_back(-1);
+        }
+    }
     void tick(int pass, cudaStream_t st) {  // pass < 0: end marker
         if (!on || used >= MAX_EVENTS) return;
         if (used == ev.size()) {
@@ -118,6 +126,7 @@ public:
     T* dtab = nullptr;
     double *dt_dev = nullptr, *t_dev = nullptr, *scal_dev = nullptr, *red_dev = nullptr;
     unsigned long long* umax2 = nullptr;
+    int* bad_dev = nullptr;   // per-sample flag: non-finite state seen (kernels_misc.cuh)
     size_t nS, nX, nY, nZ;  // complex element counts of state, X, Y, Z
     size_t red_count;
     PassProfiler prof;
@@ -147,6 +156,20 @@ public:
         if (e__ != cudaSuccess) return cuda_fail(e__, name);   \
     } while (0)
 
+    // Reads the per-sample non-finite flags (the stream is synchronised by the copy) and reports the first marked sample.
+    int check_finite() {
+        std::vector<int> bad((size_t)batch);
+        NS_CK(cudaMemcpyAsync(bad.data(), bad_dev, (size_t)batch * sizeof(int), cudaMemcpyDeviceToHost, st));
+        NS_CK(cudaStreamSynchronize(st));
+        for (int b = 0; b < batch; ++b)
+            if (bad[b]) {
+                char buf[160];
+                snprintf(buf, sizeof buf, "sample %d: the velocity field is not finite (NaN or inf); the sample is frozen", b);
+                return fail(NS_ERR_NONFINITE, buf);
+            }
+        return NS_OK;
+    }
+
     Twiddles<T> tw() const { return make_twiddles<T>(twbase, L); }
     static unsigned blocks_for(long total, int threads) { return (unsigned)((total + threads - 1) / threads); }
 
@@ -171,6 +194,7 @@ public:
         const size_t oD = take(ndt * sizeof(T));
         const size_t odt = take(b * sizeof(double)), ot = take(b * sizeof(double)), osc = take(b * sizeof(double));
         const size_t oum = take(b * sizeof(unsigned long long));
+        const size_t obad = take(b * sizeof(int));
         const size_t ored = take(red_count * sizeof(double));
         arena_bytes = off;
         cudaError_t e = cudaMalloc(&arena, arena_bytes);
@@ -192,6 +216,7 @@ public:
         t_dev = (double*)(arena + ot);
         scal_dev = (double*)(arena + osc);
         umax2 = (unsigned long long*)(arena + oum);
+        bad_dev = (int*)(arena + obad);
         red_dev = (double*)(arena + ored);
 
         const std::vector<cx<T>> htw = build_twiddle_block<T>(L);
@@ -201,6 +226,7 @@ public:
         NS_CK(cudaMemcpyAsync(dtab, hd.data(), hd.size() * sizeof(T), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemsetAsync(t_dev, 0, b * sizeof(double), st));
         NS_CK(cudaMemsetAsync(dt_dev, 0, b * sizeof(double), st));
+        NS_CK(cudaMemsetAsync(bad_dev, 0, b * sizeof(int), st));
         NS_CK(cudaStreamSynchronize(st));
         return NS_OK;
     }
@@ -254,17 +280,18 @@ public:
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
         int rc;
         const unsigned gb = blocks_for(batch, 128);
-        if (mode == DT_CFL) NS_CK(cudaMemsetAsync(umax2, 0, (size_t)batch * sizeof(unsigned long long), st));
-        if ((rc = transform(U, mode == DT_CFL)) != NS_OK) return rc;
+        // max|u|^2 is a free by-product of a3 in stage 1; besides the CFL step it is what detects a non-finite state
+        NS_CK(cudaMemsetAsync(umax2, 0, (size_t)batch * sizeof(unsigned long long), st));
+        if ((rc = transform(U, true)) != NS_OK) return rc;
         if (mode == DT_UNIFORM) {
-            set_dt_uniform_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, dt, batch);
+            set_dt_uniform_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, dt, umax2, bad_dev, batch);
             NS_LAUNCHED("set_dt_uniform");
         } else if (mode == DT_ARRAY) {
             NS_CK(cudaMemcpyAsync(scal_dev, dts_host, (size_t)batch * sizeof(double), cudaMemcpyHostToDevice, st));
-            set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, scal_dev, batch);
+            set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, scal_dev, umax2, bad_dev, batch);
             NS_LAUNCHED("set_dt_array");
         } else {
-            cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, umax2, cfl, 2.0 * 3.14159265358979323846 / N, t_end, batch);
+            cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, umax2, bad_dev, cfl, 2.0 * 3.14159265358979323846 / N, t_end, batch);
             NS_LAUNCHED("cfl_finalize");
         }
         // eq. (2.6): u1 = u + dt R(u)
@@ -286,8 +313,7 @@ public:
         if (!dts) return fail(NS_ERR_INVALID_ARG, "dt array is NULL");
         int rc = rk3(DT_ARRAY, 0, dts, 0, 0);
         if (rc != NS_OK) return rc;
-        NS_CK(cudaStreamSynchronize(st));  // dts is caller memory: do not return before it was read
-        return NS_OK;
+        return check_finite();  // synchronises: dts is caller memory, do not return before it was read
     }
     int step_cfl(double cfl, double t_end, double* dt_out) override {
         if (!(cfl > 0.0)) return fail(NS_ERR_INVALID_ARG, "cfl must be positive");
@@ -295,7 +321,7 @@ public:
         if (rc != NS_OK) return rc;
         if (dt_out) {
             NS_CK(cudaMemcpyAsync(dt_out, dt_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
-            NS_CK(cudaStreamSynchronize(st));
+            return check_finite();
         }
         return NS_OK;
     }
@@ -307,7 +333,8 @@ public:
         int n = 0;
         while (n < max_steps) {
             NS_CK(cudaMemcpyAsync(th.data(), t_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
-            NS_CK(cudaStreamSynchronize(st));
+            int rcf = check_finite();   // a non-finite sample has dt = 0 for ever: stop instead of spinning to max_steps
+            if (rcf != NS_OK) { if (steps_done) *steps_done = n; return rcf; }
             bool done = true;
             for (double tb : th) done = done && !(tb < t_end);
             if (done) break;
@@ -328,11 +355,10 @@ public:
         NS_CK(cudaMemsetAsync(umax2, 0, (size_t)batch * sizeof(unsigned long long), st));
         int rc = transform(U, true, 3);
         if (rc != NS_OK) return rc;
-        umax_read_kernel<<<blocks_for(batch, 128), 128, 0, st>>>(scal_dev, umax2, batch);
+        umax_read_kernel<<<blocks_for(batch, 128), 128, 0, st>>>(scal_dev, umax2, bad_dev, batch);
         NS_LAUNCHED("umax_read");
         NS_CK(cudaMemcpyAsync(out, scal_dev, (size_t)batch * sizeof(double), cudaMemcpyDeviceToHost, st));
-        NS_CK(cudaStreamSynchronize(st));
-        return NS_OK;
+        return check_finite();   // umax_out is filled either way (+inf / NaN for the failed sample)
     }
 
     int rhs(void* out, ns_memspace ms) override {
@@ -374,6 +400,7 @@ public:
         const long total = (long)batch * 3 * N * N * H;
         to_internal_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, U, N, total);
         NS_LAUNCHED("to_internal");
+        NS_CK(cudaMemsetAsync(bad_dev, 0, (size_t)batch * sizeof(int), st));
         if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));  // caller buffer fully consumed
         has_state = true;
         return NS_OK;
@@ -410,6 +437,7 @@ public:
         init_project_kernel<T><<<blocks_for(tot, 256), 256, 0, st>>>(X, U, N, tot, (T)(1.0 / ((double)N * N * N)));
         NS_LAUNCHED("init_project");
         NS_CK(cudaMemsetAsync(t_dev, 0, (size_t)batch * sizeof(double), st));
+        NS_CK(cudaMemsetAsync(bad_dev, 0, (size_t)batch * sizeof(int), st));
         if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));
         has_state = true;
         return NS_OK;
@@ -522,6 +550,7 @@ public:
         NS_CK(cudaStreamSynchronize(st));
         prof.reset();
         prof.on = enable != 0;
+        if (prof.on) prof.reserve(512);
         return NS_OK;
     }
     int profile_read(double* ms, long long* cnt) override {

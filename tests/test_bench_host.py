@@ -11,15 +11,19 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _worker(rank, world, port, q):
-    import torch.distributed as dist
-    os.environ["MASTER_ADDR"] = "127.0.0.1"
-    os.environ["MASTER_PORT"] = str(port)
-    dist.init_process_group("gloo", rank=rank, world_size=world)
+    # the environment torchrun gives every rank; the group is created by bench.py's own init_dist (the code path of
+    # `bench.py --gpus N`: NCCL + gloo with GPUs, gloo alone here) and the host barrier / aggregation are bench.py's
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
     sys.path.insert(0, ROOT)
     import bench
+    assert bench.dist_env() == (rank, world, rank)
+    dist = bench.init_dist(world)
+    bench.host_barrier(dist)
     ms, units = bench.aggregate(10.0 + 5.0 * rank, 100.0 * (rank + 1), world, dist)
-    q.put((rank, ms, units))
-    dist.barrier()
+    # every rank draws its own Monte-Carlo samples
+    a = bench.make_input("c1", 16, 1, rank)
+    q.put((rank, ms, units, float(a.sum())))
+    bench.host_barrier(dist)
     dist.destroy_process_group()
 
 
@@ -35,9 +39,10 @@ def test_aggregate_world_size_2_gloo():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    for _, ms, units in res:
+    for _, ms, units, _chk in res:
         assert ms == 15.0          # max over ranks
         assert units == 300.0      # whole-job units
+    assert res[0][3] != res[1][3]  # seeds offset by rank
 
 
 def test_aggregate_single_rank_is_identity():

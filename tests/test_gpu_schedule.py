@@ -1,0 +1,184 @@
+"""GPU parity schedule of SURVEY.md section 8(d) at the BASELINE.json sizes (configs[1]..configs[4]), the CUDA path
+through the C ABI against the CPU oracle on the same seeded inputs:
+
+  config 2  128^3          1 RHS + 20 CFL-0.2 RK3 steps, the oracle replaying the GPU's dt sequence, relative L2 at EVERY step
+  config 3  256^3          the config's own input: full-array orc_rhs_parts (every stored entry) + 3 replayed steps
+  config 4  32 x 128^3     one sample of the batched run replayed for 10 steps, E(K) and S_2 compared (reading A17)
+  config 5  512^3          >= 512 STRATIFIED sampled wavenumbers against the direct truncated convolution, relative L2
+                           over the sample, plus the energy identity P4 and the solenoidality P5 on the whole array
+
+Tolerances are the north_star's: relative L2 <= 1e-12 per ns_rhs, <= 1e-10 after (up to) 20 ns_step in fp64.
+Run on the B200 box:  python -m pytest tests -m gpu
+"""
+import time
+
+import numpy as np
+import pytest
+
+from paper_2401_09843_b200 import inputs
+from _sampling import stratified_modes
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS_F64, TOL_STEPS_F64 = 1e-12, 1e-10
+
+
+@pytest.fixture(scope="module")
+def ns():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2401_09843_b200 import binding
+    binding.lib()
+    return binding
+
+
+def rel(a, b):
+    return float(np.linalg.norm((np.asarray(a) - b).ravel()) / max(np.linalg.norm(np.asarray(b).ravel()), 1e-300))
+
+
+# ------------------------------------------------------------------------------------------------ config 2
+def test_config2_128_rhs_and_20_cfl_steps(ns, oracle):
+    """BASELINE.json configs[1]: N = 128, Gaussian k^4 exp field (seed 2), hyperviscosity eps = 0.05, s = 1, m = sqrt(N),
+    CFL 0.2: one RHS and the first 20 RK3 steps, the oracle replaying the GPU's dt; relative L2 at every step."""
+    N = 128
+    u = inputs.gaussian_k4(N, seed=2)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    s.set_spectral(uh[None])
+    p = oracle.Params(**kw)
+    want = oracle.rhs_parts(N, p, uh)
+    assert rel(s.rhs()[0], want["r"]) < TOL_RHS_F64
+    worst, t0, tsum = 0.0, time.perf_counter(), 0.0
+    for i in range(20):
+        dts = s.step_cfl(0.2, 1e9)
+        if i in (0, 10):     # dt against the oracle's own max|u| (costs an oracle inverse transform: not every step)
+            assert abs(dts[0] - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, uh)) < 1e-12 * dts[0]
+        tsum += dts[0]
+        uh = oracle.step(N, p, uh, dts[0])
+        worst = max(worst, rel(s.get_spectral()[0], uh))
+        assert worst < TOL_STEPS_F64, (i, worst)
+    print(f"config 2: worst rel-L2 over 20 steps {worst:.2e}; oracle {time.perf_counter() - t0:.0f} s")
+    assert abs(s.time(0) - tsum) < 1e-13 * tsum
+
+
+# ------------------------------------------------------------------------------------------------ config 3
+def test_config3_256_full_array_rhs_and_3_steps(ns, oracle):
+    """BASELINE.json configs[2] with its own input (perturbed shear layer, seed 3) at N = 256 -- the size that runs the
+    long-line kernels: EVERY stored entry of ns_rhs against orc_rhs_parts (relative L2 <= 1e-12, and the largest
+    single-entry deviation), max|u| on the padded grid, then 3 CFL steps with the oracle replaying the GPU's dt."""
+    N = 256
+    u = inputs.shear_layer(N, seed=3)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    del u
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    s.set_spectral(uh[None])
+    p = oracle.Params(**kw)
+    t0 = time.perf_counter()
+    want = oracle.rhs_parts(N, p, uh)
+    t_rhs = time.perf_counter() - t0
+    got = s.rhs()[0]
+    assert rel(got, want["r"]) < TOL_RHS_F64
+    assert np.abs(got - want["r"]).max() < 1e-12 * np.abs(want["r"]).max()     # no single entry is off (tile faults)
+    assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
+    del got, want
+    worst = 0.0
+    for i in range(3):
+        dts = s.step_cfl(0.2, 1e9)
+        uh = oracle.step(N, p, uh, dts[0])
+        worst = max(worst, rel(s.get_spectral()[0], uh))
+        assert worst < TOL_STEPS_F64, (i, worst)
+    print(f"config 3: oracle RHS {t_rhs:.0f} s; worst rel-L2 over 3 steps {worst:.2e}")
+
+
+# ------------------------------------------------------------------------------------------------ config 4
+def test_config4_one_sample_replayed_10_steps(ns, oracle):
+    """BASELINE.json configs[3]: the 32 x 128^3 shear-layer ensemble stepped in ONE batched launch at per-sample CFL 0.2;
+    the oracle replays sample 1's dt sequence for 10 steps.  State at relative L2 <= 1e-10 at every step; the reported
+    statistics E(K) and S_2(l) of that sample at the statistical tolerance of reading A17 (1e-8 relative)."""
+    N, B, pick = 128, 32, 1
+    us = inputs.shear_layer_ensemble(N, B, seed0=1000)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, batch=B, **kw)
+    s.set_initial(us)
+    uh = oracle.set_initial(N, us[pick])
+    del us
+    u0 = s.get_spectral()
+    assert rel(u0[pick], uh) < 1e-13
+    uh = u0[pick].copy()
+    del u0
+    p = oracle.Params(**kw)
+    worst = 0.0
+    for i in range(10):
+        dts = s.step_cfl(0.2, 1.0)
+        uh = oracle.step(N, p, uh, dts[pick])
+        got = s.get_spectral()[pick]
+        worst = max(worst, rel(got, uh))
+        assert worst < TOL_STEPS_F64, (i, worst)
+    E = s.energy_spectrum(N)[pick]
+    Eo = oracle.energy_spectrum(N, uh, N)
+    assert np.abs(E - Eo).max() < 1e-8 * Eo.max()
+    S = s.structure_function()[pick]
+    assert np.abs(S / oracle.structure_function(N, uh) - 1).max() < 1e-8
+    assert np.abs(s.structure_function_p(2.0, nl=8)[pick] / oracle.structure_function(N, uh, 8) - 1).max() < 1e-8
+    print(f"config 4: worst rel-L2 over 10 replayed steps {worst:.2e}")
+
+
+# ------------------------------------------------------------------------------------------------ config 5
+@pytest.mark.parametrize("N", [256, 512])
+def test_full_size_stratified_sampled_rhs(ns, oracle, N):
+    """256^3 and 512^3 (configs[4] input), same launch configuration as bench.py: ns_rhs at >= 512 stratified sampled
+    wavenumbers against the oracle's direct truncated convolution sum (orc_rhs_at_modes): relative L2 over the sample
+    <= 1e-12 and every single sampled entry within 1e-12 of max|R|; then, on the WHOLE array, the energy identity P4
+    of the inviscid RHS (a statement about every entry of the transforms: any aliasing or tile fault breaks it), the
+    masks, and the fused RK3 step against eq. 2.6 assembled on the host from ns_rhs evaluations (pins the axpy of a7)."""
+    u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5) if N == 256 else inputs.gaussian_k53(N, seed=5)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    del u
+    uh = s.get_spectral()[0]
+    r = s.rhs()[0]
+    del s
+    rmax = np.abs(r).max()
+    modes = stratified_modes(N, 512, N)
+    t0 = time.perf_counter()
+    want = oracle.rhs_at_modes(N, oracle.Params(**kw), uh, modes)
+    t_or = time.perf_counter() - t0
+    got = np.stack([r[:, ix, iy, iz] for ix, iy, iz in modes])
+    err = np.abs(got - want)
+    print(f"N = {N}: {len(modes)} sampled modes, oracle {t_or:.0f} s, rel-L2 {rel(got, want):.2e}, worst entry {err.max() / rmax:.2e} of max|R|")
+    assert np.linalg.norm(want) > 1e-2 * rmax
+    assert rel(got, want) < TOL_RHS_F64
+    assert err.max() < 1e-12 * rmax
+    assert np.all(r[:, N // 2] == 0) and np.all(r[:, :, N // 2] == 0) and np.all(r[:, :, :, N // 2] == 0)
+    del r
+    # P4 on the whole array: inviscid solver (the viscous one was destroyed first: memory)
+    w = np.full(N // 2 + 1, 2.0)
+    w[0] = 1.0
+    s = ns.Solver(N)
+    s.set_spectral(uh[None])
+    rn = s.rhs()[0]
+    num = abs(np.sum(w * np.real(np.conj(uh) * rn)))
+    den = np.sum(w * np.abs(uh) * np.abs(rn))
+    print(f"N = {N}: energy identity residual {num / den:.2e}")
+    assert num < 1e-12 * den
+    # fused RK3 step == eq. 2.6 assembled from ns_rhs (same kernels in mode 0)
+    dt = 0.2 * (2 * np.pi / N) / s.max_velocity()[0]
+    u1 = uh + dt * rn
+    del rn
+    s.set_spectral(u1[None])
+    u2 = 0.75 * uh + 0.25 * u1 + 0.25 * dt * s.rhs()[0]
+    del u1
+    s.set_spectral(u2[None])
+    un = uh / 3.0 + (2.0 / 3.0) * u2 + (2.0 / 3.0) * dt * s.rhs()[0]
+    del u2
+    s.set_spectral(uh[None])
+    dts = s.step_cfl(0.2, 1e9)
+    assert abs(dts[0] - dt) < 1e-13 * dt
+    assert rel(s.get_spectral()[0], un) < 1e-14

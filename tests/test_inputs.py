@@ -66,3 +66,15 @@ def test_oracle_on_paper_experiments_is_dissipative(oracle, name):
     k = np.fft.fftfreq(N, 1.0 / N)
     div = k[:, None, None] * uh[0] + k[None, :, None] * uh[1] + np.arange(N // 2 + 1.0)[None, None, :] * uh[2]
     assert np.abs(div).max() < 1e-13
+
+
+def test_stratified_modes_cover_every_class():
+    from _sampling import stratified_modes
+    for N in (256, 512):
+        m = stratified_modes(N, 512, 1)
+        assert len(m) >= 512
+        for ax in (0, 1):
+            assert set(range(16)) <= set(m[:, ax] % 16)                       # every R2 class / column-tile lane
+            assert {0, 7, N // 2 - 1, N // 2 + 1, N - 8, N - 1} <= set(m[:, ax])  # first / last tiles of both halves
+            assert (m[:, ax] > N // 2).sum() > 100 and (m[:, ax] < N // 2).sum() > 100
+        assert set(range(16)) <= set(m[:, 2]) and set(range(N // 2 - 16, N // 2)) <= set(m[:, 2])
