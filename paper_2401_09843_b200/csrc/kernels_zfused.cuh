@@ -52,7 +52,7 @@ __device__ __forceinline__ cx<T> prune3(cx<T> a, cx<T> c, int q, int n, const Tw
 }
 
 // in [batch][3][MM][L] complex -> out [batch][5][MM][L] complex (unnormalised transforms of the flux components)
-template <typename T, int L, int R1, int R2, int LPB, int MINB, bool SEPCMB>
+template <typename T, int L, int R1, int R2, int LPB, int MINB>
 __global__ void __launch_bounds__(3 * ZP<R1, R2>::value* LPB, MINB)
 z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, long total_tiles,
                unsigned long long* __restrict__ umax2, Twiddles<T> tw) {
@@ -63,9 +63,8 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* In = reinterpret_cast<cx<T>*>(smem_raw);   // [3][LPB][L]
     cx<T>* E = In + (size_t)3 * LPB * L;               // [LPB][3][R1][PITCH] exchange buffer
-    // combine buffer, same layout: a second buffer (SEPCMB, one barrier less per pair) or E itself
-    cx<T>* Cb = SEPCMB ? E + (size_t)LPB * ELINE : E;
-    uint64_t* full = reinterpret_cast<uint64_t*>(E + (size_t)(SEPCMB ? 2 : 1) * LPB * ELINE);
+    cx<T>* Cb = E;   // the combine reads the exchange buffer itself
+    uint64_t* full = reinterpret_cast<uint64_t*>(E + (size_t)LPB * ELINE);
 
     const int i = threadIdx.x % P;
     const int q = (threadIdx.x / P) % 3;
@@ -241,7 +240,7 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
                     }
                 }
             }
-            if (!SEPCMB) __syncthreads();  // combine reads done before E is rewritten (next pair / next tile)
+            __syncthreads();  // combine reads done before E is rewritten (next pair / next tile)
         }
     }
 }

@@ -1,0 +1,321 @@
+// kernels_zpair.cuh -- steps a3 + a4 of SURVEY.md section 8(a) in ONE kernel for L = N/2 in {64, 128, 256}: per (px,py) line,
+// pad + inverse c2r along z, the trace-free flux products, max|u|^2, forward r2c + truncate (Algorithm 2 steps 1-5,
+// PAPER.md:L132-135; symmetric flux PAPER.md:L245).  The M^3 physical arrays never touch HBM.
+//
+// Mathematics as in kernels_z.cuh (pruned radix-3 + two-for-one real transforms).  What this kernel adds:
+//
+//  * LINE PAIRS.  A line needs 3 real inverse transforms (u1, u2, u3) and 5 real forward ones (T11, T12, T13, T22, T23);
+//    done line by line, two-for-one leaves u3 and T23 alone in a complex transform whose imaginary half is zero.  Here a
+//    lane group owns TWO neighbouring lines A, B and runs 8 complex transforms for them,
+//        job 0  inverse (u3A, u3B)        job 4  inverse (u1B, u2B)
+//        job 1  inverse (u1A, u2A)        job 5  forward (T11B, T22B)
+//        job 2  forward (T11A, T22A)      job 6  forward (T12B, T13B)
+//        job 3  forward (T12A, T13A)      job 7  forward (T23A, T23B)
+//    i.e. 4 per line instead of 5: no arithmetic, shared-memory exchange or barrier is spent on zeros.
+//  * ONE TRANSFORM ROUTINE.  All 8 jobs run through one copy of the code: the job loop is rolled, the forward transforms
+//    use the inverse butterflies (F(x) = conj(F^-1(conj x)); the conjugations fold into the product formation and the
+//    radix-3 twiddle), and forward and inverse use the same flow "radix 16 in registers -> twiddle -> warp-local exchange
+//    -> radix G": a thread holds the points p = t + G j of a sub-transform before AND after it (only the register order
+//    differs, a compile-time permutation), so no mirrored forward routine is needed.  The loop body is about 1/3 of the
+//    unrolled per-line version and fits the 32 KB instruction cache.
+//  * The physical-space fields that have to wait (4 fields of 16 values per thread: u3A, u3B and either (u1, u2) of the line
+//    being worked on or T23A / T23B) are parked in TENSOR MEMORY (tmem.cuh); registers hold only the transform in flight.
+//  * Inputs are fetched by the TMA bulk-copy engine into a 2-slot ring per lane group (one slot = the two half-spectrum
+//    lines of one inverse job), issued two to three jobs ahead at the named barriers of the forward jobs.
+//
+// Thread layout: block = UNITS units of 96 threads; unit = 3 warps = the three radix-3 sub-transforms q of 32/G line pairs;
+// lane group = G = L/16 lanes = one line pair; every lane holds 16 complex values.
+#pragma once
+#include <cstdint>
+
+#include "cx.cuh"
+#include "kernels_zfused.cuh"   // mbarrier / bulk-copy helpers, prune3
+#include "kernels_zfused8.cuh"  // named_bar_sync
+#include "tmem.cuh"
+
+namespace ns {
+
+template <typename T, int L> struct ZPGeo {
+    static constexpr int G = L / 16;          // lanes per sub-transform = lanes per line pair
+    static constexpr int Hc = 16 / G;         // radix-G transforms per lane in the second stage
+    static constexpr int PL = 32 / G;         // line pairs per unit
+    static constexpr int REGION = 16 * 32;    // exchange / combine region of one warp, complex elements (16 rows x 32 lanes)
+    static constexpr int SLOT = 2 * L;        // one input slot: two lines of L complex
+    // odd lane groups are shifted by 4 elements (64 B) when G = 4 so that the two groups of a quarter warp hit disjoint banks
+    static constexpr int LGPITCH = 2 * SLOT + (G == 4 ? 4 : 0);
+    static constexpr int IN_UNIT = PL * LGPITCH;                         // input ring of one unit, complex elements
+    static constexpr size_t UNIT_BYTES = (size_t)(IN_UNIT + 3 * REGION) * sizeof(cx<T>) + (size_t)PL * 2 * sizeof(uint64_t);
+    static constexpr uint32_t C16 = 16 * sizeof(T) / 4;                  // TMEM columns of 16 scalars
+    static constexpr uint32_t WCOLS = 4 * C16;                           // TMEM columns per warp: 4 fields
+};
+
+// register holding point j (p = t + G j) after a transform: output (h, r2) <-> j = h + Hc r2 sits at h G + brev_G(r2)
+template <int G> __host__ __device__ constexpr int zp_perm(int j) {
+    constexpr int Hc = 16 / G;
+    return (j % Hc) * G + brev<G>(j / Hc);
+}
+
+// The transform of all jobs: in v[j] = s[t + G j], out v[zp_perm(j')] = sum_n s[n] w_L^{+n k}, k = t + G j'.
+// Sw: the warp's exchange region (16 rows x 32 columns, XOR-swizzled: element (row, col) at row*32 + (col ^ (row & 7))).
+template <typename T, int L>
+__device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int t, int lgcol, const cx<T>* __restrict__ tw16) {
+    constexpr int G = ZPGeo<T, L>::G, Hc = ZPGeo<T, L>::Hc;
+    fft_reg<16, +1, T>(v);
+#pragma unroll
+    for (int r1 = 0; r1 < 16; ++r1) {
+        cx<T> w = v[brev<16>(r1)];
+        if (r1 > 0) w = cmul(w, ldg(tw16 + r1 * G + t));
+        Sw[r1 * 32 + (lane ^ (r1 & 7))] = w;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int h = 0; h < Hc; ++h) {
+        const int row = t + G * h;
+        const cx<T>* Sr = Sw + row * 32 + lgcol;
+        const int rm = row & 7;
+#pragma unroll
+        for (int tt = 0; tt < G; ++tt) v[h * G + tt] = Sr[(tt & ~7) | ((tt & 7) ^ rm)];
+    }
+    __syncwarp();
+#pragma unroll
+    for (int h = 0; h < Hc; ++h) fft_reg<G, +1, T>(v + h * G);
+}
+
+// 3 -> 2 radix-3 combine + Hermitian split of one forward job: reads G_q[n] = F_q[n] W^{-qn} of the three sub-transforms
+// (regions REGION apart, swizzled as above, element n at row n / G, column lgcol + n % G) and writes the two real
+// transforms B_a^[n], B_b^[n] for n and L - n (kernels_z.cuh).  Threads tl = 0..3G-1 of the line pair cover n <= L/2.
+template <typename T, int L>
+__device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, int lgcol, cx<T>* __restrict__ Oa, cx<T>* __restrict__ Ob, int tl) {
+    constexpr int G = ZPGeo<T, L>::G, REGION = ZPGeo<T, L>::REGION, TPL = 3 * G;
+    constexpr int NIT = (L / 2 + TPL) / TPL;  // iterations covering n in [0, L/2]
+    constexpr T h3 = (T)0.86602540378443864676L;
+    auto at = [&](int qq, int n) {
+        const int row = n / G, col = lgcol + n % G;
+        return Su[qq * REGION + row * 32 + (col ^ (row & 7))];
+    };
+    cx<T> f0[NIT], g1[NIT], g2[NIT], f0m[NIT], g1m[NIT], g2m[NIT];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        int n = tl + it * TPL;
+        if (n > L / 2) n = L / 2;             // clamped duplicate, not stored
+        const int m = n == 0 ? 0 : L - n;
+        f0[it] = at(0, n); g1[it] = at(1, n); g2[it] = at(2, n);
+        f0m[it] = at(0, m); g1m[it] = at(1, m); g2m[it] = at(2, m);
+    }
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        const int n = tl + it * TPL;
+        const cx<T> Sn = g1[it] + g2[it], Dn = g1[it] - g2[it];
+        const cx<T> An = f0[it] + Sn;
+        const cx<T> Cn = mk<T>(f0[it].x - (T)0.5 * Sn.x - h3 * Dn.y, f0[it].y - (T)0.5 * Sn.y + h3 * Dn.x);
+        const cx<T> Sm = g1m[it] + g2m[it], Dm = g1m[it] - g2m[it];
+        const cx<T> Am = f0m[it] + Sm;
+        const cx<T> Cm = mk<T>(f0m[it].x - (T)0.5 * Sm.x - h3 * Dm.y, f0m[it].y - (T)0.5 * Sm.y + h3 * Dm.x);
+        if (n <= L / 2) {
+            if (n == 0) {
+                Oa[0] = mk<T>(An.x, 0);
+                Ob[0] = mk<T>(An.y, 0);
+            } else {
+                const int m = L - n;
+                Oa[n] = mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y));
+                Ob[n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
+                if (m != n) {
+                    Oa[m] = mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y));
+                    Ob[m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
+                }
+            }
+        }
+    }
+}
+
+// in [batch][3][MM][L] complex -> out [batch][5][MM][L] complex (unnormalised transforms of the flux components, order
+// 11 12 13 22 23).  total_pairs = batch * MM / 2 line pairs; (MM / 2) % (32 / G) == 0 (a warp never straddles two samples).
+template <typename T, int L, int UNITS>
+__global__ void __launch_bounds__(96 * UNITS, 1)
+z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, long total_pairs,
+              unsigned long long* __restrict__ umax2, Twiddles<T> tw) {
+    using Geo = ZPGeo<T, L>;
+    constexpr int G = Geo::G, PL = Geo::PL, REGION = Geo::REGION, SLOT = Geo::SLOT;
+    constexpr uint32_t C16 = Geo::C16;
+    constexpr uint32_t NWARPS = 3 * UNITS;
+    constexpr uint32_t COLS_NEEDED = ((NWARPS + 3) / 4) * Geo::WCOLS;
+    constexpr uint32_t NCOLS = COLS_NEEDED <= 32 ? 32 : COLS_NEEDED <= 64 ? 64 : COLS_NEEDED <= 128 ? 128 : COLS_NEEDED <= 256 ? 256 : 512;
+    static_assert(COLS_NEEDED <= 512, "tensor memory: 512 columns per SM");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t tslot;
+
+    const int unit = threadIdx.x / 96;
+    const int q = (threadIdx.x % 96) / 32;          // warp of the unit = sub-transform q
+    const int warp = threadIdx.x / 32;
+    const int lane = threadIdx.x & 31;
+    const int lg = lane / G, t = lane % G;
+    const int lgcol = lg * G;
+    const int tl = q * G + t;                        // thread within the line pair
+
+    unsigned char* ubase = smem_raw + (size_t)unit * Geo::UNIT_BYTES;
+    cx<T>* In = reinterpret_cast<cx<T>*>(ubase);                       // [PL] x (2 slots x 2 lines x L), pitch LGPITCH
+    cx<T>* Ex = In + Geo::IN_UNIT;                                      // [3][REGION]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Ex + 3 * REGION);      // [PL][2]
+    cx<T>* Sw = Ex + q * REGION;
+    const cx<T>* Ulg = In + (size_t)lg * Geo::LGPITCH;
+    uint64_t* bar_lg = bars + lg * 2;
+    const int bar_id = 1 + unit;
+    const long cs = MM * L;                          // component stride (complex) of in and out
+    constexpr uint32_t LINE_BYTES = (uint32_t)(L * sizeof(cx<T>));
+
+    // input job jn = 3 * it + k of this lane group: k = 0 (u3A, u3B), 1 (u1A, u2A), 2 (u1B, u2B); slot jn & 1
+    auto issue = [&](long pair, int k, int jn) {
+        const long lineA = 2 * pair;
+        const long b = lineA / MM, pp = lineA % MM;
+        const cx<T>* src = in + (b * 3 * MM + pp) * L;
+        cx<T>* dst = const_cast<cx<T>*>(Ulg) + (jn & 1) * SLOT;
+        uint64_t* bar = bar_lg + (jn & 1);
+        mbar_expect_tx(bar, 2 * LINE_BYTES);
+        if (k == 0) {
+            bulk_g2s(dst, src + 2 * cs, 2 * LINE_BYTES, bar);            // u3 of lines A and B are contiguous
+        } else {
+            const cx<T>* s1 = src + (k == 2 ? L : 0);
+            bulk_g2s(dst, s1, LINE_BYTES, bar);
+            bulk_g2s(dst + L, s1 + cs, LINE_BYTES, bar);
+        }
+    };
+
+    if (threadIdx.x % 96 == 0) {
+        for (int k = 0; k < 2 * PL; ++k) mbar_init(bars + k, 1);
+        mbar_fence_init();
+    }
+    if (warp == 0) tmem_alloc(&tslot, NCOLS);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    // this warp's TMEM window: lanes 32 (warp % 4) .. +31, columns (warp / 4) * WCOLS .. + WCOLS: four fields of C16 columns
+    const uint32_t tbase = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * Geo::WCOLS;
+
+    const long stride = (long)gridDim.x * UNITS * PL;
+    long pair = ((long)blockIdx.x * UNITS + unit) * PL + lg;      // (MM/2) % PL == 0: validity is uniform over the unit
+    const bool issuer = (q == 0 && t == 0);
+    if (issuer && pair < total_pairs) { issue(pair, 0, 0); issue(pair, 1, 1); }
+
+    for (int it = 0; pair < total_pairs; pair += stride, ++it) {
+        const long lineA = 2 * pair;
+        const long b = lineA / MM, pp = lineA % MM;
+        cx<T>* OpA = out + (b * 5 * MM + pp) * L;
+        const bool more = pair + stride < total_pairs;
+
+#pragma unroll 1
+        for (int job = 0; job < 8; ++job) {
+            const bool inv = (0x13 >> job) & 1;          // jobs 0, 1, 4
+            // fields (TMEM column offsets in units of C16): see the job table at the top
+            //   job:   0     1     2      3      4     5      6      7
+            //   fa     0     2     2      2      3     3      3      2      (inverse: re ->; forward: x)
+            //   fb     1     3     3      3      0     0      0      3      (inverse: im ->; forward: y)
+            //   fc     -     -     0      0      -     1      1      -      (forward: z)
+            const uint32_t fa = tbase + C16 * ((0x23332220u >> (4 * job)) & 15u);
+            const uint32_t fb = tbase + C16 * ((0x30003331u >> (4 * job)) & 15u);
+            const uint32_t fc = tbase + C16 * (job >= 4 ? 1u : 0u);
+            cx<T> v[16];
+            if (inv) {
+                const int k = job == 0 ? 0 : (job == 1 ? 1 : 2);
+                const int jn = 3 * it + k;
+                mbar_wait(bar_lg + (jn & 1), (uint32_t)((jn >> 1) & 1));
+                const cx<T>* Ua = Ulg + (jn & 1) * SLOT;
+                const cx<T>* Ub = Ua + L;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int n = t + G * j;
+                    const cx<T> pa = Ua[n], pb = Ub[n];
+                    cx<T> a, c;
+                    if (n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
+                    else {
+                        const cx<T> ma = Ua[L - n], mb = Ub[L - n];
+                        a = mk<T>(pa.x - pb.y, pa.y + pb.x);
+                        c = mk<T>(ma.x + mb.y, mb.x - ma.y);
+                    }
+                    v[j] = prune3(a, c, q, n, tw);
+                }
+            } else {
+                // products of the physical fields, conjugated (forward through the inverse butterflies), in natural order
+                const int kind = job == 7 ? 2 : ((job == 2 || job == 5) ? 0 : 1);
+                T X[16], Y[16];
+                tmem_load16(fa, X);
+                tmem_load16(fb, Y);
+                if (kind == 2) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[j] = mk<T>(X[zp_perm<G>(j)], -Y[zp_perm<G>(j)]);
+                } else {
+                    T Z[16];
+                    tmem_load16(fc, Z);
+                    if (kind == 0) {
+                        auto lmax = sq_bits((T)0);
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int i = zp_perm<G>(j);
+                            const T x2 = X[i] * X[i], y2 = Y[i] * Y[i], z2 = Z[i] * Z[i];
+                            lmax = umax_bits(lmax, sq_bits(x2 + y2 + z2));
+                            v[j] = mk<T>(x2 - z2, z2 - y2);
+                        }
+                        if (umax2 != nullptr) {
+                            lmax = warp_max_bits(lmax);
+                            if (lane == 0) atomic_max_sq(umax2 + b, lmax);
+                        }
+                    } else {
+                        T W[16];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int i = zp_perm<G>(j);
+                            v[j] = mk<T>(X[i] * Y[i], -(X[i] * Z[i]));
+                        }
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) W[i] = Y[i] * Z[i];
+                        tmem_store16(fa, W);          // T23 of this line replaces u1 (no longer needed)
+                    }
+                }
+            }
+            zp_transform<T, L>(v, Sw, lane, t, lgcol, tw.z16);
+            if (inv) {
+                T X[16], Y[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) { X[i] = v[i].x; Y[i] = v[i].y; }
+                tmem_store16(fa, X);
+                tmem_store16(fb, Y);
+                tmem_wait_st();
+            } else {
+                tmem_wait_st();
+                // G_q[k] = conj(v) W^{-qk} into this warp's region, natural order: k = t + G j at row j, column lane
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int k = t + G * j;
+                    const cx<T> y = v[zp_perm<G>(j)];
+                    cx<T> w = mk<T>(y.x, -y.y);
+                    if (q > 0) {
+                        const cx<T> r = ldg((q == 1 ? tw.w3a : tw.w3b) + k);
+                        w = mk<T>(y.x * r.x - y.y * r.y, -(y.x * r.y + y.y * r.x));
+                    }
+                    Sw[j * 32 + (lane ^ (j & 7))] = w;
+                }
+                named_bar_sync(bar_id, 96);
+                // all three warps are past the inverse jobs that read the input slots: refill them
+                if (issuer) {
+                    if (job == 2) { issue(pair, 2, 3 * it + 2); if (more) issue(pair + stride, 0, 3 * it + 3); }
+                    if (job == 5 && more) issue(pair + stride, 1, 3 * it + 4);
+                }
+                cx<T>* Oa;
+                cx<T>* Ob;
+                if (job == 7) { Oa = OpA + 4 * cs; Ob = Oa + L; }
+                else {
+                    cx<T>* Ol = OpA + (job >= 4 ? L : 0);
+                    const bool p0 = (job == 2 || job == 5);
+                    Oa = Ol + (p0 ? 0 : 1) * cs;
+                    Ob = Ol + (p0 ? 3 : 2) * cs;
+                }
+                zp_combine_store<T, L>(Ex, lgcol, Oa, Ob, tl);
+                named_bar_sync(bar_id, 96);  // combine reads done before the regions are reused
+            }
+        }
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tslot, NCOLS);
+}
+
+}  // namespace ns

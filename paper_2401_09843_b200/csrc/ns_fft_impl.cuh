@@ -4,8 +4,7 @@
 #include "kernels_z.cuh"
 #include "kernels_zfused.cuh"
 #include "kernels_zfused8.cuh"
-#include "kernels_zfused16.cuh"
-#include "kernels_zfused16t.cuh"
+#include "kernels_zpair.cuh"
 #include <cstdlib>
 #include <cstring>
 #include "ns_internal.h"
@@ -94,25 +93,18 @@ static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, 
 }
 
 template <typename T, int L>
-static cudaError_t z_fused_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+static cudaError_t z_fused_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
                              Twiddles<T> tw) {
     using C = Cfg<L>;
     constexpr int LPB = C::lpbf();
-    constexpr bool SEP = false;
-    auto k = z_fused_kernel<T, L, C::R1, C::R2, LPB, C::minbf(), SEP>;
-    const size_t smem = (size_t)LPB * (3 * L + (SEP ? 2 : 1) * 3 * C::R1 * (C::R2 + 1)) * sizeof(cx<T>) + 16;
+    auto k = z_fused_kernel<T, L, C::R1, C::R2, LPB, C::minbf()>;
+    const size_t smem = (size_t)LPB * (3 * L + 3 * C::R1 * (C::R2 + 1)) * sizeof(cx<T>) + 16;
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     if ((MM % LPB) != 0) return cudaErrorInvalidValue;
     const long tiles = MM * batch / LPB;
-    static int num_sms = 0;
-    if (num_sms == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-    }
     int occ = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 3 * C::P * LPB, smem);
     if (e != cudaSuccess) return e;
@@ -126,11 +118,9 @@ static cudaError_t z_fused_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long 
 // warp-synchronous fused z kernel for L >= 64
 template <int L> struct Z8Cfg;
 template <> struct Z8Cfg<64>  { static constexpr int LPB = 8, MINB = 2; };
-template <> struct Z8Cfg<128> { static constexpr int LPB = 4, MINB = 2; };
-template <> struct Z8Cfg<256> { static constexpr int LPB = 2, MINB = 2; };
 
 template <typename T, int L>
-static cudaError_t z_fused8_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+static cudaError_t z_fused8_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
                               Twiddles<T> tw) {
     constexpr int LPB = Z8Cfg<L>::LPB;
     constexpr int G = L / 8, R3 = G / 8;
@@ -140,12 +130,6 @@ static cudaError_t z_fused8_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long
     if (e != cudaSuccess) return e;
     if ((MM % LPB) != 0) return cudaErrorInvalidValue;
     const long lines = MM * batch;
-    static int num_sms = 0;
-    if (num_sms == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-    }
     int occ = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 3 * G * LPB, smem);
     if (e != cudaSuccess) return e;
@@ -156,36 +140,23 @@ static cudaError_t z_fused8_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long
     return cudaGetLastError();
 }
 
-// 16-values-per-lane fused z kernel with the physical fields parked in tensor memory, L >= 128
+// line-pair fused z kernel (kernels_zpair.cuh), L in {64, 128, 256}: one persistent block of UNITS units per SM slot
 template <typename T, int L>
-static cudaError_t z_fused16t_L(cudaStream_t st, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
-                                Twiddles<T> tw) {
-    using Geo = Z16Geo<L>;
-    constexpr int LPB = Geo::UL;
-    constexpr int MINB = sizeof(T) == 8 ? 4 : 6;
-    constexpr int TMEM_COLS = 3 * 16 * sizeof(T) / 4 <= 64 ? 64 : 128;
-    auto k = z_fused16t_kernel<T, L, MINB>;
-    const size_t smem = (size_t)LPB * 3 * (L + Geo::SZ) * sizeof(cx<T>) + (size_t)LPB * 8 + 16;
+static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
+                            Twiddles<T> tw) {
+    using Geo = ZPGeo<T, L>;
+    constexpr int UNITS = 4;
+    auto k = z_pair_kernel<T, L, UNITS>;
+    const size_t smem = (size_t)UNITS * Geo::UNIT_BYTES;
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
-    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
-    const long lines = MM * batch;
-    static int num_sms = 0;
-    if (num_sms == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-    }
-    // The occupancy API reports 1 CTA/SM for a kernel that allocates tensor memory; the real limits are the
-    // launch bound (registers), shared memory (227 KB per SM, 1 KB reserved per CTA) and 512 TMEM columns.
-    int occ = MINB;
-    const int by_smem = (int)((227 * 1024) / (smem + 1024));
-    if (occ > by_smem) occ = by_smem;
-    if (occ > 512 / TMEM_COLS) occ = 512 / TMEM_COLS;
-    if (occ < 1) occ = 1;
-    long grid = (long)num_sms * occ;
-    if (grid > lines / LPB) grid = lines / LPB;
-    k<<<(unsigned)grid, 96, smem, st>>>(in, out, MM, lines, umax2, tw);
+    if ((MM % 2) != 0 || ((MM / 2) % Geo::PL) != 0) return cudaErrorInvalidValue;
+    const long pairs = MM * batch / 2;
+    const long per_block = (long)UNITS * Geo::PL;
+    long grid = num_sms;   // one block per SM: registers (384 threads x 168), shared memory and 512 TMEM columns all say so
+    const long need = (pairs + per_block - 1) / per_block;
+    if (grid > need) grid = need;
+    k<<<(unsigned)grid, 96 * UNITS, smem, st>>>(in, out, MM, pairs, umax2, tw);
     return cudaGetLastError();
 }
 
@@ -199,16 +170,6 @@ static cudaError_t z_fused16t_L(cudaStream_t st, const cx<T>* in, cx<T>* out, lo
         case 256: return CALL(256);                              \
         default: return cudaErrorInvalidValue;                   \
     }
-
-// NS_COLVARIANT=reg selects the register / shared-memory column kernels for the long lines too (A/B comparison)
-static int col_variant() {
-    static int variant = -1;
-    if (variant < 0) {
-        const char* v = getenv("NS_COLVARIANT");
-        variant = (v != nullptr && strcmp(v, "reg") == 0) ? 0 : 1;
-    }
-    return variant;
-}
 
 template <typename T>
 static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab) {
@@ -228,7 +189,7 @@ cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
     // measured (profiles/): parking pays at L = 128 (0.264 -> 0.216 ms at 256^3); at L = 256 the register kernel is faster
-    if (col_variant() == 1 && L == 128) return col_inv_tmem_L<T, 128>(st, in, out, g, tw);
+    if (L == 128) return col_inv_tmem_L<T, 128>(st, in, out, g, tw);
 #define CALL(LL) col_inv_L<T, LL>(st, in, out, g, tw)
     NS_DISPATCH_L(L, CALL)
 #undef CALL
@@ -239,34 +200,29 @@ cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
-    if (col_variant() == 1 && L == 128) return col_fwd_tmem_L<T, 128>(st, in, out, g, scale, tw);
-    if (col_variant() == 1 && L == 256) return col_fwd_tmem_L<T, 256>(st, in, out, g, scale, tw);
+    if (L == 128) return col_fwd_tmem_L<T, 128>(st, in, out, g, scale, tw);
+    if (L == 256) return col_fwd_tmem_L<T, 256>(st, in, out, g, scale, tw);
 #define CALL(LL) col_fwd_L<T, LL>(st, in, out, g, scale, tw)
     NS_DISPATCH_L(L, CALL)
 #undef CALL
 }
 
 template <typename T>
-cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
+cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw) {
-    // NS_ZVARIANT=8 selects the 8-values-per-lane kernel for L >= 128 as well (A/B comparison, profiles/)
-    static int variant = -1;
-    if (variant < 0) {
-        const char* v = getenv("NS_ZVARIANT");
-        variant = (v != nullptr && strcmp(v, "8") == 0) ? 0 : 1;
-    }
-    if (variant == 1) {
-        if (L == 128) return z_fused16t_L<T, 128>(st, in, out, MM, batch, umax2, tw);
-        if (L == 256) return z_fused16t_L<T, 256>(st, in, out, MM, batch, umax2, tw);
-    }
-    if (L == 64) return z_fused8_L<T, 64>(st, in, out, MM, batch, umax2, tw);
-    if (L == 128) return z_fused8_L<T, 128>(st, in, out, MM, batch, umax2, tw);
-    if (L == 256) return z_fused8_L<T, 256>(st, in, out, MM, batch, umax2, tw);
-    // short lines: block-synchronous kernel
     switch (L) {
-        case 8: return z_fused_L<T, 8>(st, in, out, MM, batch, umax2, tw);
-        case 16: return z_fused_L<T, 16>(st, in, out, MM, batch, umax2, tw);
-        case 32: return z_fused_L<T, 32>(st, in, out, MM, batch, umax2, tw);
+        case 256: return z_pair_L<T, 256>(st, num_sms, in, out, MM, batch, umax2, tw);
+        case 128: return z_pair_L<T, 128>(st, num_sms, in, out, MM, batch, umax2, tw);
+#ifdef NS_DEV_SWITCHES   // A/B builds only (never defined by paper_2401_09843_b200/build.py)
+        case 64: return getenv("NS_Z64") && !strcmp(getenv("NS_Z64"), "8") ? z_fused8_L<T, 64>(st, num_sms, in, out, MM, batch, umax2, tw)
+                                                                            : z_pair_L<T, 64>(st, num_sms, in, out, MM, batch, umax2, tw);
+#else
+        case 64: return z_pair_L<T, 64>(st, num_sms, in, out, MM, batch, umax2, tw);
+#endif
+        // short lines: block-synchronous kernel
+        case 8: return z_fused_L<T, 8>(st, num_sms, in, out, MM, batch, umax2, tw);
+        case 16: return z_fused_L<T, 16>(st, num_sms, in, out, MM, batch, umax2, tw);
+        case 32: return z_fused_L<T, 32>(st, num_sms, in, out, MM, batch, umax2, tw);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -276,7 +232,7 @@ cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
                                            long, Twiddles<T>);                                                     \
     template cudaError_t launch_col_fwd<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, T, Twiddles<T>);                                                  \
-    template cudaError_t launch_z_fused<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, unsigned long long*,   \
+    template cudaError_t launch_z_fused<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*, \
                                            Twiddles<T>);
 
 }  // namespace ns

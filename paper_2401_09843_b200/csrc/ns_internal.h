@@ -24,7 +24,7 @@ struct Twiddles {
     const cx<T>* z8A;
     const cx<T>* z8B;
     const cx<T>* z8C;
-    // table of the 16-values-per-lane z kernel (kernels_zfused16.cuh), G = L/16 (L >= 128 only):
+    // table of the 16-values-per-lane z kernel (kernels_zpair.cuh), G = L/16 (L >= 64 only):
     //   z16[r1*G + t] = w_L^{r1 t},  r1 < 16, t < G
     const cx<T>* z16;
 };
@@ -48,10 +48,10 @@ cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, 
 template <typename T>
 cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw);
-// fused a3+a4 (kernels_zfused.cuh, kernels_zfused8.cuh): in [batch][3][MM][L] -> out [batch][NS_NFLUX][MM][L];
-// persistent grid sized from the SM count and the achievable CTAs per SM.  umax2 may be NULL.
+// fused a3+a4 (kernels_zpair.cuh; kernels_zfused.cuh for L <= 32): in [batch][3][MM][L] -> out [batch][NS_NFLUX][MM][L];
+// persistent grid sized from num_sms (the SM count of the solver's device) and the CTAs per SM.  umax2 may be NULL.
 template <typename T>
-cudaError_t launch_z_fused(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
+cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw);
 
 }  // namespace ns

@@ -115,6 +115,7 @@ template <typename T>
 class Solver final : public ns_solver {
 public:
     int N, L, M, H, batch;
+    int device = 0, num_sms = 0;   // the device the handle was created on (no process-wide caches)
     ns_params prm;
     cudaStream_t st;
     bool has_state = false;
@@ -174,6 +175,8 @@ public:
     static unsigned blocks_for(long total, int threads) { return (unsigned)((total + threads - 1) / threads); }
 
     int init() {
+        NS_CK(cudaGetDevice(&device));
+        NS_CK(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, device));
         const size_t b = (size_t)batch;
         nS = b * 3 * N * N * H;
         // Workspaces shared by all passes: X <- a1 out / a5 out / unpadded-FFT cube / R,
@@ -247,7 +250,7 @@ public:
         if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
         ++launches;
         prof.tick(2, st);
-        e = launch_z_fused<T>(st, L, Y, Z, (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
+        e = launch_z_fused<T>(st, num_sms, L, Y, Z, (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a3+a4 z_fused");
         ++launches;
         if (upto <= 3) { prof.tick(-1, st); return NS_OK; }

@@ -43,7 +43,7 @@ inline std::vector<cx<T>> build_twiddle_block(int L) {
         for (int rA = 0; rA < 8; ++rA)
             for (int tb = 0; tb < R3; ++tb) h[(size_t)6 * L + (size_t)rA * R3 + tb] = root((long)rA * tb, G);
     }
-    if (L >= 128) {
+    if (L >= 64) {
         const int G = L / 16;
         for (int r1 = 0; r1 < 16; ++r1)
             for (int t = 0; t < G; ++t) h[(size_t)7 * L + (size_t)r1 * G + t] = root((long)r1 * t, L);

@@ -16,3 +16,10 @@ def pytest_configure(config):
 def oracle():
     from oracle import ns_oracle
     return ns_oracle
+
+
+@pytest.fixture(scope="session")
+def k53_512():
+    """BASELINE.json configs[4] input (512^3 Gaussian k^-5/3 field, seed 5): 40 s of numpy FFTs, shared by the full-size tests."""
+    from paper_2401_09843_b200 import inputs
+    return inputs.gaussian_k53(512, seed=5)

@@ -131,13 +131,13 @@ def test_config4_one_sample_replayed_10_steps(ns, oracle):
 
 # ------------------------------------------------------------------------------------------------ config 5
 @pytest.mark.parametrize("N", [256, 512])
-def test_full_size_stratified_sampled_rhs(ns, oracle, N):
+def test_full_size_stratified_sampled_rhs(ns, oracle, k53_512, N):
     """256^3 and 512^3 (configs[4] input), same launch configuration as bench.py: ns_rhs at >= 512 stratified sampled
     wavenumbers against the oracle's direct truncated convolution sum (orc_rhs_at_modes): relative L2 over the sample
     <= 1e-12 and every single sampled entry within 1e-12 of max|R|; then, on the WHOLE array, the energy identity P4
     of the inviscid RHS (a statement about every entry of the transforms: any aliasing or tile fault breaks it), the
     masks, and the fused RK3 step against eq. 2.6 assembled on the host from ns_rhs evaluations (pins the axpy of a7)."""
-    u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5) if N == 256 else inputs.gaussian_k53(N, seed=5)
+    u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5) if N == 256 else k53_512
     kw = dict(eps=0.05, s=1.0)
     s = ns.Solver(N, **kw)
     s.set_initial(u[None])
