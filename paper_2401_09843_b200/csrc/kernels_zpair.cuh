@@ -71,10 +71,14 @@ __device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__
 #pragma unroll
     for (int h = 0; h < Hc; ++h) {
         const int row = t + G * h;
-        const cx<T>* Sr = Sw + row * 32 + lgcol;
+        const cx<T>* Sr = Sw + row * 32;
         const int rm = row & 7;
 #pragma unroll
-        for (int tt = 0; tt < G; ++tt) v[h * G + tt] = Sr[(tt & ~7) | ((tt & 7) ^ rm)];
+        for (int tt = 0; tt < G; ++tt) {
+            // column (lgcol + tt) ^ rm; for G >= 8 the XOR touches only the low three bits of tt (lgcol is a multiple of 8)
+            if constexpr (G >= 8) v[h * G + tt] = Sr[lgcol + ((tt & ~7) | ((tt & 7) ^ rm))];
+            else v[h * G + tt] = Sr[(lgcol + tt) ^ rm];
+        }
     }
     __syncwarp();
 #pragma unroll
@@ -132,7 +136,7 @@ __device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, i
 // 11 12 13 22 23).  total_pairs = batch * MM / 2 line pairs; (MM / 2) % (32 / G) == 0 (a warp never straddles two samples).
 template <typename T, int L, int UNITS>
 __global__ void __launch_bounds__(96 * UNITS, 1)
-z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, long total_pairs,
+z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, unsigned total_pairs,
               unsigned long long* __restrict__ umax2, Twiddles<T> tw) {
     using Geo = ZPGeo<T, L>;
     constexpr int G = Geo::G, PL = Geo::PL, REGION = Geo::REGION, SLOT = Geo::SLOT;
@@ -160,24 +164,27 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, lo
     const cx<T>* Ulg = In + (size_t)lg * Geo::LGPITCH;
     uint64_t* bar_lg = bars + lg * 2;
     const int bar_id = 1 + unit;
-    const long cs = MM * L;                          // component stride (complex) of in and out
+    const long cs = (long)MM * L;                    // component stride (complex) of in and out
     constexpr uint32_t LINE_BYTES = (uint32_t)(L * sizeof(cx<T>));
 
+    // radix-3 pruning coefficients of this warp: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q}
+    const T alpha = q == 0 ? (T)1 : (T)-0.5;
+    const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
+    const cx<T>* w3q = q == 1 ? tw.w3a : tw.w3b;
+
     // input job jn = 3 * it + k of this lane group: k = 0 (u3A, u3B), 1 (u1A, u2A), 2 (u1B, u2B); slot jn & 1
-    auto issue = [&](long pair, int k, int jn) {
-        const long lineA = 2 * pair;
-        const long b = lineA / MM, pp = lineA % MM;
-        const cx<T>* src = in + (b * 3 * MM + pp) * L;
+    auto issue = [&](unsigned pr, int k, int jn) {
+        const unsigned lineA = 2 * pr;
+        const unsigned b = lineA / MM;                                  // in offset: (b 3 MM + pp) L = (lineA + 2 b MM) L
+        const cx<T>* src = in + ((long)lineA + 2 * (long)b * MM) * L;
         cx<T>* dst = const_cast<cx<T>*>(Ulg) + (jn & 1) * SLOT;
         uint64_t* bar = bar_lg + (jn & 1);
         mbar_expect_tx(bar, 2 * LINE_BYTES);
-        if (k == 0) {
-            bulk_g2s(dst, src + 2 * cs, 2 * LINE_BYTES, bar);            // u3 of lines A and B are contiguous
-        } else {
-            const cx<T>* s1 = src + (k == 2 ? L : 0);
-            bulk_g2s(dst, s1, LINE_BYTES, bar);
-            bulk_g2s(dst + L, s1 + cs, LINE_BYTES, bar);
-        }
+        // k = 0: u3 of lines A and B (contiguous); k = 1, 2: u1 and u2 of line A / B (a component stride apart)
+        const cx<T>* s1 = src + (k == 0 ? 2 * cs : (k == 2 ? L : 0));
+        const long second = k == 0 ? L : cs;
+        bulk_g2s(dst, s1, LINE_BYTES, bar);
+        bulk_g2s(dst + L, s1 + second, LINE_BYTES, bar);
     };
 
     if (threadIdx.x % 96 == 0) {
@@ -191,15 +198,18 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, lo
     // this warp's TMEM window: lanes 32 (warp % 4) .. +31, columns (warp / 4) * WCOLS .. + WCOLS: four fields of C16 columns
     const uint32_t tbase = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * Geo::WCOLS;
 
-    const long stride = (long)gridDim.x * UNITS * PL;
-    long pair = ((long)blockIdx.x * UNITS + unit) * PL + lg;      // (MM/2) % PL == 0: validity is uniform over the unit
+    const unsigned stride = gridDim.x * UNITS * PL;
+    unsigned pair = (blockIdx.x * UNITS + unit) * PL + lg;        // (MM/2) % PL == 0: validity is uniform over the unit
     const bool issuer = (q == 0 && t == 0);
-    if (issuer && pair < total_pairs) { issue(pair, 0, 0); issue(pair, 1, 1); }
+    if (issuer && pair < total_pairs) {
+#pragma unroll 1
+        for (int k = 0; k < 2; ++k) issue(pair, k, k);
+    }
 
     for (int it = 0; pair < total_pairs; pair += stride, ++it) {
-        const long lineA = 2 * pair;
-        const long b = lineA / MM, pp = lineA % MM;
-        cx<T>* OpA = out + (b * 5 * MM + pp) * L;
+        const unsigned lineA = 2 * pair;
+        const unsigned b = lineA / MM;
+        cx<T>* OpA = out + ((long)lineA + 4 * (long)b * MM) * L;        // out offset: (b 5 MM + pp) L
         const bool more = pair + stride < total_pairs;
 
 #pragma unroll 1
@@ -220,18 +230,19 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, lo
                 mbar_wait(bar_lg + (jn & 1), (uint32_t)((jn >> 1) & 1));
                 const cx<T>* Ua = Ulg + (jn & 1) * SLOT;
                 const cx<T>* Ub = Ua + L;
+                // a_n = Ua[n] + i Ub[n], c_n = conj(Ua[L-n]) + i conj(Ub[L-n]) (kernels_z.cuh); n = 0: real parts only, c = 0
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
                     const int n = t + G * j;
                     const cx<T> pa = Ua[n], pb = Ub[n];
-                    cx<T> a, c;
-                    if (n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
-                    else {
-                        const cx<T> ma = Ua[L - n], mb = Ub[L - n];
-                        a = mk<T>(pa.x - pb.y, pa.y + pb.x);
-                        c = mk<T>(ma.x + mb.y, mb.x - ma.y);
-                    }
-                    v[j] = prune3(a, c, q, n, tw);
+                    const cx<T> ma = Ua[(L - n) & (L - 1)], mb = Ub[(L - n) & (L - 1)];
+                    cx<T> a = mk<T>(pa.x - pb.y, pa.y + pb.x);
+                    cx<T> c = mk<T>(ma.x + mb.y, mb.x - ma.y);
+                    if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
+                    // z = a + c (alpha + i beta)
+                    cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
+                    if (q > 0) z = cmul(z, ldg(w3q + n));
+                    v[j] = z;
                 }
             } else {
                 // products of the physical fields, conjugated (forward through the inverse butterflies), in natural order
@@ -246,17 +257,18 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, lo
                     T Z[16];
                     tmem_load16(fc, Z);
                     if (kind == 0) {
-                        auto lmax = sq_bits((T)0);
+                        if (umax2 != nullptr) {      // stage 1 only: max |u|^2 of the pair's two lines (same sample)
+                            auto lmax = sq_bits((T)0);
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) lmax = umax_bits(lmax, sq_bits(X[i] * X[i] + Y[i] * Y[i] + Z[i] * Z[i]));
+                            lmax = warp_max_bits(lmax);
+                            if (lane == 0) atomic_max_sq(umax2 + b, lmax);
+                        }
 #pragma unroll
                         for (int j = 0; j < 16; ++j) {
                             const int i = zp_perm<G>(j);
-                            const T x2 = X[i] * X[i], y2 = Y[i] * Y[i], z2 = Z[i] * Z[i];
-                            lmax = umax_bits(lmax, sq_bits(x2 + y2 + z2));
-                            v[j] = mk<T>(x2 - z2, z2 - y2);
-                        }
-                        if (umax2 != nullptr) {
-                            lmax = warp_max_bits(lmax);
-                            if (lane == 0) atomic_max_sq(umax2 + b, lmax);
+                            const T z2 = Z[i] * Z[i];
+                            v[j] = mk<T>(X[i] * X[i] - z2, z2 - Y[i] * Y[i]);
                         }
                     } else {
                         T W[16];
@@ -288,16 +300,18 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, lo
                     const cx<T> y = v[zp_perm<G>(j)];
                     cx<T> w = mk<T>(y.x, -y.y);
                     if (q > 0) {
-                        const cx<T> r = ldg((q == 1 ? tw.w3a : tw.w3b) + k);
+                        const cx<T> r = ldg(w3q + k);
                         w = mk<T>(y.x * r.x - y.y * r.y, -(y.x * r.y + y.y * r.x));
                     }
                     Sw[j * 32 + (lane ^ (j & 7))] = w;
                 }
                 named_bar_sync(bar_id, 96);
                 // all three warps are past the inverse jobs that read the input slots: refill them
-                if (issuer) {
-                    if (job == 2) { issue(pair, 2, 3 * it + 2); if (more) issue(pair + stride, 0, 3 * it + 3); }
-                    if (job == 5 && more) issue(pair + stride, 1, 3 * it + 4);
+                if (issuer && (job == 2 || job == 5)) {
+                    // job 2: (u1B, u2B) of this pair and (u3A, u3B) of the next one; job 5: (u1A, u2A) of the next one
+                    const int first = job == 2 ? 2 : 4, last = !more ? 2 : (job == 2 ? 3 : 4);
+#pragma unroll 1
+                    for (int kk = first; kk <= last; ++kk) issue(kk >= 3 ? pair + stride : pair, kk >= 3 ? kk - 3 : kk, 3 * it + kk);
                 }
                 cx<T>* Oa;
                 cx<T>* Ob;

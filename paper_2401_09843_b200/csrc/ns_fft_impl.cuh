@@ -152,11 +152,12 @@ static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>
     if (e != cudaSuccess) return e;
     if ((MM % 2) != 0 || ((MM / 2) % Geo::PL) != 0) return cudaErrorInvalidValue;
     const long pairs = MM * batch / 2;
+    if (MM * batch >= (1L << 31)) return cudaErrorInvalidValue;   // line indices are 32 bit in the kernel
     const long per_block = (long)UNITS * Geo::PL;
     long grid = num_sms;   // one block per SM: registers (384 threads x 168), shared memory and 512 TMEM columns all say so
     const long need = (pairs + per_block - 1) / per_block;
     if (grid > need) grid = need;
-    k<<<(unsigned)grid, 96 * UNITS, smem, st>>>(in, out, MM, pairs, umax2, tw);
+    k<<<(unsigned)grid, 96 * UNITS, smem, st>>>(in, out, (unsigned)MM, (unsigned)pairs, umax2, tw);
     return cudaGetLastError();
 }
 
