@@ -42,6 +42,26 @@ template <> __device__ __forceinline__ cx<float> ldg<float>(const cx<float>* p) 
     return mk<float>(v.x, v.y);
 }
 
+// Cache-policy variants: small tables that every warp re-reads (keep them in L1) and streamed outputs (written once, not
+// read again by this kernel: do not let them evict the tables).
+template <typename T> __device__ __forceinline__ cx<T> ldg_keep(const cx<T>* p);
+template <> __device__ __forceinline__ cx<double> ldg_keep<double>(const cx<double>* p) {
+    double x, y;
+    asm("ld.global.nc.L1::evict_last.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "l"(p));
+    return mk<double>(x, y);
+}
+template <> __device__ __forceinline__ cx<float> ldg_keep<float>(const cx<float>* p) {
+    float x, y;
+    asm("ld.global.nc.L1::evict_last.v2.f32 {%0, %1}, [%2];" : "=f"(x), "=f"(y) : "l"(p));
+    return mk<float>(x, y);
+}
+__device__ __forceinline__ void stg_stream(cx<double>* p, cx<double> v) {
+    asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void stg_stream(cx<float>* p, cx<float> v) {
+    asm volatile("st.global.L1::no_allocate.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
 // d * exp(DIR * 2 pi i * M16 / 16), M16 in [0, 8), with the trivial roots special-cased.
 // ------------------------------------------------------------------------------------------------

@@ -47,6 +47,7 @@ template <typename T, int L> struct ZPGeo {
     static constexpr size_t UNIT_BYTES = (size_t)(IN_UNIT + 3 * REGION) * sizeof(cx<T>) + (size_t)PL * 2 * sizeof(uint64_t);
     static constexpr uint32_t C16 = 16 * sizeof(T) / 4;                  // TMEM columns of 16 scalars
     static constexpr uint32_t WCOLS = 4 * C16;                           // TMEM columns per warp: 4 fields
+    static constexpr uint32_t TWCOLS = 2 * C16;                          // the thread's 16 inter-stage twiddles (complex)
 };
 
 // register holding point j (p = t + G j) after a transform: output (h, r2) <-> j = h + Hc r2 sits at h G + brev_G(r2)
@@ -55,17 +56,33 @@ template <int G> __host__ __device__ constexpr int zp_perm(int j) {
     return (j % Hc) * G + brev<G>(j / Hc);
 }
 
+// inverse of zp_perm: the point j held by register i
+template <int G> __host__ __device__ constexpr int zp_unperm(int i) {
+    for (int j = 0; j < 16; ++j)
+        if (zp_perm<G>(j) == i) return j;
+    return -1;
+}
+
 // The transform of all jobs: in v[j] = s[t + G j], out v[zp_perm(j')] = sum_n s[n] w_L^{+n k}, k = t + G j'.
 // Sw: the warp's exchange region (16 rows x 32 columns, XOR-swizzled: element (row, col) at row*32 + (col ^ (row & 7))).
+// ttw: tensor-memory address of the thread's inter-stage twiddles w_L^{r1 t}, r1 = 0..15 (they depend on the lane only, so
+// the warps that share a TMEM lane quarter share them; fetched a few at a time they cost neither registers nor L1).
 template <typename T, int L>
-__device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int t, int lgcol, const cx<T>* __restrict__ tw16) {
+__device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int t, int lgcol, uint32_t ttw) {
     constexpr int G = ZPGeo<T, L>::G, Hc = ZPGeo<T, L>::Hc;
+    constexpr int CH = tmem_cx_chunk<T>();
     fft_reg<16, +1, T>(v);
 #pragma unroll
-    for (int r1 = 0; r1 < 16; ++r1) {
-        cx<T> w = v[brev<16>(r1)];
-        if (r1 > 0) w = cmul(w, ldg(tw16 + r1 * G + t));
-        Sw[r1 * 32 + (lane ^ (r1 & 7))] = w;
+    for (int ch = 0; ch < 16 / CH; ++ch) {
+        T wr[CH], wi[CH];
+        tmem_load_cx(ttw + 16 * ch, wr, wi);
+#pragma unroll
+        for (int e = 0; e < CH; ++e) {
+            const int r1 = ch * CH + e;
+            cx<T> w = v[brev<16>(r1)];
+            if (r1 > 0) w = cmul(w, mk<T>(wr[e], wi[e]));
+            Sw[r1 * 32 + (lane ^ (r1 & 7))] = w;
+        }
     }
     __syncwarp();
 #pragma unroll
@@ -117,15 +134,15 @@ __device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, i
         const cx<T> Cm = mk<T>(f0m[it].x - (T)0.5 * Sm.x - h3 * Dm.y, f0m[it].y - (T)0.5 * Sm.y + h3 * Dm.x);
         if (n <= L / 2) {
             if (n == 0) {
-                Oa[0] = mk<T>(An.x, 0);
-                Ob[0] = mk<T>(An.y, 0);
+                stg_stream(Oa, mk<T>(An.x, 0));
+                stg_stream(Ob, mk<T>(An.y, 0));
             } else {
                 const int m = L - n;
-                Oa[n] = mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y));
-                Ob[n] = mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x));
+                stg_stream(Oa + n, mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y)));
+                stg_stream(Ob + n, mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x)));
                 if (m != n) {
-                    Oa[m] = mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y));
-                    Ob[m] = mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x));
+                    stg_stream(Oa + m, mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y)));
+                    stg_stream(Ob + m, mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x)));
                 }
             }
         }
@@ -141,8 +158,10 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     using Geo = ZPGeo<T, L>;
     constexpr int G = Geo::G, PL = Geo::PL, REGION = Geo::REGION, SLOT = Geo::SLOT;
     constexpr uint32_t C16 = Geo::C16;
+    constexpr int VPA = tmem_vals_per_access<T>();   // scalars per tensor-memory access
     constexpr uint32_t NWARPS = 3 * UNITS;
-    constexpr uint32_t COLS_NEEDED = ((NWARPS + 3) / 4) * Geo::WCOLS;
+    constexpr uint32_t FIELD_COLS = ((NWARPS + 3) / 4) * Geo::WCOLS;
+    constexpr uint32_t COLS_NEEDED = FIELD_COLS + Geo::TWCOLS;
     constexpr uint32_t NCOLS = COLS_NEEDED <= 32 ? 32 : COLS_NEEDED <= 64 ? 64 : COLS_NEEDED <= 128 ? 128 : COLS_NEEDED <= 256 ? 256 : 512;
     static_assert(COLS_NEEDED <= 512, "tensor memory: 512 columns per SM");
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -166,11 +185,6 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     const int bar_id = 1 + unit;
     const long cs = (long)MM * L;                    // component stride (complex) of in and out
     constexpr uint32_t LINE_BYTES = (uint32_t)(L * sizeof(cx<T>));
-
-    // radix-3 pruning coefficients of this warp: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q}
-    const T alpha = q == 0 ? (T)1 : (T)-0.5;
-    const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
-    const cx<T>* w3q = q == 1 ? tw.w3a : tw.w3b;
 
     // input job jn = 3 * it + k of this lane group: k = 0 (u3A, u3B), 1 (u1A, u2A), 2 (u1B, u2B); slot jn & 1
     auto issue = [&](unsigned pr, int k, int jn) {
@@ -197,6 +211,25 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     tmem_fence_after_sync();
     // this warp's TMEM window: lanes 32 (warp % 4) .. +31, columns (warp / 4) * WCOLS .. + WCOLS: four fields of C16 columns
     const uint32_t tbase = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * Geo::WCOLS;
+    const uint32_t ttw = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + FIELD_COLS;
+    if (warp < 4) {   // one warp per lane quarter parks the inter-stage twiddles of its lanes
+        constexpr int CH = tmem_cx_chunk<T>();
+#pragma unroll
+        for (int ch = 0; ch < 16 / CH; ++ch) {
+            T wr[CH], wi[CH];
+#pragma unroll
+            for (int e = 0; e < CH; ++e) {
+                const cx<T> w = ldg(tw.z16 + (ch * CH + e) * G + t);
+                wr[e] = w.x;
+                wi[e] = w.y;
+            }
+            tmem_store_cx(ttw + 16 * ch, wr, wi);
+        }
+        tmem_wait_st();
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
 
     const unsigned stride = gridDim.x * UNITS * PL;
     unsigned pair = (blockIdx.x * UNITS + unit) * PL + lg;        // (MM/2) % PL == 0: validity is uniform over the unit
@@ -230,6 +263,10 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                 mbar_wait(bar_lg + (jn & 1), (uint32_t)((jn >> 1) & 1));
                 const cx<T>* Ua = Ulg + (jn & 1) * SLOT;
                 const cx<T>* Ub = Ua + L;
+                // radix-3 pruning of this warp: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q}
+                const T alpha = q == 0 ? (T)1 : (T)-0.5;
+                const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
+                const cx<T>* w3q = q == 1 ? tw.w3a : tw.w3b;
                 // a_n = Ua[n] + i Ub[n], c_n = conj(Ua[L-n]) + i conj(Ub[L-n]) (kernels_z.cuh); n = 0: real parts only, c = 0
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
@@ -241,58 +278,65 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                     if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
                     // z = a + c (alpha + i beta)
                     cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
-                    if (q > 0) z = cmul(z, ldg(w3q + n));
+                    if (q > 0) z = cmul(z, ldg_keep(w3q + n));
                     v[j] = z;
                 }
             } else {
-                // products of the physical fields, conjugated (forward through the inverse butterflies), in natural order
+                // products of the physical fields, conjugated (forward through the inverse butterflies), in natural order;
+                // the fields are fetched from tensor memory one x16 access (VPA values) at a time to bound the live registers
                 const int kind = job == 7 ? 2 : ((job == 2 || job == 5) ? 0 : 1);
-                T X[16], Y[16];
-                tmem_load16(fa, X);
-                tmem_load16(fb, Y);
-                if (kind == 2) {
+                auto lmax = sq_bits((T)0);
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) v[j] = mk<T>(X[zp_perm<G>(j)], -Y[zp_perm<G>(j)]);
-                } else {
-                    T Z[16];
-                    tmem_load16(fc, Z);
-                    if (kind == 0) {
-                        if (umax2 != nullptr) {      // stage 1 only: max |u|^2 of the pair's two lines (same sample)
-                            auto lmax = sq_bits((T)0);
+                for (int ch = 0; ch < 16 / VPA; ++ch) {
+                    T X[VPA], Y[VPA];
+                    tmem_load_vals(fa + 16 * ch, X);
+                    tmem_load_vals(fb + 16 * ch, Y);
+                    if (kind == 2) {
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) lmax = umax_bits(lmax, sq_bits(X[i] * X[i] + Y[i] * Y[i] + Z[i] * Z[i]));
-                            lmax = warp_max_bits(lmax);
-                            if (lane == 0) atomic_max_sq(umax2 + b, lmax);
-                        }
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            const int i = zp_perm<G>(j);
-                            const T z2 = Z[i] * Z[i];
-                            v[j] = mk<T>(X[i] * X[i] - z2, z2 - Y[i] * Y[i]);
-                        }
+                        for (int e = 0; e < VPA; ++e) v[zp_unperm<G>(ch * VPA + e)] = mk<T>(X[e], -Y[e]);
                     } else {
-                        T W[16];
+                        T Z[VPA];
+                        tmem_load_vals(fc + 16 * ch, Z);
+                        if (kind == 0) {
+                            if (umax2 != nullptr) {      // stage 1 only: max |u|^2 (sticky for NaN / inf, kernels_z.cuh)
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            const int i = zp_perm<G>(j);
-                            v[j] = mk<T>(X[i] * Y[i], -(X[i] * Z[i]));
+                                for (int e = 0; e < VPA; ++e) lmax = umax_bits(lmax, sq_bits(X[e] * X[e] + Y[e] * Y[e] + Z[e] * Z[e]));
+                            }
+#pragma unroll
+                            for (int e = 0; e < VPA; ++e) {
+                                const T z2 = Z[e] * Z[e];
+                                v[zp_unperm<G>(ch * VPA + e)] = mk<T>(X[e] * X[e] - z2, z2 - Y[e] * Y[e]);
+                            }
+                        } else {
+                            T W[VPA];
+#pragma unroll
+                            for (int e = 0; e < VPA; ++e) {
+                                v[zp_unperm<G>(ch * VPA + e)] = mk<T>(X[e] * Y[e], -(X[e] * Z[e]));
+                                W[e] = Y[e] * Z[e];
+                            }
+                            tmem_store_vals(fa + 16 * ch, W);   // T23 of this line replaces u1 (no longer needed)
                         }
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) W[i] = Y[i] * Z[i];
-                        tmem_store16(fa, W);          // T23 of this line replaces u1 (no longer needed)
                     }
                 }
+                if (kind == 0 && umax2 != nullptr) {   // the lines of a warp belong to one sample
+                    lmax = warp_max_bits(lmax);
+                    if (lane == 0) atomic_max_sq(umax2 + b, lmax);
+                }
             }
-            zp_transform<T, L>(v, Sw, lane, t, lgcol, tw.z16);
+            zp_transform<T, L>(v, Sw, lane, t, lgcol, ttw);
             if (inv) {
-                T X[16], Y[16];
 #pragma unroll
-                for (int i = 0; i < 16; ++i) { X[i] = v[i].x; Y[i] = v[i].y; }
-                tmem_store16(fa, X);
-                tmem_store16(fb, Y);
+                for (int ch = 0; ch < 16 / VPA; ++ch) {
+                    T X[VPA], Y[VPA];
+#pragma unroll
+                    for (int e = 0; e < VPA; ++e) { X[e] = v[ch * VPA + e].x; Y[e] = v[ch * VPA + e].y; }
+                    tmem_store_vals(fa + 16 * ch, X);
+                    tmem_store_vals(fb + 16 * ch, Y);
+                }
                 tmem_wait_st();
             } else {
                 tmem_wait_st();
+                const cx<T>* w3q = q == 1 ? tw.w3a : tw.w3b;
                 // G_q[k] = conj(v) W^{-qk} into this warp's region, natural order: k = t + G j at row j, column lane
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
@@ -300,7 +344,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                     const cx<T> y = v[zp_perm<G>(j)];
                     cx<T> w = mk<T>(y.x, -y.y);
                     if (q > 0) {
-                        const cx<T> r = ldg(w3q + k);
+                        const cx<T> r = ldg_keep(w3q + k);
                         w = mk<T>(y.x * r.x - y.y * r.y, -(y.x * r.y + y.y * r.x));
                     }
                     Sw[j * 32 + (lane ^ (j & 7))] = w;

@@ -82,6 +82,26 @@ __device__ __forceinline__ void tmem_load16(uint32_t taddr, float (&d)[16]) {
     for (int k = 0; k < 16; ++k) d[k] = __uint_as_float(r[k]);
 }
 
+// One x16 access worth of scalars: 8 doubles or 16 floats (callers that must keep register pressure low work chunk by chunk).
+template <typename T> __host__ __device__ constexpr int tmem_vals_per_access() { return 64 / (int)sizeof(T); }
+__device__ __forceinline__ void tmem_store_vals(uint32_t taddr, const double (&d)[8]) {
+    uint32_t r[16];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        r[2 * k] = (uint32_t)__double2loint(d[k]);
+        r[2 * k + 1] = (uint32_t)__double2hiint(d[k]);
+    }
+    tmem_st16(taddr, r);
+}
+__device__ __forceinline__ void tmem_store_vals(uint32_t taddr, const float (&d)[16]) { tmem_store16(taddr, d); }
+__device__ __forceinline__ void tmem_load_vals(uint32_t taddr, double (&d)[8]) {
+    uint32_t r[16];
+    tmem_ld16(taddr, r);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) d[k] = __hiloint2double((int)r[2 * k + 1], (int)r[2 * k]);
+}
+__device__ __forceinline__ void tmem_load_vals(uint32_t taddr, float (&d)[16]) { tmem_load16(taddr, d); }
+
 // Complex values in chunks of one x16 access: 4 complex doubles or 8 complex floats (re, im interleaved).
 template <typename T> __host__ __device__ constexpr int tmem_cx_chunk() { return 16 / (2 * (int)sizeof(T) / 4); }
 __device__ __forceinline__ void tmem_store_cx(uint32_t taddr, const double (&re)[4], const double (&im)[4]) {
