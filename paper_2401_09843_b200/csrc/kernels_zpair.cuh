@@ -47,7 +47,7 @@ template <typename T, int L> struct ZPGeo {
     static constexpr size_t UNIT_BYTES = (size_t)(IN_UNIT + 3 * REGION) * sizeof(cx<T>) + (size_t)PL * 2 * sizeof(uint64_t);
     static constexpr uint32_t C16 = 16 * sizeof(T) / 4;                  // TMEM columns of 16 scalars
     static constexpr uint32_t WCOLS = 4 * C16;                           // TMEM columns per warp: 4 fields
-    static constexpr uint32_t TWCOLS = 2 * C16;                          // the thread's 16 inter-stage twiddles (complex)
+    static constexpr uint32_t TWCOLS = 4 * C16;                          // the thread's 16 inter-stage + 16 radix-3 twiddles (complex)
 };
 
 // register holding point j (p = t + G j) after a transform: output (h, r2) <-> j = h + Hc r2 sits at h G + brev_G(r2)
@@ -212,18 +212,23 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     // this warp's TMEM window: lanes 32 (warp % 4) .. +31, columns (warp / 4) * WCOLS .. + WCOLS: four fields of C16 columns
     const uint32_t tbase = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * Geo::WCOLS;
     const uint32_t ttw = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + FIELD_COLS;
-    if (warp < 4) {   // one warp per lane quarter parks the inter-stage twiddles of its lanes
+    const uint32_t tw3 = ttw + 2 * C16;
+    if (warp < 4) {   // one warp per lane quarter parks the twiddles of its lanes: w_L^{r1 t} and W^{t + G j} (both depend on the lane only)
         constexpr int CH = tmem_cx_chunk<T>();
 #pragma unroll
         for (int ch = 0; ch < 16 / CH; ++ch) {
-            T wr[CH], wi[CH];
+            T wr[CH], wi[CH], vr[CH], vi[CH];
 #pragma unroll
             for (int e = 0; e < CH; ++e) {
                 const cx<T> w = ldg(tw.z16 + (ch * CH + e) * G + t);
                 wr[e] = w.x;
                 wi[e] = w.y;
+                const cx<T> u = ldg(tw.w3a + t + G * (ch * CH + e));
+                vr[e] = u.x;
+                vi[e] = u.y;
             }
             tmem_store_cx(ttw + 16 * ch, wr, wi);
+            tmem_store_cx(tw3 + 16 * ch, vr, vi);
         }
         tmem_wait_st();
     }
@@ -263,23 +268,32 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                 mbar_wait(bar_lg + (jn & 1), (uint32_t)((jn >> 1) & 1));
                 const cx<T>* Ua = Ulg + (jn & 1) * SLOT;
                 const cx<T>* Ub = Ua + L;
-                // radix-3 pruning of this warp: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q}
+                // radix-3 pruning of this warp: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q},
+                // with the third sub-transform taken as q = -1 (physical points 3r - 1 instead of 3r + 2: the physical z order
+                // never leaves this kernel), so that both q != 0 warps use the same twiddles W^{n}, one of them conjugated
                 const T alpha = q == 0 ? (T)1 : (T)-0.5;
                 const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
-                const cx<T>* w3q = q == 1 ? tw.w3a : tw.w3b;
+                const T sg = q == 2 ? (T)-1 : (T)1;     // sign of the imaginary part of the twiddle: W^{+n} (q = 1), W^{-n} (q = -1)
                 // a_n = Ua[n] + i Ub[n], c_n = conj(Ua[L-n]) + i conj(Ub[L-n]) (kernels_z.cuh); n = 0: real parts only, c = 0
+                constexpr int CH = tmem_cx_chunk<T>();
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int n = t + G * j;
-                    const cx<T> pa = Ua[n], pb = Ub[n];
-                    const cx<T> ma = Ua[(L - n) & (L - 1)], mb = Ub[(L - n) & (L - 1)];
-                    cx<T> a = mk<T>(pa.x - pb.y, pa.y + pb.x);
-                    cx<T> c = mk<T>(ma.x + mb.y, mb.x - ma.y);
-                    if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
-                    // z = a + c (alpha + i beta)
-                    cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
-                    if (q > 0) z = cmul(z, ldg_keep(w3q + n));
-                    v[j] = z;
+                for (int ch = 0; ch < 16 / CH; ++ch) {
+                    T wr[CH], wi[CH];
+                    tmem_load_cx(tw3 + 16 * ch, wr, wi);
+#pragma unroll
+                    for (int e = 0; e < CH; ++e) {
+                        const int j = ch * CH + e;
+                        const int n = t + G * j;
+                        const cx<T> pa = Ua[n], pb = Ub[n];
+                        const cx<T> ma = Ua[(L - n) & (L - 1)], mb = Ub[(L - n) & (L - 1)];
+                        cx<T> a = mk<T>(pa.x - pb.y, pa.y + pb.x);
+                        cx<T> c = mk<T>(ma.x + mb.y, mb.x - ma.y);
+                        if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
+                        // z = a + c (alpha + i beta)
+                        cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
+                        if (q > 0) z = cmul(z, mk<T>(wr[e], sg * wi[e]));
+                        v[j] = z;
+                    }
                 }
             } else {
                 // products of the physical fields, conjugated (forward through the inverse butterflies), in natural order;
@@ -336,18 +350,24 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                 tmem_wait_st();
             } else {
                 tmem_wait_st();
-                const cx<T>* w3q = q == 1 ? tw.w3a : tw.w3b;
                 // G_q[k] = conj(v) W^{-qk} into this warp's region, natural order: k = t + G j at row j, column lane
+                constexpr int CH = tmem_cx_chunk<T>();
+                const T sg = q == 2 ? (T)-1 : (T)1;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int k = t + G * j;
-                    const cx<T> y = v[zp_perm<G>(j)];
-                    cx<T> w = mk<T>(y.x, -y.y);
-                    if (q > 0) {
-                        const cx<T> r = ldg_keep(w3q + k);
-                        w = mk<T>(y.x * r.x - y.y * r.y, -(y.x * r.y + y.y * r.x));
+                for (int ch = 0; ch < 16 / CH; ++ch) {
+                    T wr[CH], wi[CH];
+                    tmem_load_cx(tw3 + 16 * ch, wr, wi);
+#pragma unroll
+                    for (int e = 0; e < CH; ++e) {
+                        const int j = ch * CH + e;
+                        const cx<T> y = v[zp_perm<G>(j)];
+                        cx<T> w = mk<T>(y.x, -y.y);
+                        if (q > 0) {   // conj(y) conj(r) = conj(y r), r = W^{qk}
+                            const T rx = wr[e], ry = sg * wi[e];
+                            w = mk<T>(y.x * rx - y.y * ry, -(y.x * ry + y.y * rx));
+                        }
+                        Sw[j * 32 + (lane ^ (j & 7))] = w;
                     }
-                    Sw[j * 32 + (lane ^ (j & 7))] = w;
                 }
                 named_bar_sync(bar_id, 96);
                 // all three warps are past the inverse jobs that read the input slots: refill them
