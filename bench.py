@@ -40,6 +40,8 @@ WORKLOADS = {
     # the paper's own experiments, hyperviscosity order s = 1.5
     "tg3d": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.1-6.3: 256^3 perturbed 3-D Taylor-Green, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=128),
     "cyl": dict(cfg=None, N=256, batch=1, params=dict(eps=0.05, s=1.5), cfl=0.2, desc="paper eq. 6.4-6.6: 256^3 cylindrical shear flow rho=0.05, hyperviscosity eps=0.05 s=1.5, CFL 0.2", cpuN=128),
+    # a size N = 3 * 2^a, the c5 recipe at 384^3 (padded 576^3)
+    "n384": dict(cfg=None, N=384, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="NEXT-3: 384^3 = (3 * 2^7)^3 Gaussian k^-5/3 (the configs[4] recipe), hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=96),
     "c5": dict(cfg=4, N=512, batch=1, params=dict(eps=0.05, s=1.0), cfl=0.2, desc="configs[4]: 512^3 Gaussian k^-5/3, hyperviscosity eps=0.05 s=1, CFL 0.2", cpuN=128),
 }
 
@@ -56,7 +58,7 @@ def make_input(name: str, N: int, batch: int, rank: int = 0) -> np.ndarray:
         return inputs.shear_layer(N, seed=3 + o)[None]
     if name == "c4":
         return inputs.shear_layer_ensemble(N, batch, seed0=1000 + o)
-    if name == "c5":
+    if name in ("c5", "n384"):
         return inputs.gaussian_k53(N, seed=5 + o)[None]
     if name == "tg3d":
         return inputs.taylor_green_3d_perturbed(N, seed=6 + o)[None]

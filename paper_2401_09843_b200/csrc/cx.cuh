@@ -119,13 +119,13 @@ template <typename T> struct Tw16 { T p, q, c; };
 template <int DIR, int M, typename T>
 __host__ __device__ constexpr Tw16<T> tw16_split() {
     // cos, sin of m pi/8
-    constexpr long double C[16] = {1.0L, 0.92387953251128675613L, 0.70710678118654752440L, 0.38268343236508977173L, 0.0L,
-                                   -0.38268343236508977173L, -0.70710678118654752440L, -0.92387953251128675613L, -1.0L,
-                                   -0.92387953251128675613L, -0.70710678118654752440L, -0.38268343236508977173L, 0.0L,
-                                   0.38268343236508977173L, 0.70710678118654752440L, 0.92387953251128675613L};
+    constexpr double C[16] = {1.0, 0.92387953251128675613, 0.70710678118654752440, 0.38268343236508977173, 0.0,
+                                   -0.38268343236508977173, -0.70710678118654752440, -0.92387953251128675613, -1.0,
+                                   -0.92387953251128675613, -0.70710678118654752440, -0.38268343236508977173, 0.0,
+                                   0.38268343236508977173, 0.70710678118654752440, 0.92387953251128675613};
     constexpr int m = ((M % 16) + 16) % 16;
-    const long double co = C[m], si = (DIR > 0 ? 1.0L : -1.0L) * C[(m + 12) % 16];   // sin(x) = cos(x - pi/2)
-    const long double aco = co < 0 ? -co : co, asi = si < 0 ? -si : si;
+    const double co = C[m], si = (DIR > 0 ? 1.0 : -1.0) * C[(m + 12) % 16];   // sin(x) = cos(x - pi/2)
+    const double aco = co < 0 ? -co : co, asi = si < 0 ? -si : si;
     if (aco >= asi) return Tw16<T>{(T)1, (T)(si / co), (T)co};
     // |sin| > |cos|: w = si (co/si + i)
     return Tw16<T>{(T)(co / si), (T)1, (T)si};
@@ -188,17 +188,61 @@ __device__ __forceinline__ void fft16_fma(cx<T>* v) {
     fft16_stage_b<DIR, 3, T>(v);
 }
 
-// In-place decimation-in-frequency FFT of v[0..R), R in {1,2,4,8,16}, kernel exp(DIR 2 pi i jk/R).
-// Output X[k] is left at v[brev<R>(k)].
+// radix-3 butterfly X_k = sum_n x_n w3^{DIR nk} in place (12 fp operations)
+template <int DIR, typename T>
+__device__ __forceinline__ void bf3(cx<T>& x0, cx<T>& x1, cx<T>& x2) {
+    constexpr T h = (T)DIR * (T)0.86602540378443864676L;
+    const cx<T> s = x1 + x2, d = x1 - x2;
+    const cx<T> m = mk<T>(x0.x - (T)0.5 * s.x, x0.y - (T)0.5 * s.y);
+    x0 = x0 + s;
+    x1 = mk<T>(m.x - h * d.y, m.y + h * d.x);
+    x2 = mk<T>(m.x + h * d.y, m.y - h * d.x);
+}
+
+// Lengths 6 and 12 by the prime-factor algorithm (3 x 2, 3 x 4: no twiddle factors).  Input index n = (N2 n1 + 3 n2) mod N
+// (n1 < 3, n2 < N2), output index k = (N2' k1 + 3' k2) mod N by the Chinese remainder theorem; everything in place, so that
+// X[k] ends at register (N2 (k mod 3) + 3 (k mod N2)) mod N.
+template <int R, int DIR, typename T>
+__device__ __forceinline__ void fft_pfa3(cx<T>* v) {
+    constexpr int N2 = R / 3;
+    static_assert(R == 6 || R == 12, "3 x 2 or 3 x 4");
+#pragma unroll
+    for (int n2 = 0; n2 < N2; ++n2) bf3<DIR, T>(v[(3 * n2) % R], v[(N2 + 3 * n2) % R], v[(2 * N2 + 3 * n2) % R]);
+#pragma unroll
+    for (int k1 = 0; k1 < 3; ++k1) {
+        if constexpr (N2 == 2) {
+            const cx<T> a = v[(N2 * k1) % R], b = v[(N2 * k1 + 3) % R];
+            v[(N2 * k1) % R] = a + b;
+            v[(N2 * k1 + 3) % R] = a - b;
+        } else {
+            cx<T>&r0 = v[(N2 * k1) % R], &r1 = v[(N2 * k1 + 3) % R], &r2 = v[(N2 * k1 + 6) % R], &r3 = v[(N2 * k1 + 9) % R];
+            const cx<T> x0 = r0, x1 = r1, x2 = r2, x3 = r3;
+            bf4_plain<DIR, T>(x0, x1, x2, x3, r0, r1, r2, r3);
+        }
+    }
+}
+
+// In-place FFT of v[0..R), R in {1,2,3,4,6,8,12,16}, kernel exp(DIR 2 pi i jk/R): decimation in frequency for the powers
+// of two, prime-factor for 6 and 12.  Output X[k] is left at v[outpos<R>(k)].
 template <int R, int DIR, typename T>
 __device__ __forceinline__ void fft_reg(cx<T>* v) {
     if constexpr (R == 16) {
         fft16_fma<DIR, T>(v);
+    } else if constexpr (R == 3) {
+        bf3<DIR, T>(v[0], v[1], v[2]);
+    } else if constexpr (R == 6 || R == 12) {
+        fft_pfa3<R, DIR, T>(v);
     } else if constexpr (R >= 2) {
         DifButterflies<R, DIR, 0, T>::run(v);
         fft_reg<R / 2, DIR, T>(v);
         fft_reg<R / 2, DIR, T>(v + R / 2);
     }
+}
+template <int R>
+__host__ __device__ __forceinline__ constexpr int outpos(int k) {
+    if constexpr (R == 3) return k;
+    else if constexpr (R == 6 || R == 12) return ((R / 3) * (k % 3) + 3 * (k % (R / 3))) % R;
+    else return brev<R>(k);
 }
 
 }  // namespace ns

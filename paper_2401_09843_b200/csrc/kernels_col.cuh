@@ -29,14 +29,30 @@ struct ColArgs {
     long in_slab, out_slab;   // slab strides, in complex elements
     int tiles_per_slab;       // column tiles per slab (columns / TC)
     long total_tiles;         // slabs * tiles_per_slab
+    int pf_dist;              // tiles ahead to prefetch into L2 (kernels instantiated with PF): about the CTAs resident on the GPU
 };
 
 template <int R1, int R2> struct ColP { static constexpr int value = R1 > R2 ? R1 : R2; };
 
+// L2 prefetch of the input rows of a LATER tile (the one this SM will work on a few CTAs from now), issued while the
+// current tile is in its butterflies: one tile per CTA and blocking loads leave HBM idle during the compute phases
+// (ncu: DRAM 59-70 % busy, stalls = global-load latency); the prefetch keeps requests in flight.  `rows` input rows of
+// 128 bytes; thread `tid` of `nthreads` takes every nthreads-th row.  Measured (profiles/r02_notes.md): it pays for the
+// short lines (L = 64: a5 1.68 -> 1.52 ms, a6 1.15 -> 1.01 ms at 32 x 128^3) and loses for L = 256, so PF is a template flag.
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+template <typename T>
+__device__ __forceinline__ void col_prefetch_tile(const cx<T>* __restrict__ in, const ColArgs& g, long tile, int rows, int TC, int tid,
+                                                  int nthreads) {
+    if (tile >= g.total_tiles) return;
+    const long slab = tile / g.tiles_per_slab;
+    const cx<T>* base = in + slab * g.in_slab + (long)(tile % g.tiles_per_slab) * TC;
+    for (int r = tid; r < rows; r += nthreads) prefetch_l2(base + (long)r * g.istride);
+}
+
 // ------------------------------------------------------------------------------------------------
 // inverse (spectral rows [0,2L) -> physical rows [0,3L)), exp(+i...)
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R1, int R2, int TC, int TPB>
+template <typename T, int L, int R1, int R2, int TC, int TPB, bool PF>
 __global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
 col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
                Twiddles<T> tw) {
@@ -71,6 +87,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
             cc[n1] = (n == 0) ? mk<T>(0, 0) : ldg(ip + (long)(L + n) * g.istride);
         }
     }
+    if constexpr (PF) col_prefetch_tile<T>(in, g, (long)blockIdx.x * TPB + g.pf_dist + tl, 2 * L, TC, lt, TT);
     int buf = 0;
 #pragma unroll 1
     for (int q = 0; q < 3; ++q) {
@@ -97,7 +114,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
             fft_reg<R1, +1, T>(s);
 #pragma unroll
             for (int r1 = 0; r1 < R1; ++r1) {
-                cx<T> v = s[brev<R1>(r1)];
+                cx<T> v = s[outpos<R1>(r1)];
                 if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
                 Et[buf * EBUF + (size_t)(r1 * R2 + i) * TC + c] = v;
             }
@@ -109,7 +126,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
             for (int n2 = 0; n2 < R2; ++n2) y[n2] = Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c];
             fft_reg<R2, +1, T>(y);
 #pragma unroll
-            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[brev<R2>(r2)];
+            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[outpos<R2>(r2)];
         }
         buf ^= 1;
     }
@@ -118,7 +135,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 // ------------------------------------------------------------------------------------------------
 // forward (physical rows [0,3L) -> spectral rows [0,2L), truncated), exp(-i...), output * scale
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R1, int R2, int TC, int TPB>
+template <typename T, int L, int R1, int R2, int TC, int TPB, bool PF>
 __global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
 col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale,
                Twiddles<T> tw) {
@@ -148,24 +165,25 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 #pragma unroll
         for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(i + R1 * r2) * g.istride);
     }
-    // PF: rows of the next sub-transform are fetched while this one goes through its second stage
+    if constexpr (PF) col_prefetch_tile<T>(in, g, (long)blockIdx.x * TPB + g.pf_dist + tl, 3 * L, TC, lt, TT);
+    // NEXTQ: rows of the next sub-transform are fetched while this one goes through its second stage
     // (more bytes in flight per SM; only where the registers allow it)
-    constexpr bool PF = R1 * R2 <= 64;
+    constexpr bool NEXTQ = R1 * R2 <= 64;
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
         if (i < R1) {
-            if (!PF && q > 0) {
+            if (!NEXTQ && q > 0) {
 #pragma unroll
                 for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(q * L + i + R1 * r2) * g.istride);
             }
             fft_reg<R2, -1, T>(x);
 #pragma unroll
             for (int n2 = 0; n2 < R2; ++n2) {
-                cx<T> v = x[brev<R2>(n2)];
+                cx<T> v = x[outpos<R2>(n2)];
                 if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
                 Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c] = v;
             }
-            if (PF && q < 2) {
+            if (NEXTQ && q < 2) {
 #pragma unroll
                 for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)((q + 1) * L + i + R1 * r2) * g.istride);
             }
@@ -178,18 +196,18 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
             fft_reg<R1, -1, T>(y);
             if (q == 0) {
 #pragma unroll
-                for (int n1 = 0; n1 < R1; ++n1) F0[n1] = y[brev<R1>(n1)];
+                for (int n1 = 0; n1 < R1; ++n1) F0[n1] = y[outpos<R1>(n1)];
             } else if (q == 1) {
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) {
                     const int n = R2 * n1 + i;
-                    G1[(size_t)n * TC + c] = cmulc(y[brev<R1>(n1)], ldg(tw.w3a + n));
+                    G1[(size_t)n * TC + c] = cmulc(y[outpos<R1>(n1)], ldg(tw.w3a + n));
                 }
             } else {
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) {
                     const int n = R2 * n1 + i;
-                    const cx<T> g2 = cmulc(y[brev<R1>(n1)], ldg(tw.w3b + n));
+                    const cx<T> g2 = cmulc(y[outpos<R1>(n1)], ldg(tw.w3b + n));
                     const cx<T> g1 = G1[(size_t)n * TC + c];
                     const cx<T> S = g1 + g2, D = g1 - g2;
                     constexpr T h3 = (T)0.86602540378443864676L;
@@ -212,7 +230,7 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 // thread and a third of the shared memory, which is what bounded the kernel at two CTAs (8 warps) per SM.
 // One tile per CTA; CTAs of 4 (fp64) or 8 (fp32) warps; warp w uses TMEM lanes 32 (w % 4), columns of set w / 4.
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R2, int TC, int MINB>
+template <typename T, int L, int R2, int TC, int MINB, bool PF>
 __global__ void __launch_bounds__(TC * 16, MINB)
 col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale, Twiddles<T> tw) {
     constexpr int R1 = 16;
@@ -244,13 +262,14 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
     cx<T> x[R2];
 #pragma unroll
     for (int r2 = 0; r2 < R2; ++r2) x[r2] = ldg(ip + (long)(i + R1 * r2) * g.istride);
+    if constexpr (PF) col_prefetch_tile<T>(in, g, tile + g.pf_dist, 3 * L, TC, threadIdx.x, TC * 16);
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
         {
             fft_reg<R2, -1, T>(x);
 #pragma unroll
             for (int n2 = 0; n2 < R2; ++n2) {
-                cx<T> v = x[brev<R2>(n2)];
+                cx<T> v = x[outpos<R2>(n2)];
                 if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
                 E[buf * EBUF + (size_t)(i * R2 + n2) * TC + c] = v;
             }
@@ -275,7 +294,7 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
 #pragma unroll
                 for (int k = 0; k < CH; ++k) {
                     const int n1 = ch * CH + k;
-                    cx<T> v = y[brev<R1>(n1)];
+                    cx<T> v = y[outpos<R1>(n1)];
                     if (q == 1) v = cmulc(v, ldg(tw.w3a + R2 * n1 + ii));
                     px[k] = v.x;
                     py[k] = v.y;
@@ -294,7 +313,7 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
                     for (int k = 0; k < CH; ++k) {
                         const int n1 = ch * CH + k;
                         const int n = R2 * n1 + i;
-                        const cx<T> g2 = cmulc(y[brev<R1>(n1)], ldg(tw.w3b + n));
+                        const cx<T> g2 = cmulc(y[outpos<R1>(n1)], ldg(tw.w3b + n));
                         const cx<T> f0 = mk<T>(fx[k], fy[k]), g1 = mk<T>(gx[k], gy[k]);
                         const cx<T> S = g1 + g2, D = g1 - g2;
                         constexpr T h3 = (T)0.86602540378443864676L;
@@ -320,7 +339,7 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
 // fits on the SM (the register-resident version needs 254 registers; ncu: 1.9 warps per scheduler, stalls
 // dominated by the global loads).  Thread layout and TMEM window as in col_fwd_tmem_kernel.
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R2, int TC, int MINB>
+template <typename T, int L, int R2, int TC, int MINB, bool PF>
 __global__ void __launch_bounds__(TC * 16, MINB)
 col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, Twiddles<T> tw) {
     constexpr int R1 = 16;
@@ -352,6 +371,7 @@ col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
         const int n = R2 * n1 + ii;
         cc[n1] = (n == 0) ? mk<T>(0, 0) : ldg(ip + (long)(L + n) * g.istride);
     }
+    if constexpr (PF) col_prefetch_tile<T>(in, g, tile + g.pf_dist, 2 * L, TC, threadIdx.x, TC * 16);
     if (warp == 0) tmem_alloc(&tslot, NCOLS);
     tmem_fence_before_sync();
     __syncthreads();
@@ -399,7 +419,7 @@ col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
             fft_reg<R1, +1, T>(s);
 #pragma unroll
             for (int r1 = 0; r1 < R1; ++r1) {
-                cx<T> v = s[brev<R1>(r1)];
+                cx<T> v = s[outpos<R1>(r1)];
                 if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
                 E[buf * EBUF + (size_t)(r1 * R2 + i) * TC + c] = v;
             }
@@ -411,7 +431,7 @@ col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
             for (int n2 = 0; n2 < R2; ++n2) y[n2] = E[buf * EBUF + (size_t)(i * R2 + n2) * TC + c];
             fft_reg<R2, +1, T>(y);
 #pragma unroll
-            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[brev<R2>(r2)];
+            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[outpos<R2>(r2)];
         }
         buf ^= 1;
     }

@@ -262,31 +262,24 @@ __global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __re
 }
 
 // ------------------------------------------------------------------------------------------------
-// unpadded N-grid transforms for ns_set_initial / ns_get_fields (NOT on the hot path): a plain
-// shared-memory radix-2 FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place.
+// unpadded N-grid transforms for ns_set_initial / ns_get_fields / the physical-space statistics (NOT on the hot path):
+// a shared-memory FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place, n = 2^a or 3 * 2^a.
 //   axis 0: element stride n*n, axis 1: n, axis 2: 1.
+// n = 3 m: the three decimated sequences x[3r + q] are transformed by radix-2 stages (m = 2^a) and combined by one
+// radix-3 stage, X[k + m t] = sum_q w_n^{q (k + m t)} F_q[k].  Twiddles come from the table gtw[j] = exp(+2 pi i j / n).
 // ------------------------------------------------------------------------------------------------
-template <typename T> __device__ __forceinline__ cx<T> unit_root_pi(T frac);  // exp(i*pi*frac)
-template <> __device__ __forceinline__ cx<double> unit_root_pi<double>(double f) {
-    double s, c;
-    sincospi(f, &s, &c);
-    return mk<double>(c, s);
-}
-template <> __device__ __forceinline__ cx<float> unit_root_pi<float>(float f) {
-    float s, c;
-    sincospif(f, &s, &c);
-    return mk<float>(c, s);
-}
-
 template <typename T>
 __global__ void __launch_bounds__(256)
-generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2n, int axis, int sign, long total_tiles) {
+generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis, int sign, long total_tiles,
+                   const cx<T>* __restrict__ gtw) {
     constexpr int TL = 8;  // lines per tile
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);  // [n][TL+1]
     constexpr int PITCH = TL + 1;
     const long tile = blockIdx.x;
     if (tile >= total_tiles) return;
+    const int m = 1 << log2m;          // n = m or 3 m
+    const int nsub = radix3 ? 3 : 1;
     const long n2 = (long)n * n;
     const long tiles_per_cube = n2 / TL;
     const long cube = tile / tiles_per_cube;
@@ -299,25 +292,45 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2n, int axis, int sign, 
         if (axis == 1) return (l / n) * n2 + (l % n);
         return l * n;
     };
-    // load with bit-reversed row index
+    auto root = [&](int j) -> cx<T> {   // exp(sign 2 pi i j / n), 0 <= j < n
+        const cx<T> w = ldg(gtw + j);
+        return sign > 0 ? w : conj(w);
+    };
+    // load: element j = nsub r + q goes to q m + bitrev_m(r)
     for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
         int j, c;
         if (axis == 2) { j = e % n; c = e / n; } else { c = e % TL; j = e / TL; }
-        const int jr = (int)(__brev((unsigned)j) >> (32 - log2n));
-        S[jr * PITCH + c] = base[line_base(l0 + c) + (long)j * es];
+        const int q = j % nsub, r = j / nsub;
+        const int rr = log2m == 0 ? 0 : (int)(__brev((unsigned)r) >> (32 - log2m));
+        S[(q * m + rr) * PITCH + c] = base[line_base(l0 + c) + (long)j * es];
     }
     __syncthreads();
-    for (int s = 1; s <= log2n; ++s) {
+    for (int s = 1; s <= log2m; ++s) {
         const int half = 1 << (s - 1);
         for (int e = threadIdx.x; e < (n / 2) * TL; e += blockDim.x) {
             const int c = e % TL, bf = e / TL;
             const int j = bf & (half - 1);
             const int i0 = ((bf >> (s - 1)) << s) + j;
-            const cx<T> w = unit_root_pi<T>((T)sign * (T)j / (T)half);
+            const cx<T> w = root(j * (n >> s));          // w_{2^s}^j
             const cx<T> a = S[i0 * PITCH + c];
             const cx<T> bq = cmul(S[(i0 + half) * PITCH + c], w);
             S[i0 * PITCH + c] = a + bq;
             S[(i0 + half) * PITCH + c] = a - bq;
+        }
+        __syncthreads();
+    }
+    if (radix3) {
+        const T h = (T)sign * (T)0.86602540378443864676L;
+        for (int e = threadIdx.x; e < m * TL; e += blockDim.x) {
+            const int c = e % TL, k = e / TL;
+            const cx<T> f0 = S[k * PITCH + c];
+            const cx<T> f1 = cmul(S[(m + k) * PITCH + c], root(k));
+            const cx<T> f2 = cmul(S[(2 * m + k) * PITCH + c], root(2 * k));
+            const cx<T> sm = f1 + f2, d = f1 - f2;
+            const cx<T> mm = mk<T>(f0.x - (T)0.5 * sm.x, f0.y - (T)0.5 * sm.y);
+            S[k * PITCH + c] = f0 + sm;
+            S[(m + k) * PITCH + c] = mk<T>(mm.x - h * d.y, mm.y + h * d.x);
+            S[(2 * m + k) * PITCH + c] = mk<T>(mm.x + h * d.y, mm.y - h * d.x);
         }
         __syncthreads();
     }

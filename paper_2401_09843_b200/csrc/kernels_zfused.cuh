@@ -120,7 +120,7 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
             fft_reg<R1, +1, T>(s);
 #pragma unroll
             for (int r1 = 0; r1 < R1; ++r1) {
-                cx<T> v = s[brev<R1>(r1)];
+                cx<T> v = s[outpos<R1>(r1)];
                 if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
                 Eq[r1 * PITCH + i] = v;
             }
@@ -154,7 +154,7 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
             fft_reg<R1, +1, T>(s);
 #pragma unroll
             for (int r1 = 0; r1 < R1; ++r1) {
-                cx<T> v = s[brev<R1>(r1)];
+                cx<T> v = s[outpos<R1>(r1)];
                 if (r1 > 0) v = cmul(v, ldg(tw.twA + r1 * R2 + i));
                 Eq[r1 * PITCH + i] = v;
             }
@@ -186,15 +186,15 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
                 cx<T> x[R2];
 #pragma unroll
                 for (int r2 = 0; r2 < R2; ++r2) {
-                    const cx<T> w = u12[brev<R2>(r2)];
-                    const T w3 = u3r[brev<R2>(r2)];
+                    const cx<T> w = u12[outpos<R2>(r2)];
+                    const T w3 = u3r[outpos<R2>(r2)];
                     x[r2] = pair == 0 ? mk<T>(w.x * w.x - w3 * w3, w.y * w.y - w3 * w3) : (pair == 1 ? mk<T>(w.x * w.y, w.x * w3) : mk<T>(w.y * w3, 0));
                 }
                 fft_reg<R2, -1, T>(x);
                 // pair 0: this thread overwrites the row only it has read in stage B above; later pairs: barrier above
 #pragma unroll
                 for (int n2 = 0; n2 < R2; ++n2) {
-                    cx<T> v = x[brev<R2>(n2)];
+                    cx<T> v = x[outpos<R2>(n2)];
                     if (n2 > 0) v = cmulc(v, ldg(tw.twB + n2 * R1 + i));
                     Eq[i * PITCH + n2] = v;
                 }
@@ -208,7 +208,7 @@ z_fused_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, long MM, l
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) {
                     const int n = R2 * n1 + i;
-                    cx<T> v = y[brev<R1>(n1)];
+                    cx<T> v = y[outpos<R1>(n1)];
                     if (q > 0) v = cmulc(v, ldg((q == 1 ? tw.w3a : tw.w3b) + n));
                     Cq[n1 * PITCH + i] = v;  // when aliased: overwrites exactly the column this thread has just read
                 }

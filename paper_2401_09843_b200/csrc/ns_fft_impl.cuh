@@ -19,6 +19,11 @@ template <> struct Split<32>  { static constexpr int R1 = 8,  R2 = 4;  };
 template <> struct Split<64>  { static constexpr int R1 = 8,  R2 = 8;  };
 template <> struct Split<128> { static constexpr int R1 = 16, R2 = 8;  };
 template <> struct Split<256> { static constexpr int R1 = 16, R2 = 16; };
+// N = 3 * 2^a (sizes with small prime factors): L = 3 * 2^(a-1), first stage 6 or 12
+template <> struct Split<24>  { static constexpr int R1 = 6,  R2 = 4;  };
+template <> struct Split<48>  { static constexpr int R1 = 12, R2 = 4;  };
+template <> struct Split<96>  { static constexpr int R1 = 12, R2 = 8;  };
+template <> struct Split<192> { static constexpr int R1 = 12, R2 = 16; };
 
 template <int L> struct Cfg {
     static constexpr int R1 = Split<L>::R1, R2 = Split<L>::R2;
@@ -28,10 +33,10 @@ template <int L> struct Cfg {
         constexpr int tt = tile_cols<T>() * P;
         return tt >= 128 ? 1 : 128 / tt;
     }
-    // lines per block for the fused z kernel: ~96 threads for the long lines (shared memory bound), 192 otherwise
-    static constexpr int lpbf() { return L >= 128 ? 2 : 192 / (3 * P); }
+    // lines per block of the block-synchronous fused z kernel (must divide M^2): about 96-192 threads
+    static constexpr int lpbf() { return L == 24 ? 8 : (L % 3 == 0 ? (L >= 192 ? 2 : 4) : 192 / (3 * P)); }
     // target CTAs per SM of the fused z kernel (bounds its registers)
-    static constexpr int minbf() { return L >= 128 ? 4 : 2; }
+    static constexpr int minbf() { return 2; }
 };
 
 template <typename K>
@@ -40,11 +45,11 @@ static cudaError_t set_smem(K kernel, size_t bytes) {
     return cudaSuccess;
 }
 
-template <typename T, int L>
+template <typename T, int L, bool PF>
 static cudaError_t col_inv_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, Twiddles<T> tw) {
     using C = Cfg<L>;
     constexpr int TC = tile_cols<T>(), TPB = C::template tpb<T>();
-    auto k = col_inv_kernel<T, L, C::R1, C::R2, TC, TPB>;
+    auto k = col_inv_kernel<T, L, C::R1, C::R2, TC, TPB, PF>;
     const size_t smem = (size_t)2 * TPB * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -53,11 +58,11 @@ static cudaError_t col_inv_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     return cudaGetLastError();
 }
 
-template <typename T, int L>
+template <typename T, int L, bool PF>
 static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
     using C = Cfg<L>;
     constexpr int TC = tile_cols<T>(), TPB = C::template tpb<T>();
-    auto k = col_fwd_kernel<T, L, C::R1, C::R2, TC, TPB>;
+    auto k = col_fwd_kernel<T, L, C::R1, C::R2, TC, TPB, PF>;
     const size_t smem = (size_t)3 * TPB * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -67,11 +72,11 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
 }
 
 // long lines (L = 128, 256): inverse pass with its inputs parked in tensor memory
-template <typename T, int L>
+template <typename T, int L, bool PF>
 static cudaError_t col_inv_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, Twiddles<T> tw) {
     constexpr int TC = tile_cols<T>(), R2 = L / 16;
     constexpr int MINB = sizeof(T) == 8 ? 3 : 2;
-    auto k = col_inv_tmem_kernel<T, L, R2, TC, MINB>;
+    auto k = col_inv_tmem_kernel<T, L, R2, TC, MINB, PF>;
     const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -80,11 +85,11 @@ static cudaError_t col_inv_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, 
 }
 
 // long lines (L = 128, 256): forward pass with F_0 / G_1 parked in tensor memory
-template <typename T, int L>
+template <typename T, int L, bool PF>
 static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
     constexpr int TC = tile_cols<T>(), R2 = L / 16;
     constexpr int MINB = sizeof(T) == 8 ? 3 : 2;
-    auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB>;
+    auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB, PF>;
     const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -163,6 +168,10 @@ static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>
 
 #define NS_DISPATCH_L(L, CALL)                                   \
     switch (L) {                                                 \
+        case 24: return CALL(24);                                \
+        case 48: return CALL(48);                                \
+        case 96: return CALL(96);                                \
+        case 192: return CALL(192);                              \
         case 8: return CALL(8);                                  \
         case 16: return CALL(16);                                \
         case 32: return CALL(32);                                \
@@ -172,8 +181,25 @@ static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>
         default: return cudaErrorInvalidValue;                   \
     }
 
+// L2 prefetch distance of the column passes in tiles (kernels_col.cuh): the CTAs resident on the GPU (2-3 per SM)
+static int col_pf_dist(int num_sms, int L) {
+#ifdef NS_DEV_SWITCHES
+    if (const char* v = getenv("NS_COLPF")) return atoi(v) * num_sms;
+#endif
+    return (L <= 64 ? 2 : 1) * num_sms;
+}
+// which passes prefetch: measured per length (profiles/r02_notes.md): it pays up to L = 128; at L = 256 only for the inverse
+// pass along y (a2 2.13 -> 1.93 ms at 512^3) -- along x every row of a tile lies in another 2 MB page and the extra requests lose
+static bool col_pf_on(bool fwd, int L, long row_stride_bytes) {
+#ifdef NS_DEV_SWITCHES
+    if (const char* v = getenv(fwd ? "NS_COLPF_FWD" : "NS_COLPF_INV")) return atoi(v) != 0;
+#endif
+    if (L <= 128) return true;
+    return !fwd && L == 256 && row_stride_bytes < (1L << 16);
+}
+
 template <typename T>
-static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab) {
+static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab, int pf_dist) {
     ColArgs g;
     g.istride = istride;
     g.ostride = ostride;
@@ -181,29 +207,32 @@ static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride
     g.out_slab = out_slab;
     g.tiles_per_slab = (int)(ncols / tile_cols<T>());
     g.total_tiles = (long)g.tiles_per_slab * nslabs;
+    g.pf_dist = pf_dist;
     return g;
 }
 
 template <typename T>
-cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+cudaError_t launch_col_inv(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
-    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
+    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
     // measured (profiles/): parking pays at L = 128 (0.264 -> 0.216 ms at 256^3); at L = 256 the register kernel is faster
-    if (L == 128) return col_inv_tmem_L<T, 128>(st, in, out, g, tw);
-#define CALL(LL) col_inv_L<T, LL>(st, in, out, g, tw)
+    const bool pf = col_pf_on(false, L, istride * (long)sizeof(cx<T>));
+    if (L == 128) return pf ? col_inv_tmem_L<T, 128, true>(st, in, out, g, tw) : col_inv_tmem_L<T, 128, false>(st, in, out, g, tw);
+#define CALL(LL) (pf ? col_inv_L<T, LL, true>(st, in, out, g, tw) : col_inv_L<T, LL, false>(st, in, out, g, tw))
     NS_DISPATCH_L(L, CALL)
 #undef CALL
 }
 
 template <typename T>
-cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+cudaError_t launch_col_fwd(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
-    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab);
-    if (L == 128) return col_fwd_tmem_L<T, 128>(st, in, out, g, scale, tw);
-    if (L == 256) return col_fwd_tmem_L<T, 256>(st, in, out, g, scale, tw);
-#define CALL(LL) col_fwd_L<T, LL>(st, in, out, g, scale, tw)
+    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
+    const bool pf = col_pf_on(true, L, istride * (long)sizeof(cx<T>));
+    if (L == 128) return pf ? col_fwd_tmem_L<T, 128, true>(st, in, out, g, scale, tw) : col_fwd_tmem_L<T, 128, false>(st, in, out, g, scale, tw);
+    if (L == 256) return pf ? col_fwd_tmem_L<T, 256, true>(st, in, out, g, scale, tw) : col_fwd_tmem_L<T, 256, false>(st, in, out, g, scale, tw);
+#define CALL(LL) (pf ? col_fwd_L<T, LL, true>(st, in, out, g, scale, tw) : col_fwd_L<T, LL, false>(st, in, out, g, scale, tw))
     NS_DISPATCH_L(L, CALL)
 #undef CALL
 }
@@ -224,14 +253,19 @@ cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in,
         case 8: return z_fused_L<T, 8>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 16: return z_fused_L<T, 16>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 32: return z_fused_L<T, 32>(st, num_sms, in, out, MM, batch, umax2, tw);
+        // N = 3 * 2^a: the same kernel with a radix-6 / radix-12 first stage
+        case 24: return z_fused_L<T, 24>(st, num_sms, in, out, MM, batch, umax2, tw);
+        case 48: return z_fused_L<T, 48>(st, num_sms, in, out, MM, batch, umax2, tw);
+        case 96: return z_fused_L<T, 96>(st, num_sms, in, out, MM, batch, umax2, tw);
+        case 192: return z_fused_L<T, 192>(st, num_sms, in, out, MM, batch, umax2, tw);
         default: return cudaErrorInvalidValue;
     }
 }
 
 #define NS_INSTANTIATE_FFT(T)                                                                                      \
-    template cudaError_t launch_col_inv<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
+    template cudaError_t launch_col_inv<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, Twiddles<T>);                                                     \
-    template cudaError_t launch_col_fwd<T>(cudaStream_t, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
+    template cudaError_t launch_col_fwd<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, T, Twiddles<T>);                                                  \
     template cudaError_t launch_z_fused<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*, \
                                            Twiddles<T>);

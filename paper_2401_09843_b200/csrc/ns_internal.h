@@ -27,10 +27,12 @@ struct Twiddles {
     // table of the 16-values-per-lane z kernel (kernels_zpair.cuh), G = L/16 (L >= 64 only):
     //   z16[r1*G + t] = w_L^{r1 t},  r1 < 16, t < G
     const cx<T>* z16;
+    // gN[j] = exp(+2 pi i j / N), j < N = 2L: the unpadded N-grid transforms (generic_fft_kernel)
+    const cx<T>* gN;
 };
 // number of complex entries of the table block and its host-side construction (long double arguments);
 // make_twiddles() returns the views into a device copy of that block
-inline size_t twiddle_table_len(int L) { return (size_t)8 * L; }
+inline size_t twiddle_table_len(int L) { return (size_t)10 * L; }
 // register-stage split L = R1 x R2 used by the kernels (needed by the host to build twA / twB)
 void fft_split(int L, int* R1, int* R2);
 
@@ -43,10 +45,10 @@ template <typename T> constexpr int tile_cols() { return 128 / (2 * (int)sizeof(
 // Strided-axis passes.  `ncols` contiguous columns per slab (multiple of tile_cols<T>()), `nslabs` slabs.
 // Input rows [0,2L) -> output rows [0,3L) (inverse) or the reverse (forward, output multiplied by scale).
 template <typename T>
-cudaError_t launch_col_inv(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+cudaError_t launch_col_inv(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw);
 template <typename T>
-cudaError_t launch_col_fwd(cudaStream_t st, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+cudaError_t launch_col_fwd(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw);
 // fused a3+a4 (kernels_zpair.cuh; kernels_zfused.cuh for L <= 32): in [batch][3][MM][L] -> out [batch][NS_NFLUX][MM][L];
 // persistent grid sized from num_sms (the SM count of the solver's device) and the CTAs per SM.  umax2 may be NULL.

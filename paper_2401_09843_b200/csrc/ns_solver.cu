@@ -242,11 +242,11 @@ public:
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
         prof.tick(0, st);
-        e = launch_col_inv<T>(st, L, Uin, X, NH, (long)batch * 3, NH, NH, (long)N * NH, (long)M * NH, tw());
+        e = launch_col_inv<T>(st, num_sms, L, Uin, X, NH, (long)batch * 3, NH, NH, (long)N * NH, (long)M * NH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a1 col_inv x");
         ++launches;
         prof.tick(1, st);
-        e = launch_col_inv<T>(st, L, X, Y, H, (long)batch * 3 * M, H, H, NH, MH, tw());
+        e = launch_col_inv<T>(st, num_sms, L, X, Y, H, (long)batch * 3 * M, H, H, NH, MH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
         ++launches;
         prof.tick(2, st);
@@ -255,11 +255,11 @@ public:
         ++launches;
         if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
         prof.tick(4, st);
-        e = launch_col_fwd<T>(st, L, Z, X, H, (long)batch * NS_NFLUX * M, H, H, MH, NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, num_sms, L, Z, X, H, (long)batch * NS_NFLUX * M, H, H, MH, NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a5 col_fwd y");
         ++launches;
         prof.tick(5, st);
-        e = launch_col_fwd<T>(st, L, X, Y, NH, (long)batch * NS_NFLUX, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, num_sms, L, X, Y, NH, (long)batch * NS_NFLUX, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a6 col_fwd x");
         ++launches;
         prof.tick(7, st);
@@ -410,14 +410,16 @@ public:
     }
 
     int generic_fft3(cx<T>* W, long cubes, int sign) {
-        int log2n = 0;
-        while ((1 << log2n) < N) ++log2n;
+        const int radix3 = N % 3 == 0 ? 1 : 0;
+        const int m = radix3 ? N / 3 : N;
+        int log2m = 0;
+        while ((1 << log2m) < m) ++log2m;
         const long tiles = cubes * (long)N * N / 8;
         const size_t smem = (size_t)N * 9 * sizeof(cx<T>);
         if (smem > 48 * 1024)
             NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         for (int axis = 0; axis < 3; ++axis) {
-            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2n, axis, sign, tiles);
+            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2m, radix3, axis, sign, tiles, tw().gN);
             NS_LAUNCHED("generic_fft");
         }
         return NS_OK;
@@ -595,9 +597,11 @@ int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dt
     g_create_error.clear();
     if (!out) { g_create_error = "out is NULL"; return NS_ERR_INVALID_ARG; }
     *out = nullptr;
-    const int min_n = dtype == NS_F32 ? 32 : 16;
-    if (N < min_n || N > 512 || (N & (N - 1)) != 0 || !fft_supported(N / 2)) {
-        g_create_error = "N must be a power of two in [16, 512] (fp32: [32, 512])";
+    // N = 2^a or 3 * 2^a (sizes with small prime factors); a column tile is 128 bytes = 8 (fp64) / 16 (fp32)
+    // complex values of the N/2 stored kz entries
+    const int tile = dtype == NS_F32 ? 16 : 8;
+    if (N < 16 || N > 512 || (N % 2) != 0 || !fft_supported(N / 2) || (N / 2) % tile != 0) {
+        g_create_error = "N must be 2^a or 3 * 2^a with 16 <= N <= 512 (fp32: N/2 a multiple of 16, i.e. N >= 32 and N != 48)";
         return NS_ERR_INVALID_ARG;
     }
     if (batch < 1) { g_create_error = "batch must be >= 1"; return NS_ERR_INVALID_ARG; }

@@ -182,3 +182,81 @@ def test_full_size_stratified_sampled_rhs(ns, oracle, k53_512, N):
     dts = s.step_cfl(0.2, 1e9)
     assert abs(dts[0] - dt) < 1e-13 * dt
     assert rel(s.get_spectral()[0], un) < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-3: N = 3 * 2^a
+@pytest.mark.parametrize("N", [48, 96])
+def test_sizes_3x2a_rhs_and_20_steps(ns, oracle, N):
+    """SURVEY.md 8(f) NEXT-3, first slice (transform sizes with small prime factors): N = 3 * 2^a, i.e.
+    sub-transforms of length L = N/2 = 3 * 2^(a-1) with a radix-6 / radix-12 first register stage.  set_initial,
+    get_fields, one RHS and 20 CFL steps (the oracle replaying the GPU's dt) at 48^3 and 96^3, every stored entry."""
+    u = inputs.gaussian_field(N, 300 + N, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    u += 0.2 * inputs.normal01(N, 3, 3 * N ** 3).reshape(3, N, N, N)          # not solenoidal: exercises the projection
+    kw = dict(nu=0.002, eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    assert rel(s.get_fields()[0], oracle.get_fields(N, uh)) < 1e-13
+    s.set_spectral(uh[None])
+    p = oracle.Params(**kw)
+    want = oracle.rhs_parts(N, p, uh)
+    got = s.rhs()[0]
+    assert rel(got, want["r"]) < TOL_RHS_F64
+    assert np.all(got[:, N // 2] == 0) and np.all(got[:, :, N // 2] == 0) and np.all(got[:, :, :, N // 2] == 0)
+    assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
+    worst = 0.0
+    for i in range(20):
+        dts = s.step_cfl(0.2, 1e9)
+        uh = oracle.step(N, p, uh, dts[0])
+        worst = max(worst, rel(s.get_spectral()[0], uh))
+        assert worst < TOL_STEPS_F64, (i, worst)
+    E = s.energy_spectrum(N)[0]
+    assert np.abs(E - oracle.energy_spectrum(N, uh, N)).max() < 1e-13
+    assert np.abs(s.structure_function_p(3.0, nl=6)[0] / oracle.structure_function_p(N, uh, 3.0, 6) - 1).max() < 1e-11
+    print(f"N = {N}: worst rel-L2 over 20 steps {worst:.2e}")
+
+
+def test_sizes_3x2a_192_full_and_384_sampled(ns, oracle):
+    """N = 192 (L = 96 = 12 x 8): every stored entry of ns_rhs against orc_rhs_parts, two samples in one launch;
+    N = 384 (L = 192 = 12 x 16, padded 576^3): 524 stratified sampled wavenumbers against the direct truncated
+    convolution, the energy identity on the whole array, and fp32 against the fp64 result."""
+    N = 192
+    us = np.stack([inputs.taylor_green_3d_perturbed(N, 31), inputs.gaussian_field(N, 392, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)])
+    kw = dict(eps=0.05, s=1.5)
+    s = ns.Solver(N, batch=2, **kw)
+    s.set_initial(us)
+    del us
+    uh = s.get_spectral()
+    r = s.rhs()
+    um = s.max_velocity()
+    for b in range(2):
+        want = oracle.rhs_parts(N, oracle.Params(**kw), uh[b])
+        assert rel(r[b], want["r"]) < TOL_RHS_F64
+        assert abs(um[b] - want["umax"]) < 1e-13 * want["umax"]
+    del s, r, uh
+    N = 384
+    u = inputs.gaussian_field(N, 384, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    kw = dict(eps=0.05, s=1.0)
+    s = ns.Solver(N, **kw)
+    s.set_initial(u[None])
+    del u
+    uh = s.get_spectral()[0]
+    r = s.rhs()[0]
+    del s
+    rmax = np.abs(r).max()
+    modes = stratified_modes(N, 512, N)
+    want = oracle.rhs_at_modes(N, oracle.Params(**kw), uh, modes)
+    got = np.stack([r[:, ix, iy, iz] for ix, iy, iz in modes])
+    print(f"N = 384: rel-L2 over {len(modes)} sampled modes {rel(got, want):.2e}")
+    assert rel(got, want) < TOL_RHS_F64 and np.abs(got - want).max() < 1e-12 * rmax
+    w = np.full(N // 2 + 1, 2.0)
+    w[0] = 1.0
+    s = ns.Solver(N)
+    s.set_spectral(uh[None])
+    rn = s.rhs()[0]
+    assert abs(np.sum(w * np.real(np.conj(uh) * rn))) < 1e-12 * np.sum(w * np.abs(uh) * np.abs(rn))
+    del s, rn
+    s32 = ns.Solver(N, dtype="f32", **kw)
+    s32.set_spectral(uh[None].astype(np.complex64))
+    assert rel(s32.rhs()[0], r) < 1e-5
