@@ -207,3 +207,52 @@ def cylindrical_shear(N: int, seed: int, rho: float = 0.05, delta: float = 0.025
 
 def checksum(a: np.ndarray) -> str:
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()[:16]
+
+
+# ------------------------------------------------------------------------------------------------ two-dimensional inputs
+# (the paper validates its 2-D solver on the Taylor-Green vortex and the vortex patch)
+def grid2(N: int):
+    x = 2.0 * np.pi * np.arange(N) / N
+    return np.meshgrid(x, x, indexing="ij")
+
+
+def taylor_green_2d_plane(N: int) -> np.ndarray:
+    """2-D Taylor-Green vortex u = (sin x cos y, -cos x sin y) on [0,2pi)^2: u[2][N][N]."""
+    X, Y = grid2(N)
+    return np.stack([np.sin(X) * np.cos(Y), -np.cos(X) * np.sin(Y)])
+
+
+def gaussian_field_2d(N: int, seed: int, spectrum, e_tot: float = 0.5) -> np.ndarray:
+    """Band-limited Gaussian random solenoidal 2-D field with ring spectrum E(|k|) ~ spectrum(|k|): the curl of a white-noise
+    stream function shaped by sqrt(E)/|k|^(3/2) (so |u_hat| ~ sqrt(E/|k|), ring energy ~ E); rescaled to 1/2 <|u|^2> = e_tot."""
+    k = np.fft.fftfreq(N, 1.0 / N)
+    KX, KY = np.meshgrid(k, np.fft.rfftfreq(N, 1.0 / N), indexing="ij")
+    kabs = np.sqrt(KX * KX + KY * KY)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        shape = np.where(kabs > 0, np.sqrt(np.maximum(spectrum(kabs), 0.0)) / kabs ** 1.5, 0.0)
+    shape[(np.abs(KX) == N // 2) | (np.abs(KY) == N // 2)] = 0.0
+    psi = np.fft.rfft2(normal01(seed, 0, N * N).reshape(N, N)) * shape
+    u = np.stack([np.fft.irfft2(1j * KY * psi, s=(N, N)), np.fft.irfft2(-1j * KX * psi, s=(N, N))])
+    return u * np.sqrt(e_tot / (0.5 * float(np.mean(np.sum(u * u, axis=0)))))
+
+
+def vortex_patch(N: int, seed: int = 0, radius: float = 1.0, delta: float = 0.0) -> np.ndarray:
+    """Vortex patch ([19]): vorticity 1 inside a disc of the given radius centred at (pi, pi) (optionally
+    displaced by a seeded offset of size delta), minus its mean so that it is the curl of a periodic velocity; the velocity
+    is obtained from the stream function -Laplace psi = omega with numpy.fft.  u[2][N][N]."""
+    X, Y = grid2(N)
+    off = (2.0 * uniform01(seed, 300, 2) - 1.0) * delta
+    om = ((X - np.pi - off[0]) ** 2 + (Y - np.pi - off[1]) ** 2 <= radius ** 2).astype(np.float64)
+    om -= om.mean()
+    k = np.fft.fftfreq(N, 1.0 / N)
+    KX, KY = np.meshgrid(k, np.fft.rfftfreq(N, 1.0 / N), indexing="ij")
+    k2 = KX * KX + KY * KY
+    k2[0, 0] = 1.0
+    psi = np.fft.rfft2(om) / k2
+    psi[0, 0] = 0.0
+    return np.stack([np.fft.irfft2(1j * KY * psi, s=(N, N)), np.fft.irfft2(-1j * KX * psi, s=(N, N))])
+
+
+def shear_layer_2d(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmodes: int = 10) -> np.ndarray:
+    """The doubly periodic perturbed shear layer of configs 3/4 as a genuinely two-dimensional field: u[2][N][N]."""
+    return shear_layer(N, seed, rho, delta, nmodes)[:2, :, :, 0].copy()

@@ -23,3 +23,9 @@ def k53_512():
     """BASELINE.json configs[4] input (512^3 Gaussian k^-5/3 field, seed 5): 40 s of numpy FFTs, shared by the full-size tests."""
     from paper_2401_09843_b200 import inputs
     return inputs.gaussian_k53(512, seed=5)
+
+
+@pytest.fixture(scope="session")
+def oracle2d():
+    from oracle import ns2d_oracle
+    return ns2d_oracle
