@@ -24,6 +24,12 @@ EXPORTS = [
     "ns_step_cfl", "ns_step_dts", "ns_advance", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
     "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
+# include/ns2d.h: the two-dimensional solver
+EXPORTS_2D = [
+    "ns2d_create", "ns2d_destroy", "ns2d_set_initial", "ns2d_set_spectral", "ns2d_get_spectral", "ns2d_rhs", "ns2d_step", "ns2d_step_cfl",
+    "ns2d_step_dts", "ns2d_advance", "ns2d_max_velocity", "ns2d_get_fields", "ns2d_energy_spectrum", "ns2d_enstrophy_spectrum", "ns2d_time",
+    "ns2d_profile", "ns2d_profile_read", "ns2d_kernel_launches", "ns2d_device_bytes", "ns2d_last_error",
+]
 
 
 class ns_params(ctypes.Structure):
@@ -76,6 +82,28 @@ def lib():
         L.ns_device_bytes.restype = ctypes.c_longlong
         L.ns_last_error.argtypes = [vp]
         L.ns_last_error.restype = ctypes.c_char_p
+        # include/ns2d.h
+        L.ns2d_create.argtypes = [ctypes.POINTER(vp), i, i, ctypes.POINTER(ns_params), i, vp]
+        L.ns2d_destroy.argtypes = [vp]
+        for name in ("ns2d_set_initial", "ns2d_set_spectral", "ns2d_get_spectral", "ns2d_rhs", "ns2d_get_fields"):
+            getattr(L, name).argtypes = [vp, vp, i]
+        L.ns2d_step.argtypes = [vp, d]
+        L.ns2d_step_cfl.argtypes = [vp, d, d, vp]
+        L.ns2d_step_dts.argtypes = [vp, vp]
+        L.ns2d_advance.argtypes = [vp, d, d, i, ctypes.POINTER(ctypes.c_int)]
+        L.ns2d_max_velocity.argtypes = [vp, vp]
+        L.ns2d_energy_spectrum.argtypes = [vp, vp, i]
+        L.ns2d_enstrophy_spectrum.argtypes = [vp, vp, i]
+        L.ns2d_time.argtypes = [vp, i]
+        L.ns2d_time.restype = d
+        L.ns2d_profile.argtypes = [vp, i]
+        L.ns2d_profile_read.argtypes = [vp, vp, vp]
+        L.ns2d_kernel_launches.argtypes = [vp]
+        L.ns2d_kernel_launches.restype = ctypes.c_longlong
+        L.ns2d_device_bytes.argtypes = [vp]
+        L.ns2d_device_bytes.restype = ctypes.c_longlong
+        L.ns2d_last_error.argtypes = [vp]
+        L.ns2d_last_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -265,3 +293,135 @@ class Solver:
 
     def device_bytes(self):
         return int(lib().ns_device_bytes(self._h))
+
+
+class Solver2D:
+    """Owner of one ns2d_solver handle (include/ns2d.h).  Method names follow the C entry points without the ns2d_ prefix."""
+
+    PASS_NAMES = ["b1_x_inv", "b2_y_fused", "b3_x_fwd", "b4_spectral"]
+
+    def __init__(self, N, batch=1, nu=0.0, eps=0.0, s=1.0, m_cut=-1.0, q_exp=-1.0, q_sharp=0, dtype="f64", stream=None):
+        self.N, self.batch = int(N), int(batch)
+        self.dtype = {"f64": NS_F64, "f32": NS_F32, NS_F64: NS_F64, NS_F32: NS_F32}[dtype]
+        self.real = np.float64 if self.dtype == NS_F64 else np.float32
+        self.cplx = np.complex128 if self.dtype == NS_F64 else np.complex64
+        self._h = ctypes.c_void_p()
+        p = ns_params(nu, eps, s, m_cut, q_exp, q_sharp)
+        if stream is None:
+            import torch  # device memory and streams only
+            stream = torch.cuda.current_stream().cuda_stream
+        rc = lib().ns2d_create(ctypes.byref(self._h), self.N, self.batch, ctypes.byref(p), self.dtype, ctypes.c_void_p(stream))
+        if rc != NS_OK:
+            raise NSError(rc, lib().ns2d_last_error(None).decode())
+
+    @property
+    def spectral_shape(self):
+        return (self.batch, 2, self.N, self.N // 2 + 1)
+
+    @property
+    def physical_shape(self):
+        return (self.batch, 2, self.N, self.N)
+
+    def _check(self, rc):
+        if rc != NS_OK:
+            raise NSError(rc, lib().ns2d_last_error(self._h).decode())
+
+    _typed = Solver._typed
+
+    def close(self):
+        if self._h:
+            lib().ns2d_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_initial(self, u_phys):
+        u = self._typed(u_phys, "real")
+        assert tuple(u.shape) == self.physical_shape, (tuple(u.shape), self.physical_shape)
+        p, ms, _k = _buf(u)
+        self._check(lib().ns2d_set_initial(self._h, p, ms))
+
+    def set_spectral(self, u_hat):
+        u = self._typed(u_hat, "cplx")
+        assert tuple(u.shape) == self.spectral_shape
+        p, ms, _k = _buf(u)
+        self._check(lib().ns2d_set_spectral(self._h, p, ms))
+
+    def get_spectral(self, out=None):
+        if out is None:
+            out = np.empty(self.spectral_shape, dtype=self.cplx)
+        p, ms, _k = _buf(out, writable=True)
+        self._check(lib().ns2d_get_spectral(self._h, p, ms))
+        return out
+
+    def rhs(self, out=None):
+        if out is None:
+            out = np.empty(self.spectral_shape, dtype=self.cplx)
+        p, ms, _k = _buf(out, writable=True)
+        self._check(lib().ns2d_rhs(self._h, p, ms))
+        return out
+
+    def get_fields(self, out=None):
+        if out is None:
+            out = np.empty(self.physical_shape, dtype=self.real)
+        p, ms, _k = _buf(out, writable=True)
+        self._check(lib().ns2d_get_fields(self._h, p, ms))
+        return out
+
+    def step(self, dt):
+        self._check(lib().ns2d_step(self._h, float(dt)))
+
+    def step_cfl(self, cfl, t_end, return_dt=True):
+        if return_dt:
+            dts = np.empty(self.batch, dtype=np.float64)
+            self._check(lib().ns2d_step_cfl(self._h, float(cfl), float(t_end), ctypes.c_void_p(dts.ctypes.data)))
+            return dts
+        self._check(lib().ns2d_step_cfl(self._h, float(cfl), float(t_end), None))
+        return None
+
+    def step_dts(self, dts):
+        d = np.ascontiguousarray(dts, dtype=np.float64)
+        assert d.shape == (self.batch,)
+        self._check(lib().ns2d_step_dts(self._h, ctypes.c_void_p(d.ctypes.data)))
+
+    def advance(self, cfl, t_end, max_steps=1 << 30):
+        n = ctypes.c_int(0)
+        self._check(lib().ns2d_advance(self._h, float(cfl), float(t_end), int(max_steps), ctypes.byref(n)))
+        return n.value
+
+    def max_velocity(self):
+        out = np.empty(self.batch, dtype=np.float64)
+        self._check(lib().ns2d_max_velocity(self._h, ctypes.c_void_p(out.ctypes.data)))
+        return out
+
+    def energy_spectrum(self, nbins):
+        E = np.empty((self.batch, int(nbins)), dtype=np.float64)
+        self._check(lib().ns2d_energy_spectrum(self._h, ctypes.c_void_p(E.ctypes.data), int(nbins)))
+        return E
+
+    def enstrophy_spectrum(self, nbins):
+        Z = np.empty((self.batch, int(nbins)), dtype=np.float64)
+        self._check(lib().ns2d_enstrophy_spectrum(self._h, ctypes.c_void_p(Z.ctypes.data), int(nbins)))
+        return Z
+
+    def profile(self, enable=True):
+        self._check(lib().ns2d_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        ms = np.zeros(4, dtype=np.float64)
+        cnt = np.zeros(4, dtype=np.int64)
+        self._check(lib().ns2d_profile_read(self._h, ctypes.c_void_p(ms.ctypes.data), ctypes.c_void_p(cnt.ctypes.data)))
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(self.PASS_NAMES)}
+
+    def time(self, sample=0):
+        return float(lib().ns2d_time(self._h, int(sample)))
+
+    def kernel_launches(self):
+        return int(lib().ns2d_kernel_launches(self._h))
+
+    def device_bytes(self):
+        return int(lib().ns2d_device_bytes(self._h))

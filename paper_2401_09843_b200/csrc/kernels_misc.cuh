@@ -104,14 +104,14 @@ __device__ __forceinline__ bool nonfinite_sq(unsigned long long bits) {
     const double um2 = __longlong_as_double((long long)bits);
     return !(um2 < CUDART_INF);
 }
-__global__ void set_dt_uniform_kernel(double* dt, double* t, double value, const unsigned long long* umax2, int* bad, int batch) {
+static __global__ void set_dt_uniform_kernel(double* dt, double* t, double value, const unsigned long long* umax2, int* bad, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
     if (nonfinite_sq(umax2[b])) { bad[b] = 1; value = 0.0; }
     dt[b] = value;
     t[b] += value;
 }
-__global__ void set_dt_array_kernel(double* dt, double* t, const double* src, const unsigned long long* umax2, int* bad, int batch) {
+static __global__ void set_dt_array_kernel(double* dt, double* t, const double* src, const unsigned long long* umax2, int* bad, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
     double value = src[b];
@@ -120,7 +120,7 @@ __global__ void set_dt_array_kernel(double* dt, double* t, const double* src, co
     t[b] += value;
 }
 // dt_b = min(cfl * dx / umax_b, t_end - t_b); 0 for finished samples.
-__global__ void cfl_finalize_kernel(double* dt, double* t, const unsigned long long* umax2, int* bad, double cfl, double dx,
+static __global__ void cfl_finalize_kernel(double* dt, double* t, const unsigned long long* umax2, int* bad, double cfl, double dx,
                                     double t_end, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
@@ -136,7 +136,7 @@ __global__ void cfl_finalize_kernel(double* dt, double* t, const unsigned long l
     dt[b] = v;
     t[b] += v;
 }
-__global__ void umax_read_kernel(double* out, const unsigned long long* umax2, int* bad, int batch) {
+static __global__ void umax_read_kernel(double* out, const unsigned long long* umax2, int* bad, int batch) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
     if (nonfinite_sq(umax2[b])) bad[b] = 1;
@@ -244,7 +244,7 @@ __global__ void sf_marginals_kernel(const cx<T>* __restrict__ U, double* __restr
         if (bins[i] != 0.0) atomicAdd(&marg[b * 3 * N + i], bins[i]);
 }
 // one block per sample, thread per l
-__global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __restrict__ S, int N, int nl) {
+static __global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __restrict__ S, int N, int nl) {
     const int b = blockIdx.x;
     for (int l = 1 + threadIdx.x; l <= nl; l += blockDim.x) {
         double acc = 0.0;
@@ -264,14 +264,14 @@ __global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __re
 // ------------------------------------------------------------------------------------------------
 // unpadded N-grid transforms for ns_set_initial / ns_get_fields / the physical-space statistics (NOT on the hot path):
 // a shared-memory FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place, n = 2^a or 3 * 2^a.
-//   axis 0: element stride n*n, axis 1: n, axis 2: 1.
+//   axis 0: element stride n*n, axis 1: n, axis 2: 1.  dim = 2: the same on [planes][n][n] (axes 1 and 2).
 // n = 3 m: the three decimated sequences x[3r + q] are transformed by radix-2 stages (m = 2^a) and combined by one
 // radix-3 stage, X[k + m t] = sum_q w_n^{q (k + m t)} F_q[k].  Twiddles come from the table gtw[j] = exp(+2 pi i j / n).
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(256)
 generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis, int sign, long total_tiles,
-                   const cx<T>* __restrict__ gtw) {
+                   const cx<T>* __restrict__ gtw, int dim) {
     constexpr int TL = 8;  // lines per tile
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);  // [n][TL+1]
@@ -280,16 +280,18 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis
     if (tile >= total_tiles) return;
     const int m = 1 << log2m;          // n = m or 3 m
     const int nsub = radix3 ? 3 : 1;
+    // dim = 3: cubes [n][n][n], n^2 lines per cube and axis; dim = 2: planes [n][n] (axes 1 and 2 only), n lines per plane
     const long n2 = (long)n * n;
-    const long tiles_per_cube = n2 / TL;
+    const long lines = dim == 3 ? n2 : n;
+    const long tiles_per_cube = lines / TL;
     const long cube = tile / tiles_per_cube;
     const long l0 = (tile % tiles_per_cube) * TL;  // first line id within the cube
-    cx<T>* base = A + cube * n2 * n;
+    cx<T>* base = A + cube * (dim == 3 ? n2 * n : n2);
     const long es = axis == 0 ? n2 : (axis == 1 ? n : 1);
     // line id l -> offset of element 0
     auto line_base = [&](long l) -> long {
         if (axis == 0) return l;
-        if (axis == 1) return (l / n) * n2 + (l % n);
+        if (axis == 1) return dim == 3 ? (l / n) * n2 + (l % n) : l;
         return l * n;
     };
     auto root = [&](int j) -> cx<T> {   // exp(sign 2 pi i j / n), 0 <= j < n
@@ -447,7 +449,7 @@ __global__ void sf_p_kernel(const T* __restrict__ u, double* __restrict__ S, int
     }
 }
 
-__global__ void scale_kernel(double* __restrict__ a, double s, int n) {
+static __global__ void scale_kernel(double* __restrict__ a, double s, int n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) a[i] *= s;
 }

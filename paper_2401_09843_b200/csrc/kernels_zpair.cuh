@@ -149,6 +149,86 @@ __device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, i
     }
 }
 
+// One warp per tensor-memory lane quarter parks the twiddles of its lanes: ttw <- w_L^{r1 t} (r1 = 0..15), tw3 <- W^{t + G j}
+// (j = 0..15); both depend on the lane only, so the warps that share the quarter share them.
+template <typename T, int L>
+__device__ __forceinline__ void zp_park_twiddles(uint32_t ttw, uint32_t tw3, int t, const Twiddles<T>& tw) {
+    constexpr int G = ZPGeo<T, L>::G, CH = tmem_cx_chunk<T>();
+#pragma unroll
+    for (int ch = 0; ch < 16 / CH; ++ch) {
+        T wr[CH], wi[CH], vr[CH], vi[CH];
+#pragma unroll
+        for (int e = 0; e < CH; ++e) {
+            const cx<T> w = ldg(tw.z16 + (ch * CH + e) * G + t);
+            wr[e] = w.x;
+            wi[e] = w.y;
+            const cx<T> u = ldg(tw.w3a + t + G * (ch * CH + e));
+            vr[e] = u.x;
+            vi[e] = u.y;
+        }
+        tmem_store_cx(ttw + 16 * ch, wr, wi);
+        tmem_store_cx(tw3 + 16 * ch, vr, vi);
+    }
+    tmem_wait_st();
+}
+
+// Input of an inverse job: v[j] = s_q[t + G j] for the two-for-one field ua + i ub with half spectra Ua, Ub (shared memory).
+// Radix-3 pruning of warp q: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q}, with the third
+// sub-transform taken as q = -1 (physical points 3r - 1 instead of 3r + 2: the physical order along the contiguous axis never
+// leaves the kernel), so that both q != 0 warps use the same twiddles W^{n}, one of them conjugated.
+// a_n = Ua[n] + i Ub[n], c_n = conj(Ua[L-n]) + i conj(Ub[L-n]) (kernels_z.cuh); n = 0: real parts only, c = 0.
+template <typename T, int L>
+__device__ __forceinline__ void zp_form_inverse(cx<T> (&v)[16], const cx<T>* __restrict__ Ua, const cx<T>* __restrict__ Ub, int q, int t,
+                                                uint32_t tw3) {
+    constexpr int G = ZPGeo<T, L>::G, CH = tmem_cx_chunk<T>();
+    const T alpha = q == 0 ? (T)1 : (T)-0.5;
+    const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
+    const T sg = q == 2 ? (T)-1 : (T)1;     // sign of the imaginary part of the twiddle: W^{+n} (q = 1), W^{-n} (q = -1)
+#pragma unroll
+    for (int ch = 0; ch < 16 / CH; ++ch) {
+        T wr[CH], wi[CH];
+        tmem_load_cx(tw3 + 16 * ch, wr, wi);
+#pragma unroll
+        for (int e = 0; e < CH; ++e) {
+            const int j = ch * CH + e;
+            const int n = t + G * j;
+            const cx<T> pa = Ua[n], pb = Ub[n];
+            const cx<T> ma = Ua[(L - n) & (L - 1)], mb = Ub[(L - n) & (L - 1)];
+            cx<T> a = mk<T>(pa.x - pb.y, pa.y + pb.x);
+            cx<T> c = mk<T>(ma.x + mb.y, mb.x - ma.y);
+            if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
+            // z = a + c (alpha + i beta)
+            cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
+            if (q > 0) z = cmul(z, mk<T>(wr[e], sg * wi[e]));
+            v[j] = z;
+        }
+    }
+}
+
+// Output of a forward job (run through the inverse butterflies on conjugated input): G_q[k] = conj(v) W^{-qk} into the warp's
+// region in natural order, k = t + G j at row j, column lane.
+template <typename T, int L>
+__device__ __forceinline__ void zp_post_forward(const cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int q, uint32_t tw3) {
+    constexpr int G = ZPGeo<T, L>::G, CH = tmem_cx_chunk<T>();
+    const T sg = q == 2 ? (T)-1 : (T)1;
+#pragma unroll
+    for (int ch = 0; ch < 16 / CH; ++ch) {
+        T wr[CH], wi[CH];
+        tmem_load_cx(tw3 + 16 * ch, wr, wi);
+#pragma unroll
+        for (int e = 0; e < CH; ++e) {
+            const int j = ch * CH + e;
+            const cx<T> y = v[zp_perm<G>(j)];
+            cx<T> w = mk<T>(y.x, -y.y);
+            if (q > 0) {   // conj(y) conj(r) = conj(y r), r = W^{qk}
+                const T rx = wr[e], ry = sg * wi[e];
+                w = mk<T>(y.x * rx - y.y * ry, -(y.x * ry + y.y * rx));
+            }
+            Sw[j * 32 + (lane ^ (j & 7))] = w;
+        }
+    }
+}
+
 // in [batch][3][MM][L] complex -> out [batch][5][MM][L] complex (unnormalised transforms of the flux components, order
 // 11 12 13 22 23).  total_pairs = batch * MM / 2 line pairs; (MM / 2) % (32 / G) == 0 (a warp never straddles two samples).
 template <typename T, int L, int UNITS>
@@ -213,25 +293,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     const uint32_t tbase = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + (uint32_t)(warp / 4) * Geo::WCOLS;
     const uint32_t ttw = tslot + ((uint32_t)(32 * (warp % 4)) << 16) + FIELD_COLS;
     const uint32_t tw3 = ttw + 2 * C16;
-    if (warp < 4) {   // one warp per lane quarter parks the twiddles of its lanes: w_L^{r1 t} and W^{t + G j} (both depend on the lane only)
-        constexpr int CH = tmem_cx_chunk<T>();
-#pragma unroll
-        for (int ch = 0; ch < 16 / CH; ++ch) {
-            T wr[CH], wi[CH], vr[CH], vi[CH];
-#pragma unroll
-            for (int e = 0; e < CH; ++e) {
-                const cx<T> w = ldg(tw.z16 + (ch * CH + e) * G + t);
-                wr[e] = w.x;
-                wi[e] = w.y;
-                const cx<T> u = ldg(tw.w3a + t + G * (ch * CH + e));
-                vr[e] = u.x;
-                vi[e] = u.y;
-            }
-            tmem_store_cx(ttw + 16 * ch, wr, wi);
-            tmem_store_cx(tw3 + 16 * ch, vr, vi);
-        }
-        tmem_wait_st();
-    }
+    if (warp < 4) zp_park_twiddles<T, L>(ttw, tw3, t, tw);
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
@@ -268,33 +330,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                 mbar_wait(bar_lg + (jn & 1), (uint32_t)((jn >> 1) & 1));
                 const cx<T>* Ua = Ulg + (jn & 1) * SLOT;
                 const cx<T>* Ub = Ua + L;
-                // radix-3 pruning of this warp: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q},
-                // with the third sub-transform taken as q = -1 (physical points 3r - 1 instead of 3r + 2: the physical z order
-                // never leaves this kernel), so that both q != 0 warps use the same twiddles W^{n}, one of them conjugated
-                const T alpha = q == 0 ? (T)1 : (T)-0.5;
-                const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
-                const T sg = q == 2 ? (T)-1 : (T)1;     // sign of the imaginary part of the twiddle: W^{+n} (q = 1), W^{-n} (q = -1)
-                // a_n = Ua[n] + i Ub[n], c_n = conj(Ua[L-n]) + i conj(Ub[L-n]) (kernels_z.cuh); n = 0: real parts only, c = 0
-                constexpr int CH = tmem_cx_chunk<T>();
-#pragma unroll
-                for (int ch = 0; ch < 16 / CH; ++ch) {
-                    T wr[CH], wi[CH];
-                    tmem_load_cx(tw3 + 16 * ch, wr, wi);
-#pragma unroll
-                    for (int e = 0; e < CH; ++e) {
-                        const int j = ch * CH + e;
-                        const int n = t + G * j;
-                        const cx<T> pa = Ua[n], pb = Ub[n];
-                        const cx<T> ma = Ua[(L - n) & (L - 1)], mb = Ub[(L - n) & (L - 1)];
-                        cx<T> a = mk<T>(pa.x - pb.y, pa.y + pb.x);
-                        cx<T> c = mk<T>(ma.x + mb.y, mb.x - ma.y);
-                        if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
-                        // z = a + c (alpha + i beta)
-                        cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
-                        if (q > 0) z = cmul(z, mk<T>(wr[e], sg * wi[e]));
-                        v[j] = z;
-                    }
-                }
+                zp_form_inverse<T, L>(v, Ua, Ub, q, t, tw3);
             } else {
                 // products of the physical fields, conjugated (forward through the inverse butterflies), in natural order;
                 // the fields are fetched from tensor memory one x16 access (VPA values) at a time to bound the live registers
@@ -350,25 +386,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                 tmem_wait_st();
             } else {
                 tmem_wait_st();
-                // G_q[k] = conj(v) W^{-qk} into this warp's region, natural order: k = t + G j at row j, column lane
-                constexpr int CH = tmem_cx_chunk<T>();
-                const T sg = q == 2 ? (T)-1 : (T)1;
-#pragma unroll
-                for (int ch = 0; ch < 16 / CH; ++ch) {
-                    T wr[CH], wi[CH];
-                    tmem_load_cx(tw3 + 16 * ch, wr, wi);
-#pragma unroll
-                    for (int e = 0; e < CH; ++e) {
-                        const int j = ch * CH + e;
-                        const cx<T> y = v[zp_perm<G>(j)];
-                        cx<T> w = mk<T>(y.x, -y.y);
-                        if (q > 0) {   // conj(y) conj(r) = conj(y r), r = W^{qk}
-                            const T rx = wr[e], ry = sg * wi[e];
-                            w = mk<T>(y.x * rx - y.y * ry, -(y.x * ry + y.y * rx));
-                        }
-                        Sw[j * 32 + (lane ^ (j & 7))] = w;
-                    }
-                }
+                zp_post_forward<T, L>(v, Sw, lane, q, tw3);
                 named_bar_sync(bar_id, 96);
                 // all three warps are past the inverse jobs that read the input slots: refill them
                 if (issuer && (job == 2 || job == 5)) {

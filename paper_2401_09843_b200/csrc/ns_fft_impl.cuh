@@ -5,6 +5,7 @@
 #include "kernels_zfused.cuh"
 #include "kernels_zfused8.cuh"
 #include "kernels_zpair.cuh"
+#include "kernels_y2d.cuh"
 #include <cstdlib>
 #include <cstring>
 #include "ns_internal.h"
@@ -262,12 +263,43 @@ cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in,
     }
 }
 
+template <typename T, int L>
+static cudaError_t y2d_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long M, long batch, unsigned long long* umax2,
+                         Twiddles<T> tw) {
+    using Geo = ZPGeo<T, L>;
+    constexpr int UNITS = 4;
+    auto k = y2d_kernel<T, L, UNITS>;
+    const size_t smem = (size_t)UNITS * Geo::UNIT_BYTES;
+    cudaError_t e = set_smem(k, smem);
+    if (e != cudaSuccess) return e;
+    if ((M % Geo::PL) != 0 || M * batch >= (1L << 31)) return cudaErrorInvalidValue;
+    const long lines = M * batch, per_block = (long)UNITS * Geo::PL;
+    long grid = num_sms;
+    const long need = (lines + per_block - 1) / per_block;
+    if (grid > need) grid = need;
+    k<<<(unsigned)grid, 96 * UNITS, smem, st>>>(in, out, (unsigned)M, (unsigned)lines, umax2, tw);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_y2d(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long M, long batch,
+                       unsigned long long* umax2, Twiddles<T> tw) {
+    switch (L) {
+        case 64: return y2d_L<T, 64>(st, num_sms, in, out, M, batch, umax2, tw);
+        case 128: return y2d_L<T, 128>(st, num_sms, in, out, M, batch, umax2, tw);
+        case 256: return y2d_L<T, 256>(st, num_sms, in, out, M, batch, umax2, tw);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
 #define NS_INSTANTIATE_FFT(T)                                                                                      \
     template cudaError_t launch_col_inv<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, Twiddles<T>);                                                     \
     template cudaError_t launch_col_fwd<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
                                            long, T, Twiddles<T>);                                                  \
     template cudaError_t launch_z_fused<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*, \
-                                           Twiddles<T>);
+                                           Twiddles<T>);                                                           \
+    template cudaError_t launch_y2d<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*,     \
+                                       Twiddles<T>);
 
 }  // namespace ns

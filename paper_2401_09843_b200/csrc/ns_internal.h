@@ -56,4 +56,9 @@ template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw);
 
+// fused contiguous-axis kernel of the 2-D solver (kernels_y2d.cuh), L in {64, 128, 256}: in [batch][2][M][L] -> out [batch][2][M][L]
+template <typename T>
+cudaError_t launch_y2d(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long M, long batch,
+                       unsigned long long* umax2, Twiddles<T> tw);
+
 }  // namespace ns

@@ -419,7 +419,7 @@ public:
         if (smem > 48 * 1024)
             NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         for (int axis = 0; axis < 3; ++axis) {
-            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2m, radix3, axis, sign, tiles, tw().gN);
+            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2m, radix3, axis, sign, tiles, tw().gN, 3);
             NS_LAUNCHED("generic_fft");
         }
         return NS_OK;

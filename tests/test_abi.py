@@ -16,10 +16,10 @@ def libns():
     return binding.lib()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "ns.h")).read()
+def declared_symbols(header="ns.h", prefix="ns_"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(ns_[a-z_0-9]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(" + prefix + r"[a-z_0-9]+)\s*\(", text)))
 
 
 def test_header_symbols_exported(libns):
@@ -29,6 +29,11 @@ def test_header_symbols_exported(libns):
     for s in syms:
         assert hasattr(libns, s), f"libns.so does not export {s}"
     assert sorted(binding.EXPORTS) == syms
+    syms2 = declared_symbols("ns2d.h", "ns2d_")
+    assert len(syms2) >= 15
+    for s in syms2:
+        assert hasattr(libns, s), f"libns.so does not export {s}"
+    assert sorted(binding.EXPORTS_2D) == syms2
 
 
 def test_no_torch_types_in_header():
@@ -51,6 +56,9 @@ def test_create_rejects_bad_arguments(libns):
     assert libns.ns_create(None, 32, 1, None, 0, None) == binding.NS_ERR_INVALID_ARG
     assert libns.ns_destroy(None) == binding.NS_ERR_INVALID_ARG
     assert libns.ns_step(None, 0.1) == binding.NS_ERR_INVALID_ARG
+    for N, batch, dtype in [(64, 1, 0), (96, 1, 0), (1024, 1, 0), (256, 0, 0), (256, 1, 7)]:
+        assert libns.ns2d_create(ctypes.byref(h), N, batch, None, dtype, None) == binding.NS_ERR_INVALID_ARG and not h.value
+    assert libns.ns2d_destroy(None) == binding.NS_ERR_INVALID_ARG and libns.ns2d_step(None, 0.1) == binding.NS_ERR_INVALID_ARG
 
 
 def test_no_cpu_fallback(libns):
@@ -65,6 +73,9 @@ def test_no_cpu_fallback(libns):
     assert b"no usable CUDA device" in libns.ns_last_error(None)
     with pytest.raises(binding.NSError):
         binding.Solver(32, stream=0)
+    assert libns.ns2d_create(ctypes.byref(h), 256, 4, None, 0, None) == binding.NS_ERR_CUDA
+    with pytest.raises(binding.NSError):
+        binding.Solver2D(256, stream=0)
 
 
 def test_product_does_not_import_oracle():
@@ -102,9 +113,9 @@ def test_sass_is_blackwell_native():
             for m in ("UBLKCP", "LDTM", "STTM", "UTCATOMSWS", "DFMA"):
                 if m in line:
                     per_fn[name].add(m)
-    z = {k: v for k, v in per_fn.items() if "z_fused" in k}
-    assert z and all("UBLKCP" in v for v in z.values())
-    tm = {k: v for k, v in per_fn.items() if "z_fused16t" in k or "_tmem_kernel" in k}
-    assert len(tm) >= 6 and all({"LDTM", "STTM", "UTCATOMSWS"} <= v for v in tm.values())
+    z = {k: v for k, v in per_fn.items() if "z_fused" in k or "z_pair" in k or "y2d_kernel" in k}
+    assert len(z) >= 12 and all("UBLKCP" in v for v in z.values())
+    tm = {k: v for k, v in per_fn.items() if "z_pair" in k or "y2d_kernel" in k or "_tmem_kernel" in k}
+    assert len(tm) >= 12 and all({"LDTM", "STTM", "UTCATOMSWS"} <= v for v in tm.values())
     ldd = subprocess.run(["ldd", binding.LIB_PATH], capture_output=True, text=True).stdout
     assert "cufft" not in ldd.lower() and "cublas" not in ldd.lower()
