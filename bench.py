@@ -333,12 +333,79 @@ def run_workload(binding, torch, name, dtype, steps, warmup, dist, world, rank, 
     return rec, s, one_step
 
 
+WORKLOADS_2D = {
+    # the two-dimensional solver on a large ensemble in one launch
+    "e2d": dict(N=512, batch=1024, params=dict(eps=0.05, s=1.0), cfl=0.2,
+                desc="NEXT-4: 1024 x 512^2 two-dimensional perturbed shear-layer ensemble in one launch, hyperviscosity eps=0.05 s=1, CFL 0.2"),
+}
+
+
+def run_workload_2d(binding, torch, name, dtype, steps, warmup, local, rank=0):
+    """The 2-D solver on a large batch: same timing rules as run_workload (CUDA events on the solver's stream, profiler off in
+    the timed region, split from a second short run)."""
+    w = WORKLOADS_2D[name]
+    N, batch = w["N"], w["batch"]
+    cbytes = 16 if dtype == "f64" else 8
+    t0 = time.perf_counter()
+    u0 = np.stack([inputs.shear_layer_2d(N, 2000 + 10007 * rank + i) for i in range(batch)])
+    s = binding.Solver2D(N, batch=batch, dtype=dtype, **w["params"])
+    s.set_initial(u0)
+    chk = inputs.checksum(u0[0])
+    del u0
+    setup = time.perf_counter() - t0
+    for _ in range(warmup):
+        s.step_cfl(w["cfl"], 1e30, return_dt=False)
+    torch.cuda.synchronize()
+    launches0 = s.kernel_launches()
+    sampler = ClockSampler(local)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(steps):
+        s.step_cfl(w["cfl"], 1e30, return_dt=False)
+    b.record()
+    torch.cuda.synchronize()
+    total_ms = a.elapsed_time(b)
+    clocks = sampler.stop()
+    launches = s.kernel_launches() - launches0
+    nsplit = min(steps, 5)
+    s.profile(True)
+    for _ in range(nsplit):
+        s.step_cfl(w["cfl"], 1e30, return_dt=False)
+    prof = s.profile_read()
+    s.profile(False)
+    E = s.energy_spectrum(N)
+    finite = bool(np.isfinite(E).all() and (E.sum(axis=1) > 0).all())
+    ms_per_step = total_ms / steps
+    peak, peak_src = measured_peaks()
+    built = roofline.built_pass_bytes_per_step_2d(N, batch, cbytes)
+    split_ms = sum(prof[k][0] for k in built) / nsplit
+    kernels = {}
+    for k, nbytes in built.items():
+        ms, cnt = prof[k]
+        if cnt:
+            gbs = nbytes * nsplit / (ms * 1e-3) / 1e9
+            kernels[k] = {"ms_per_launch": ms / cnt, "launches": cnt, "alg_bytes_per_launch": nbytes * nsplit / cnt, "gbs": gbs,
+                          "frac": gbs / peak, "share_of_step": ms / nsplit / split_ms}
+    dom = max(kernels, key=lambda k: kernels[k]["ms_per_launch"] * kernels[k]["launches"])
+    actual = sum(built.values())
+    model = roofline.fixed_step_bytes_2d(N, batch, cbytes)
+    return {"workload": name, "desc": w["desc"], "dtype": dtype, "ms_per_step": ms_per_step, "steps": steps,
+            "value": roofline.grid_point_stages_2d(N, batch, steps) / (total_ms * 1e-3), "unit": "grid-point-stages/s (2-D: batch * N^2 * 3 per step)",
+            "step_roofline": {"bound": "hbm", "bytes_per_step": actual, "achieved_gbs": actual / (ms_per_step * 1e-3) / 1e9, "peak": peak,
+                              "frac": actual / (ms_per_step * 1e-3) / 1e9 / peak,
+                              "fixed_model": {"bytes_per_step": model, "speed_ratio_vs_model_at_measured_peak": model / (peak * 1e9) * 1e3 / ms_per_step}},
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s", "frac": kernels[dom]["frac"],
+                         "traffic": None, "peak_source": peak_src},
+            "kernels": kernels, "clocks": clocks, "gpu_launches": launches, "state_finite": finite, "input_checksum": chk,
+            "setup_s": round(setup, 1), "device_bytes": s.device_bytes(), "l2": "inputs exceed L2 (126 MB): no flush needed"}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS) + sorted(WORKLOADS_2D))
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
@@ -362,6 +429,18 @@ def main():
         dist.all_reduce(x)
         assert int(x.item()) == world
     from paper_2401_09843_b200 import binding
+
+    if args.workload in WORKLOADS_2D:      # the 2-D solver as the headline of this invocation (single GPU)
+        r = run_workload_2d(binding, torch, args.workload, args.dtype, args.steps, args.warmup, local, rank)
+        if rank == 0:
+            print(json.dumps({"metric": "grid_point_stages_per_s", "value": r["value"], "unit": r["unit"], "n_gpus": 1, "steps": args.steps,
+                              "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                              "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+                              "config": {"workload": r["desc"], "N": WORKLOADS_2D[args.workload]["N"], "batch_per_gpu": WORKLOADS_2D[args.workload]["batch"],
+                                         "l2": r["l2"], "state_finite": r["state_finite"], "input_checksum": r["input_checksum"]},
+                              "roofline": r["roofline"], "step_roofline": r["step_roofline"], "kernels": r["kernels"], "cpu_baseline": None,
+                              "e2e": None, "also": {}, "gpu_launches": r["gpu_launches"], "clocks": r["clocks"], "device_bytes": r["device_bytes"]}))
+        return 0
 
     w = WORKLOADS[args.workload]
     N, batch = w["N"], w["batch"]
@@ -409,6 +488,8 @@ def main():
         r4, s4, _ = run_workload(binding, torch, "c4", "f64", 10, 3, dist, world, rank, local)
         del s4
         also["c4_f64"] = r4
+        if world == 1:
+            also["e2d_f64"] = run_workload_2d(binding, torch, "e2d", "f64", 10, 3, local, rank)
     else:
         del s
 

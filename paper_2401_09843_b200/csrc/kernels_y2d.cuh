@@ -32,7 +32,6 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
     const int lane = threadIdx.x & 31;
     const int lg = lane / G, t = lane % G;
     const int lgcol = lg * G;
-    const int tl = q * G + t;
 
     unsigned char* ubase = smem_raw + (size_t)unit * Geo::UNIT_BYTES;
     cx<T>* In = reinterpret_cast<cx<T>*>(ubase);
@@ -107,7 +106,7 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
         named_bar_sync(bar_id, 96);
         // all three warps have consumed this line's slot: refill it with the line after next
         if (issuer && line + 2 * (unsigned long long)stride < total_lines) issue(line + 2 * stride, it + 2);
-        zp_combine_store<T, L>(Ex, lgcol, Oa, Oa + cs, tl);
+        zp_combine_store<T, L>(Ex, lgcol, Oa, Oa + cs, q, t);
         named_bar_sync(bar_id, 96);
     }
     tmem_fence_before_sync();

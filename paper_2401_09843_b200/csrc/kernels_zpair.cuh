@@ -103,51 +103,67 @@ __device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__
 }
 
 // 3 -> 2 radix-3 combine + Hermitian split of one forward job: reads G_q[n] = F_q[n] W^{-qn} of the three sub-transforms
-// (regions REGION apart, swizzled as above, element n at row n / G, column lgcol + n % G) and writes the two real
-// transforms B_a^[n], B_b^[n] for n and L - n (kernels_z.cuh).  Threads tl = 0..3G-1 of the line pair cover n <= L/2.
+// (regions REGION apart, swizzled as above, element n at row n / G, column lgcol + n % G) and writes TWICE the two real
+// transforms, 2 B_a^[n] and 2 B_b^[n], for n and L - n (kernels_z.cuh; the factor 1/2 of the Hermitian split is folded into the
+// normalisation of the spectral kernel, see zp_output_scale).  The 8G + 1 values n <= L/2 are shared out unevenly on
+// purpose: the q = 0 warp has no radix-3 twiddles to apply in the transforms, so it takes half of the combine
+// (n < 4G), the other two a quarter each -- the three warps then reach the named barriers at about the same time.
 template <typename T, int L>
-__device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, int lgcol, cx<T>* __restrict__ Oa, cx<T>* __restrict__ Ob, int tl) {
-    constexpr int G = ZPGeo<T, L>::G, REGION = ZPGeo<T, L>::REGION, TPL = 3 * G;
-    constexpr int NIT = (L / 2 + TPL) / TPL;  // iterations covering n in [0, L/2]
+__device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, int lgcol, cx<T>* __restrict__ Oa, cx<T>* __restrict__ Ob, int q,
+                                                 int t) {
+    constexpr int G = ZPGeo<T, L>::G, REGION = ZPGeo<T, L>::REGION;
     constexpr T h3 = (T)0.86602540378443864676L;
     auto at = [&](int qq, int n) {
         const int row = n / G, col = lgcol + n % G;
         return Su[qq * REGION + row * 32 + (col ^ (row & 7))];
     };
-    cx<T> f0[NIT], g1[NIT], g2[NIT], f0m[NIT], g1m[NIT], g2m[NIT];
+    // q = 0: n = t + G i, i < 4;  q = 1: n = 4G + t + G i, i < 2;  q = 2: n = 6G + t + G i, i < 2;  n = 8G = L/2: lane t = 0 of q = 2
+    const int n0 = q == 0 ? t : (q == 1 ? 4 * G + t : 6 * G + t);
+    auto one = [&](cx<T> f0, cx<T> g1, cx<T> g2, cx<T>& A, cx<T>& C) {
+        const cx<T> S = g1 + g2, D = g1 - g2;
+        A = f0 + S;
+        C = mk<T>(f0.x - (T)0.5 * S.x - h3 * D.y, f0.y - (T)0.5 * S.y + h3 * D.x);
+    };
 #pragma unroll
-    for (int it = 0; it < NIT; ++it) {
-        int n = tl + it * TPL;
-        if (n > L / 2) n = L / 2;             // clamped duplicate, not stored
-        const int m = n == 0 ? 0 : L - n;
-        f0[it] = at(0, n); g1[it] = at(1, n); g2[it] = at(2, n);
-        f0m[it] = at(0, m); g1m[it] = at(1, m); g2m[it] = at(2, m);
-    }
+    for (int half = 0; half < 2; ++half) {
+        if (half == 1 && q != 0) break;          // warp-uniform: only the q = 0 warp has a second pair of values
+        cx<T> f0[2], g1[2], g2[2], f0m[2], g1m[2], g2m[2];
 #pragma unroll
-    for (int it = 0; it < NIT; ++it) {
-        const int n = tl + it * TPL;
-        const cx<T> Sn = g1[it] + g2[it], Dn = g1[it] - g2[it];
-        const cx<T> An = f0[it] + Sn;
-        const cx<T> Cn = mk<T>(f0[it].x - (T)0.5 * Sn.x - h3 * Dn.y, f0[it].y - (T)0.5 * Sn.y + h3 * Dn.x);
-        const cx<T> Sm = g1m[it] + g2m[it], Dm = g1m[it] - g2m[it];
-        const cx<T> Am = f0m[it] + Sm;
-        const cx<T> Cm = mk<T>(f0m[it].x - (T)0.5 * Sm.x - h3 * Dm.y, f0m[it].y - (T)0.5 * Sm.y + h3 * Dm.x);
-        if (n <= L / 2) {
+        for (int k = 0; k < 2; ++k) {
+            const int n = n0 + G * (2 * half + k);
+            const int m = n == 0 ? 0 : L - n;
+            f0[k] = at(0, n); g1[k] = at(1, n); g2[k] = at(2, n);
+            f0m[k] = at(0, m); g1m[k] = at(1, m); g2m[k] = at(2, m);
+        }
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const int n = n0 + G * (2 * half + k);
+            cx<T> An, Cn, Am, Cm;
+            one(f0[k], g1[k], g2[k], An, Cn);
+            one(f0m[k], g1m[k], g2m[k], Am, Cm);
             if (n == 0) {
-                stg_stream(Oa, mk<T>(An.x, 0));
-                stg_stream(Ob, mk<T>(An.y, 0));
+                stg_stream(Oa, mk<T>(An.x + An.x, 0));
+                stg_stream(Ob, mk<T>(An.y + An.y, 0));
             } else {
                 const int m = L - n;
-                stg_stream(Oa + n, mk<T>((T)0.5 * (An.x + Cm.x), (T)0.5 * (An.y - Cm.y)));
-                stg_stream(Ob + n, mk<T>((T)0.5 * (An.y + Cm.y), (T)0.5 * (Cm.x - An.x)));
-                if (m != n) {
-                    stg_stream(Oa + m, mk<T>((T)0.5 * (Am.x + Cn.x), (T)0.5 * (Am.y - Cn.y)));
-                    stg_stream(Ob + m, mk<T>((T)0.5 * (Am.y + Cn.y), (T)0.5 * (Cn.x - Am.x)));
-                }
+                stg_stream(Oa + n, mk<T>(An.x + Cm.x, An.y - Cm.y));
+                stg_stream(Ob + n, mk<T>(An.y + Cm.y, Cm.x - An.x));
+                stg_stream(Oa + m, mk<T>(Am.x + Cn.x, Am.y - Cn.y));
+                stg_stream(Ob + m, mk<T>(Am.y + Cn.y, Cn.x - Am.x));
             }
         }
     }
+    if (q == 2 && t == 0) {                      // n = L/2 is its own partner
+        constexpr int n = L / 2;
+        cx<T> An, Cn;
+        one(at(0, n), at(1, n), at(2, n), An, Cn);
+        stg_stream(Oa + n, mk<T>(An.x + Cn.x, An.y - Cn.y));
+        stg_stream(Ob + n, mk<T>(An.y + Cn.y, Cn.x - An.x));
+    }
 }
+
+// factor carried by the outputs of zp_combine_store relative to the plain unnormalised transform
+constexpr int zp_output_scale() { return 2; }
 
 // One warp per tensor-memory lane quarter parks the twiddles of its lanes: ttw <- w_L^{r1 t} (r1 = 0..15), tw3 <- W^{t + G j}
 // (j = 0..15); both depend on the lane only, so the warps that share the quarter share them.
@@ -253,7 +269,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     const int lane = threadIdx.x & 31;
     const int lg = lane / G, t = lane % G;
     const int lgcol = lg * G;
-    const int tl = q * G + t;                        // thread within the line pair
+
 
     unsigned char* ubase = smem_raw + (size_t)unit * Geo::UNIT_BYTES;
     cx<T>* In = reinterpret_cast<cx<T>*>(ubase);                       // [PL] x (2 slots x 2 lines x L), pitch LGPITCH
@@ -404,7 +420,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                     Oa = Ol + (p0 ? 0 : 1) * cs;
                     Ob = Ol + (p0 ? 3 : 2) * cs;
                 }
-                zp_combine_store<T, L>(Ex, lgcol, Oa, Ob, tl);
+                zp_combine_store<T, L>(Ex, lgcol, Oa, Ob, q, t);
                 named_bar_sync(bar_id, 96);  // combine reads done before the regions are reused
             }
         }

@@ -5,6 +5,7 @@ NS_INSTANTIATE_FFT(double)
 bool fft_supported(int L) {
     return L == 8 || L == 16 || L == 32 || L == 64 || L == 128 || L == 256 || L == 24 || L == 48 || L == 96 || L == 192;
 }
+int z_fused_output_scale(int L) { return (L == 64 || L == 128 || L == 256) ? zp_output_scale() : 1; }
 void fft_split(int L, int* R1, int* R2) {
     switch (L) {
         case 8: *R1 = Split<8>::R1; *R2 = Split<8>::R2; break;

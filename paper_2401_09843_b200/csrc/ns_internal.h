@@ -56,6 +56,10 @@ template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw);
 
+// factor carried by the output of launch_z_fused / launch_y2d relative to the plain unnormalised transform (the kernels of
+// kernels_zpair.cuh fold the 1/2 of their Hermitian split into the normalisation of the spectral kernel)
+int z_fused_output_scale(int L);
+
 // fused contiguous-axis kernel of the 2-D solver (kernels_y2d.cuh), L in {64, 128, 256}: in [batch][2][M][L] -> out [batch][2][M][L]
 template <typename T>
 cudaError_t launch_y2d(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long M, long batch,

@@ -268,7 +268,7 @@ public:
 
     int spectral(const cx<T>* Us, const cx<T>* Un, cx<T>* out, double alpha, double beta, double gamma, int mode) {
         const long total = (long)batch * N * N * H;
-        const T scale = (T)(1.0 / ((double)M * M * M));
+        const T scale = (T)(1.0 / ((double)M * M * M * z_fused_output_scale(L)));
         prof.tick(6, st);
         spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y, Us, Un, out, N, total, dtab, scale, (T)alpha, (T)beta,
                                                                     (T)gamma, dt_dev, mode);

@@ -137,12 +137,8 @@ def gaussian_k53(N: int = 512, seed: int = 5) -> np.ndarray:
     return gaussian_field(N, seed, spec, e_tot=0.5)
 
 
-def shear_layer(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmodes: int = 10) -> np.ndarray:
-    """Configs 3/4: doubly periodic perturbed shear layer (BASELINE.json configs[2]; cf. PAPER.md:L363-375).
-
-    u1 = tanh((y - pi/2 - s1(x))/rho) for y <= pi, tanh((3pi/2 + s2(x) - y)/rho) for y > pi;
-    u2 = 0.05 sin x; u3 = 0;  s_j(x) = sum_{k=1..10} a_jk sin(k x + b_jk), a ~ U[0,delta], b ~ U[0,2pi].
-    Not solenoidal as written; `set_initial` projects it."""
+def _shear_layer_plane(N: int, seed: int, rho: float, delta: float, nmodes: int):
+    """(u1, u2)(x, y) of the perturbed doubly periodic shear layer, each [N][N]."""
     x = 2.0 * np.pi * np.arange(N) / N
     a = uniform01(seed, 100, 2 * nmodes) * delta
     b = uniform01(seed, 101, 2 * nmodes) * 2.0 * np.pi
@@ -153,10 +149,19 @@ def shear_layer(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmod
     Y = x[None, :]
     lower = np.tanh((Y - 0.5 * np.pi - s1[:, None]) / rho)
     upper = np.tanh((1.5 * np.pi + s2[:, None] - Y) / rho)
-    u1 = np.where(Y <= np.pi, lower, upper)
+    return np.where(Y <= np.pi, lower, upper), 0.05 * np.sin(X) * np.ones_like(Y)
+
+
+def shear_layer(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmodes: int = 10) -> np.ndarray:
+    """Configs 3/4: doubly periodic perturbed shear layer (BASELINE.json configs[2]; cf. PAPER.md:L363-375).
+
+    u1 = tanh((y - pi/2 - s1(x))/rho) for y <= pi, tanh((3pi/2 + s2(x) - y)/rho) for y > pi;
+    u2 = 0.05 sin x; u3 = 0;  s_j(x) = sum_{k=1..10} a_jk sin(k x + b_jk), a ~ U[0,delta], b ~ U[0,2pi].
+    Not solenoidal as written; `set_initial` projects it."""
+    u1, u2 = _shear_layer_plane(N, seed, rho, delta, nmodes)
     u = np.zeros((3, N, N, N))
     u[0] = u1[:, :, None]
-    u[1] = (0.05 * np.sin(X) * np.ones_like(Y))[:, :, None]
+    u[1] = u2[:, :, None]
     return u
 
 
@@ -255,4 +260,4 @@ def vortex_patch(N: int, seed: int = 0, radius: float = 1.0, delta: float = 0.0)
 
 def shear_layer_2d(N: int, seed: int, rho: float = 0.05, delta: float = 0.025, nmodes: int = 10) -> np.ndarray:
     """The doubly periodic perturbed shear layer of configs 3/4 as a genuinely two-dimensional field: u[2][N][N]."""
-    return shear_layer(N, seed, rho, delta, nmodes)[:2, :, :, 0].copy()
+    return np.stack(_shear_layer_plane(N, seed, rho, delta, nmodes))

@@ -91,6 +91,31 @@ def grid_point_stages(N: int, batch: int, steps: float) -> float:
     return float(batch) * N ** 3 * 3.0 * steps
 
 
+# ---- two-dimensional solver: same accounting with d = 2.  Per sample, c = bytes per complex,
+#   S = N (N/2+1) c,  A1 = M H c,  P = M^2 c / 2.  Built passes: b1 x inverse 2(S+A1), b2 fused y (2 in + 2 trace-free flux out) 4 A1,
+#   b3 x forward 2(A1+S), b4 spectral 6 S (stage 1) / 8 S.  Fixed (unfused, three products) model: b2 = 2 A1 + 3 P, 3 (P + A1);
+#   b3 = 3 (A1 + S); b4 = 7 S / 9 S.
+BUILT_PASS_NAMES_2D = ["b1_x_inv", "b2_y_fused", "b3_x_fwd", "b4_spectral"]
+
+
+def built_pass_bytes_per_step_2d(N: int, batch: int = 1, complex_bytes: int = 16) -> dict:
+    M, H, Hs = 3 * N // 2, N // 2, N // 2 + 1
+    S, A1 = N * Hs * complex_bytes, M * H * complex_bytes
+    b = {"b1_x_inv": 3 * 2 * (S + A1), "b2_y_fused": 3 * 4 * A1, "b3_x_fwd": 3 * 2 * (A1 + S), "b4_spectral": (6 + 8 + 8) * S}
+    return {k: v * batch for k, v in b.items()}
+
+
+def fixed_step_bytes_2d(N: int, batch: int = 1, complex_bytes: int = 16) -> int:
+    M, H, Hs = 3 * N // 2, N // 2, N // 2 + 1
+    S, A1, P = N * Hs * complex_bytes, M * H * complex_bytes, M * M * complex_bytes // 2
+    per_stage = 2 * (S + A1) + (2 * A1 + 3 * P) + 3 * (P + A1) + 3 * (A1 + S)
+    return batch * (3 * per_stage + (7 + 9 + 9) * S)
+
+
+def grid_point_stages_2d(N: int, batch: int, steps: float) -> float:
+    return float(batch) * N ** 2 * 3.0 * steps
+
+
 # ---- the paper's own lower bounds, eq. (5.1)-(5.3); s = sizeof(scalar), 2s = bytes per complex, p = ranks
 def paper_t_pad(N, p, s, beta):
     return 213.0 / 16.0 * N ** 3 / p * 2 * s / beta

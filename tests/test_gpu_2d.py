@@ -32,8 +32,8 @@ def field2(N, seed):
 
 @pytest.mark.parametrize("N", [128, 256, 512])
 def test_2d_rhs_and_steps_fp64(ns, oracle2d, N):
-    """set_initial (non-solenoidal input), get_fields, one RHS (every stored entry) and 20 CFL steps with the oracle replaying
-    the GPU's dt, three samples of different recipes in one launch; spectra of the final state."""
+    """set_initial (non-solenoidal input), get_fields, one RHS (every stored entry) and 20 / 8 / 3 CFL steps with the oracle
+    replaying the GPU's dt, three samples of different recipes in one launch; spectra of the final state."""
     us = np.stack([field2(N, 100 + N) + 0.2 * inputs.normal01(N, 7, 2 * N * N).reshape(2, N, N),
                    inputs.shear_layer_2d(N, 3), inputs.vortex_patch(N, seed=5, radius=1.0, delta=0.3)])
     kw = dict(nu=0.001, eps=0.05, s=1.0)
@@ -53,11 +53,13 @@ def test_2d_rhs_and_steps_fp64(ns, oracle2d, N):
     for b in range(3):
         want = oracle2d.rhs_parts(N, p, uh[b])
         assert rel(r[b], want["r"]) < TOL_RHS_F64
-        assert np.abs(r[b] - want["r"]).max() < 1e-12 * np.abs(want["r"]).max()
+        # no single entry is off; round-off scales with the flux before the projection (for the shear layer and the vortex
+        # patch most of it is a gradient that the projection removes), so the bound is relative to max|b|, not max|R|
+        assert np.abs(r[b] - want["r"]).max() < 1e-13 * np.abs(want["b"]).max()
         assert np.all(r[b][:, N // 2] == 0) and np.all(r[b][:, :, N // 2] == 0) and np.all(r[b][:, 0, 0] == 0)
         assert abs(um[b] - want["umax"]) < 1e-13 * want["umax"]
     assert np.array_equal(s.get_spectral(), np.stack(uh))          # state unchanged by ns2d_rhs
-    nsteps = 20 if N <= 256 else 8
+    nsteps = {128: 20, 256: 8, 512: 3}[N]     # the single-threaded naive oracle needs 1.3 s per 512^2 step and sample
     worst = 0.0
     for i in range(nsteps):
         dts = s.step_cfl(0.2, 1e9)
