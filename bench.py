@@ -204,6 +204,56 @@ def run_reference(args):
     return 0
 
 
+def cufft_compare(torch, N: int, batch: int, dtype: str, reps: int = 3):
+    """Comparison line only (north_star: "cuFFT may be timed only as a comparison line"; SURVEY.md 8(d) last paragraph): the
+    transform structure of the paper's own design ("cuFFT on the device", Algorithm 2) on the same box --
+    library c2r / r2c on FULLY padded arrays with separate pad, product and truncate passes -- through torch.fft (cuFFT).  One
+    "RHS" = 3 padded inverse transforms, 6 pointwise products, 6 forward transforms, 6 truncations; the spectral / RK kernel is
+    left out (it favours the library line).  Random data; nothing here is linked into libns.so or used by the product."""
+    M, H, Hp = 3 * N // 2, N // 2 + 1, 3 * N // 4 + 1
+    rt = torch.float64 if dtype == "f64" else torch.float32
+    ct = torch.complex128 if dtype == "f64" else torch.complex64
+    g = torch.Generator(device="cuda").manual_seed(7)
+    uh = torch.view_as_complex(torch.randn(3, N, N, H, 2, dtype=rt, device="cuda", generator=g))
+    pad = torch.zeros(M, M, Hp, dtype=ct, device="cuda")
+    h = N // 2
+    pairs = [(0, 0), (0, 1), (0, 2), (1, 1), (1, 2), (2, 2)]
+
+    def one_rhs():
+        u = []
+        for c in range(3):      # Algorithm 2 steps 1-2: pad, inverse transform
+            pad[:h, :h, :H] = uh[c, :h, :h]
+            pad[:h, M - h:, :H] = uh[c, :h, h:]
+            pad[M - h:, :h, :H] = uh[c, h:, :h]
+            pad[M - h:, M - h:, :H] = uh[c, h:, h:]
+            u.append(torch.fft.irfftn(pad, s=(M, M, M), norm="forward"))
+        out = []
+        for i, j in pairs:      # steps 3-5: product, forward transform, truncate
+            bh = torch.fft.rfftn(u[i] * u[j], norm="forward")
+            out.append(torch.cat([torch.cat([bh[:h, :h, :H], bh[:h, M - h:, :H]], 1), torch.cat([bh[M - h:, :h, :H], bh[M - h:, M - h:, :H]], 1)], 0))
+            del bh
+        return out
+
+    try:
+        one_rhs()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            one_rhs()
+        b.record()
+        torch.cuda.synchronize()
+        ms_rhs = a.elapsed_time(b) / reps * batch      # samples one after the other
+    except Exception as e:      # a comparison line must never fail the bench
+        return {"unavailable": f"{type(e).__name__}: {e}"[:200]}
+    finally:
+        del pad, uh
+        torch.cuda.empty_cache()
+    return {"ms_per_rhs": ms_rhs, "ms_per_step_3_rhs": 3 * ms_rhs, "library": "cuFFT via torch.fft.irfftn / rfftn",
+            "what": f"{batch} x (3 padded {M}^3 c2r + 6 products + 6 r2c + truncation), {dtype}; pad / product / truncate as separate "
+                    "passes, no spectral kernel: the paper's Algorithm 2 with the library FFT, timed for context only"}
+
+
 PROF_LABEL = {"a1_col_inv_x": "a1_col_inv_x", "a2_col_inv_y": "a2_col_inv_y", "a3_z_inv_prod": "a3a4_z_fused",
               "a5_col_fwd_y": "a5_col_fwd_y", "a6_col_fwd_x": "a6_col_fwd_x", "a7_spectral": "a7_spectral"}
 
@@ -410,6 +460,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT (torch.fft) comparison line")
     ap.add_argument("--no-also", action="store_true", help="skip the sub-records of the other north-star targets")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
@@ -493,6 +544,10 @@ def main():
     else:
         del s
 
+    cufft = None
+    if rank == 0 and world == 1 and not args.no_cufft:
+        cufft = cufft_compare(torch, N, batch, args.dtype)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         nst = 20 if args.workload == "c1" else 3   # 128^3: about 6 s per step on the GPU box's 16 cores
@@ -510,7 +565,7 @@ def main():
                        "input_checksum": rec["input_checksum"], "setup_s": rec["setup_s"], "state_finite": rec["state_finite"],
                        "profiler": rec["profiler"]},
             "roofline": rec["roofline"], "step_roofline": rec["step_roofline"], "kernels": rec["kernels"], "cpu_baseline": cpu,
-            "e2e": e2e, "also": also, "gpu_launches": rec["gpu_launches"], "clocks": rec["clocks"], "device_bytes": rec["device_bytes"],
+            "e2e": e2e, "cufft_compare": cufft, "also": also, "gpu_launches": rec["gpu_launches"], "clocks": rec["clocks"], "device_bytes": rec["device_bytes"],
         }
         print(json.dumps(line))
     if dist is not None:
