@@ -199,40 +199,113 @@ __device__ __forceinline__ void bf3(cx<T>& x0, cx<T>& x1, cx<T>& x2) {
     x2 = mk<T>(m.x + h * d.y, m.y - h * d.x);
 }
 
-// Lengths 6 and 12 by the prime-factor algorithm (3 x 2, 3 x 4: no twiddle factors).  Input index n = (N2 n1 + 3 n2) mod N
-// (n1 < 3, n2 < N2), output index k = (N2' k1 + 3' k2) mod N by the Chinese remainder theorem; everything in place, so that
-// X[k] ends at register (N2 (k mod 3) + 3 (k mod N2)) mod N.
-template <int R, int DIR, typename T>
-__device__ __forceinline__ void fft_pfa3(cx<T>* v) {
-    constexpr int N2 = R / 3;
-    static_assert(R == 6 || R == 12, "3 x 2 or 3 x 4");
+// ------------------------------------------------------------------------------------------------
+// Odd prime radices 3, 5, 7 (sizes 2^a 3^b 5^c 7^d) and the composite register
+// lengths built from them by the prime-factor algorithm (no twiddle factors between coprime factors).
+// ------------------------------------------------------------------------------------------------
+// cos / sin of 2 pi m / P, P in {3, 5, 7}
+template <int P> __host__ __device__ constexpr double root_cos(int m) {
+    constexpr double c3[3] = {1.0, -0.5, -0.5};
+    constexpr double c5[5] = {1.0, 0.30901699437494742410, -0.80901699437494742410, -0.80901699437494742410, 0.30901699437494742410};
+    constexpr double c7[7] = {1.0, 0.62348980185873353053, -0.22252093395631440429, -0.90096886790241912624,
+                              -0.90096886790241912624, -0.22252093395631440429, 0.62348980185873353053};
+    static_assert(P == 3 || P == 5 || P == 7, "prime radix");
+    return P == 3 ? c3[m % 3] : (P == 5 ? c5[m % 5] : c7[m % 7]);
+}
+template <int P> __host__ __device__ constexpr double root_sin(int m) {
+    constexpr double s3[3] = {0.0, 0.86602540378443864676, -0.86602540378443864676};
+    constexpr double s5[5] = {0.0, 0.95105651629515357212, 0.58778525229247312917, -0.58778525229247312917, -0.95105651629515357212};
+    constexpr double s7[7] = {0.0, 0.78183148246802980871, 0.97492791218182360702, 0.43388373911755812048,
+                              -0.43388373911755812048, -0.97492791218182360702, -0.78183148246802980871};
+    return P == 3 ? s3[m % 3] : (P == 5 ? s5[m % 5] : s7[m % 7]);
+}
+
+// P-point DFT X_k = sum_n x_n exp(DIR 2 pi i nk/P), P an odd prime, on the registers v[(OFF + STR n) % MOD], in place and in
+// natural order: pairs (x_j, x_{P-j}) give X_k and X_{P-k} from the same cosine sum m and sine sum s, X = m +- i DIR s.
+template <int P, int DIR, int OFF, int STR, int MOD, typename T>
+__device__ __forceinline__ void bf_prime(cx<T>* v) {
+    constexpr int Hh = (P - 1) / 2;
+    auto at = [](int n) { return (OFF + STR * n) % MOD; };
+    const cx<T> x0 = v[at(0)];
+    cx<T> t[Hh], d[Hh];
 #pragma unroll
-    for (int n2 = 0; n2 < N2; ++n2) bf3<DIR, T>(v[(3 * n2) % R], v[(N2 + 3 * n2) % R], v[(2 * N2 + 3 * n2) % R]);
+    for (int j = 1; j <= Hh; ++j) {
+        t[j - 1] = v[at(j)] + v[at(P - j)];
+        d[j - 1] = v[at(j)] - v[at(P - j)];
+    }
+    cx<T> sum = x0;
 #pragma unroll
-    for (int k1 = 0; k1 < 3; ++k1) {
-        if constexpr (N2 == 2) {
-            const cx<T> a = v[(N2 * k1) % R], b = v[(N2 * k1 + 3) % R];
-            v[(N2 * k1) % R] = a + b;
-            v[(N2 * k1 + 3) % R] = a - b;
-        } else {
-            cx<T>&r0 = v[(N2 * k1) % R], &r1 = v[(N2 * k1 + 3) % R], &r2 = v[(N2 * k1 + 6) % R], &r3 = v[(N2 * k1 + 9) % R];
-            const cx<T> x0 = r0, x1 = r1, x2 = r2, x3 = r3;
-            bf4_plain<DIR, T>(x0, x1, x2, x3, r0, r1, r2, r3);
+    for (int j = 0; j < Hh; ++j) sum = sum + t[j];
+    v[at(0)] = sum;
+#pragma unroll
+    for (int k = 1; k <= Hh; ++k) {
+        cx<T> m = x0, s = mk<T>(0, 0);
+#pragma unroll
+        for (int j = 1; j <= Hh; ++j) {
+            const T co = (T)root_cos<P>(j * k), si = (T)root_sin<P>(j * k);
+            m = mk<T>(m.x + co * t[j - 1].x, m.y + co * t[j - 1].y);
+            s = mk<T>(s.x + si * d[j - 1].x, s.y + si * d[j - 1].y);
         }
+        v[at(k)] = mk<T>(m.x - (T)DIR * s.y, m.y + (T)DIR * s.x);
+        v[at(P - k)] = mk<T>(m.x + (T)DIR * s.y, m.y - (T)DIR * s.x);
     }
 }
 
-// In-place FFT of v[0..R), R in {1,2,3,4,6,8,12,16}, kernel exp(DIR 2 pi i jk/R): decimation in frequency for the powers
-// of two, prime-factor for 6 and 12.  Output X[k] is left at v[outpos<R>(k)].
+// Length R = P x Q by the prime-factor algorithm, P in {3, 5, 7}, Q in {2, 4} or another of those primes (gcd(P, Q) = 1).
+// Input index n = (Q n1 + P n2) mod R (n1 < P, n2 < Q), output index k with k = k1 mod P, k = k2 mod Q (Chinese remainder
+// theorem); everything in place, so that X[k] ends at register (Q (k mod P) + P (k mod Q)) mod R.
+template <int P, int Q, int DIR, typename T, int N2 = 0>
+__device__ __forceinline__ void fft_pfa_stage1(cx<T>* v) {
+    if constexpr (N2 < Q) {
+        bf_prime<P, DIR, (P * N2) % (P * Q), Q, P * Q, T>(v);
+        fft_pfa_stage1<P, Q, DIR, T, N2 + 1>(v);
+    }
+}
+template <int P, int Q, int DIR, typename T, int K1 = 0>
+__device__ __forceinline__ void fft_pfa_stage2(cx<T>* v) {
+    constexpr int R = P * Q;
+    if constexpr (K1 < P) {
+        if constexpr (Q == 2) {
+            const cx<T> a = v[(Q * K1) % R], b = v[(Q * K1 + P) % R];
+            v[(Q * K1) % R] = a + b;
+            v[(Q * K1 + P) % R] = a - b;
+        } else if constexpr (Q == 4) {
+            cx<T>&r0 = v[(Q * K1) % R], &r1 = v[(Q * K1 + P) % R], &r2 = v[(Q * K1 + 2 * P) % R], &r3 = v[(Q * K1 + 3 * P) % R];
+            const cx<T> x0 = r0, x1 = r1, x2 = r2, x3 = r3;
+            bf4_plain<DIR, T>(x0, x1, x2, x3, r0, r1, r2, r3);
+        } else {
+            bf_prime<Q, DIR, (Q * K1) % R, P, R, T>(v);
+        }
+        fft_pfa_stage2<P, Q, DIR, T, K1 + 1>(v);
+    }
+}
+
+// register lengths with a prime-factor decomposition P x Q (P odd prime first); 0 = none
+template <int R> struct Pfa { static constexpr int P = 0, Q = 0; };
+template <> struct Pfa<6>  { static constexpr int P = 3, Q = 2; };
+template <> struct Pfa<12> { static constexpr int P = 3, Q = 4; };
+template <> struct Pfa<10> { static constexpr int P = 5, Q = 2; };
+template <> struct Pfa<20> { static constexpr int P = 5, Q = 4; };
+template <> struct Pfa<14> { static constexpr int P = 7, Q = 2; };
+template <> struct Pfa<28> { static constexpr int P = 7, Q = 4; };
+template <> struct Pfa<15> { static constexpr int P = 3, Q = 5; };
+template <> struct Pfa<21> { static constexpr int P = 3, Q = 7; };
+
+// In-place FFT of v[0..R), kernel exp(DIR 2 pi i jk/R): decimation in frequency for R = 2^a <= 16, one butterfly for the primes
+// 3, 5, 7, prime-factor for 6, 10, 12, 14, 15, 20, 21, 28.  Output X[k] is left at v[outpos<R>(k)].
 template <int R, int DIR, typename T>
 __device__ __forceinline__ void fft_reg(cx<T>* v) {
     if constexpr (R == 16) {
         fft16_fma<DIR, T>(v);
     } else if constexpr (R == 3) {
         bf3<DIR, T>(v[0], v[1], v[2]);
-    } else if constexpr (R == 6 || R == 12) {
-        fft_pfa3<R, DIR, T>(v);
+    } else if constexpr (R == 5 || R == 7) {
+        bf_prime<R, DIR, 0, 1, R, T>(v);
+    } else if constexpr (Pfa<R>::P != 0) {
+        fft_pfa_stage1<Pfa<R>::P, Pfa<R>::Q, DIR, T>(v);
+        fft_pfa_stage2<Pfa<R>::P, Pfa<R>::Q, DIR, T>(v);
     } else if constexpr (R >= 2) {
+        static_assert((R & (R - 1)) == 0, "unsupported register length");
         DifButterflies<R, DIR, 0, T>::run(v);
         fft_reg<R / 2, DIR, T>(v);
         fft_reg<R / 2, DIR, T>(v + R / 2);
@@ -240,8 +313,8 @@ __device__ __forceinline__ void fft_reg(cx<T>* v) {
 }
 template <int R>
 __host__ __device__ __forceinline__ constexpr int outpos(int k) {
-    if constexpr (R == 3) return k;
-    else if constexpr (R == 6 || R == 12) return ((R / 3) * (k % 3) + 3 * (k % (R / 3))) % R;
+    if constexpr (R == 3 || R == 5 || R == 7) return k;
+    else if constexpr (Pfa<R>::P != 0) return (Pfa<R>::Q * (k % Pfa<R>::P) + Pfa<R>::P * (k % Pfa<R>::Q)) % R;
     else return brev<R>(k);
 }
 

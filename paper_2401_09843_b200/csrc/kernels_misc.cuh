@@ -265,12 +265,12 @@ static __global__ void sf_finalize_kernel(const double* __restrict__ marg, doubl
 // unpadded N-grid transforms for ns_set_initial / ns_get_fields / the physical-space statistics (NOT on the hot path):
 // a shared-memory FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place, n = 2^a or 3 * 2^a.
 //   axis 0: element stride n*n, axis 1: n, axis 2: 1.  dim = 2: the same on [planes][n][n] (axes 1 and 2).
-// n = 3 m: the three decimated sequences x[3r + q] are transformed by radix-2 stages (m = 2^a) and combined by one
-// radix-3 stage, X[k + m t] = sum_q w_n^{q (k + m t)} F_q[k].  Twiddles come from the table gtw[j] = exp(+2 pi i j / n).
+// n = p m, p in {3, 5, 7, 15}: the p decimated sequences x[p r + q] are transformed by radix-2 stages (m = 2^a) and combined by
+// one radix-p stage, X[k + m t] = sum_q w_n^{q (k + m t)} F_q[k].  Twiddles come from the table gtw[j] = exp(+2 pi i j / n).
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(256)
-generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis, int sign, long total_tiles,
+generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int nsub, int axis, int sign, long total_tiles,
                    const cx<T>* __restrict__ gtw, int dim) {
     constexpr int TL = 8;  // lines per tile
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -278,8 +278,7 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis
     constexpr int PITCH = TL + 1;
     const long tile = blockIdx.x;
     if (tile >= total_tiles) return;
-    const int m = 1 << log2m;          // n = m or 3 m
-    const int nsub = radix3 ? 3 : 1;
+    const int m = 1 << log2m;          // n = nsub m, nsub in {1, 3, 5, 7, 15}
     // dim = 3: cubes [n][n][n], n^2 lines per cube and axis; dim = 2: planes [n][n] (axes 1 and 2 only), n lines per plane
     const long n2 = (long)n * n;
     const long lines = dim == 3 ? n2 : n;
@@ -321,7 +320,7 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis
         }
         __syncthreads();
     }
-    if (radix3) {
+    if (nsub == 3) {
         const T h = (T)sign * (T)0.86602540378443864676L;
         for (int e = threadIdx.x; e < m * TL; e += blockDim.x) {
             const int c = e % TL, k = e / TL;
@@ -333,6 +332,19 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int radix3, int axis
             S[k * PITCH + c] = f0 + sm;
             S[(m + k) * PITCH + c] = mk<T>(mm.x - h * d.y, mm.y + h * d.x);
             S[(2 * m + k) * PITCH + c] = mk<T>(mm.x + h * d.y, mm.y - h * d.x);
+        }
+        __syncthreads();
+    } else if (nsub > 1) {
+        // odd factor 5, 7 or 15: the plain nsub-point combine, X[k + m t] = sum_q w_n^{qk} F_q[k] w_nsub^{qt}
+        for (int e = threadIdx.x; e < m * TL; e += blockDim.x) {
+            const int c = e % TL, k = e / TL;
+            cx<T> f[15];
+            for (int q = 0; q < nsub; ++q) f[q] = q == 0 ? S[k * PITCH + c] : cmul(S[(q * m + k) * PITCH + c], root((q * k) % n));
+            for (int t = 0; t < nsub; ++t) {
+                cx<T> acc = f[0];
+                for (int q = 1; q < nsub; ++q) acc = acc + cmul(f[q], root(((q * t) % nsub) * m));
+                S[(t * m + k) * PITCH + c] = acc;
+            }
         }
         __syncthreads();
     }

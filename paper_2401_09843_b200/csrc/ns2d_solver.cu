@@ -324,7 +324,7 @@ public:
         if (smem > 48 * 1024)
             NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         for (int axis = 1; axis < 3; ++axis) {
-            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2n, 0, axis, sign, tiles, tw().gN, 2);
+            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2n, 1, axis, sign, tiles, tw().gN, 2);
             NS_LAUNCHED("generic_fft 2d");
         }
         return NS_OK;

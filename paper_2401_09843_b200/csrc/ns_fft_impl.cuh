@@ -25,6 +25,16 @@ template <> struct Split<24>  { static constexpr int R1 = 6,  R2 = 4;  };
 template <> struct Split<48>  { static constexpr int R1 = 12, R2 = 4;  };
 template <> struct Split<96>  { static constexpr int R1 = 12, R2 = 8;  };
 template <> struct Split<192> { static constexpr int R1 = 12, R2 = 16; };
+// N = 5 * 2^a, 7 * 2^a, 15 * 2^a (radix-5 / radix-7 butterflies, prime-factor first stages 10, 14, 15, 20)
+template <> struct Split<40>  { static constexpr int R1 = 10, R2 = 4;  };
+template <> struct Split<80>  { static constexpr int R1 = 10, R2 = 8;  };
+template <> struct Split<160> { static constexpr int R1 = 10, R2 = 16; };
+template <> struct Split<320> { static constexpr int R1 = 20, R2 = 16; };
+template <> struct Split<56>  { static constexpr int R1 = 14, R2 = 4;  };
+template <> struct Split<112> { static constexpr int R1 = 14, R2 = 8;  };
+template <> struct Split<224> { static constexpr int R1 = 14, R2 = 16; };
+template <> struct Split<120> { static constexpr int R1 = 15, R2 = 8;  };
+template <> struct Split<240> { static constexpr int R1 = 15, R2 = 16; };
 
 template <int L> struct Cfg {
     static constexpr int R1 = Split<L>::R1, R2 = Split<L>::R2;
@@ -35,7 +45,10 @@ template <int L> struct Cfg {
         return tt >= 128 ? 1 : 128 / tt;
     }
     // lines per block of the block-synchronous fused z kernel (must divide M^2): about 96-192 threads
-    static constexpr int lpbf() { return L == 24 ? 8 : (L % 3 == 0 ? (L >= 192 ? 2 : 4) : 192 / (3 * P)); }
+    static constexpr int lpbf() {
+        if (L % 5 == 0 || L % 7 == 0) return P <= 8 ? 8 : (P <= 14 ? 4 : 2);
+        return L == 24 ? 8 : (L % 3 == 0 ? (L >= 192 ? 2 : 4) : 192 / (3 * P));
+    }
     // target CTAs per SM of the fused z kernel (bounds its registers)
     static constexpr int minbf() { return 2; }
 };
@@ -167,12 +180,32 @@ static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>
     return cudaGetLastError();
 }
 
+// Two kernel families, compiled in separate translation units (ns_fft_*.cu define NS_FAMILY_SMOOTH or not):
+//   pow2    L = 2^a, 8..256: column kernels (+ tensor-memory variants), line-pair z kernel for L >= 64, y2d kernel
+//   smooth  L = 3, 5, 7 or 15 times 2^a: column kernels + block-synchronous z kernel
+#ifdef NS_FAMILY_SMOOTH
+#define NS_FAM(x) x##_smooth
 #define NS_DISPATCH_L(L, CALL)                                   \
     switch (L) {                                                 \
         case 24: return CALL(24);                                \
         case 48: return CALL(48);                                \
         case 96: return CALL(96);                                \
         case 192: return CALL(192);                              \
+        case 40: return CALL(40);                                \
+        case 80: return CALL(80);                                \
+        case 160: return CALL(160);                              \
+        case 320: return CALL(320);                              \
+        case 56: return CALL(56);                                \
+        case 112: return CALL(112);                              \
+        case 224: return CALL(224);                              \
+        case 120: return CALL(120);                              \
+        case 240: return CALL(240);                              \
+        default: return cudaErrorInvalidValue;                   \
+    }
+#else
+#define NS_FAM(x) x##_pow2
+#define NS_DISPATCH_L(L, CALL)                                   \
+    switch (L) {                                                 \
         case 8: return CALL(8);                                  \
         case 16: return CALL(16);                                \
         case 32: return CALL(32);                                \
@@ -181,6 +214,7 @@ static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>
         case 256: return CALL(256);                              \
         default: return cudaErrorInvalidValue;                   \
     }
+#endif
 
 // L2 prefetch distance of the column passes in tiles (kernels_col.cuh): the CTAs resident on the GPU (2-3 per SM)
 static int col_pf_dist(int num_sms, int L) {
@@ -213,34 +247,44 @@ static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride
 }
 
 template <typename T>
-cudaError_t launch_col_inv(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+cudaError_t NS_FAM(launch_col_inv)(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
     // measured (profiles/): parking pays at L = 128 (0.264 -> 0.216 ms at 256^3); at L = 256 the register kernel is faster
     const bool pf = col_pf_on(false, L, istride * (long)sizeof(cx<T>));
+#ifndef NS_FAMILY_SMOOTH
     if (L == 128) return pf ? col_inv_tmem_L<T, 128, true>(st, in, out, g, tw) : col_inv_tmem_L<T, 128, false>(st, in, out, g, tw);
+#endif
 #define CALL(LL) (pf ? col_inv_L<T, LL, true>(st, in, out, g, tw) : col_inv_L<T, LL, false>(st, in, out, g, tw))
     NS_DISPATCH_L(L, CALL)
 #undef CALL
 }
 
 template <typename T>
-cudaError_t launch_col_fwd(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+cudaError_t NS_FAM(launch_col_fwd)(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
                            long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
     const bool pf = col_pf_on(true, L, istride * (long)sizeof(cx<T>));
+#ifndef NS_FAMILY_SMOOTH
     if (L == 128) return pf ? col_fwd_tmem_L<T, 128, true>(st, in, out, g, scale, tw) : col_fwd_tmem_L<T, 128, false>(st, in, out, g, scale, tw);
     if (L == 256) return pf ? col_fwd_tmem_L<T, 256, true>(st, in, out, g, scale, tw) : col_fwd_tmem_L<T, 256, false>(st, in, out, g, scale, tw);
+#endif
 #define CALL(LL) (pf ? col_fwd_L<T, LL, true>(st, in, out, g, scale, tw) : col_fwd_L<T, LL, false>(st, in, out, g, scale, tw))
     NS_DISPATCH_L(L, CALL)
 #undef CALL
 }
 
 template <typename T>
-cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
-                           unsigned long long* umax2, Twiddles<T> tw) {
+cudaError_t NS_FAM(launch_z_fused)(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
+                                   unsigned long long* umax2, Twiddles<T> tw) {
+#ifdef NS_FAMILY_SMOOTH
+    // N = 3, 5, 7, 15 times 2^a: the block-synchronous kernel with a prime-factor first stage
+#define CALL(LL) z_fused_L<T, LL>(st, num_sms, in, out, MM, batch, umax2, tw)
+    NS_DISPATCH_L(L, CALL)
+#undef CALL
+#else
     switch (L) {
         case 256: return z_pair_L<T, 256>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 128: return z_pair_L<T, 128>(st, num_sms, in, out, MM, batch, umax2, tw);
@@ -254,15 +298,12 @@ cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in,
         case 8: return z_fused_L<T, 8>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 16: return z_fused_L<T, 16>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 32: return z_fused_L<T, 32>(st, num_sms, in, out, MM, batch, umax2, tw);
-        // N = 3 * 2^a: the same kernel with a radix-6 / radix-12 first stage
-        case 24: return z_fused_L<T, 24>(st, num_sms, in, out, MM, batch, umax2, tw);
-        case 48: return z_fused_L<T, 48>(st, num_sms, in, out, MM, batch, umax2, tw);
-        case 96: return z_fused_L<T, 96>(st, num_sms, in, out, MM, batch, umax2, tw);
-        case 192: return z_fused_L<T, 192>(st, num_sms, in, out, MM, batch, umax2, tw);
         default: return cudaErrorInvalidValue;
     }
+#endif
 }
 
+#ifndef NS_FAMILY_SMOOTH
 template <typename T, int L>
 static cudaError_t y2d_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long M, long batch, unsigned long long* umax2,
                          Twiddles<T> tw) {
@@ -292,14 +333,43 @@ cudaError_t launch_y2d(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<
     }
 }
 
-#define NS_INSTANTIATE_FFT(T)                                                                                      \
-    template cudaError_t launch_col_inv<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
-                                           long, Twiddles<T>);                                                     \
-    template cudaError_t launch_col_fwd<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long,  \
-                                           long, T, Twiddles<T>);                                                  \
-    template cudaError_t launch_z_fused<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*, \
-                                           Twiddles<T>);                                                           \
-    template cudaError_t launch_y2d<T>(cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*,     \
-                                       Twiddles<T>);
+// the public launchers route by family (defined once, in the pow2 translation unit)
+template <typename T>
+cudaError_t launch_col_inv(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
+    if ((L & (L - 1)) == 0) return launch_col_inv_pow2<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, tw);
+    return launch_col_inv_smooth<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, tw);
+}
+template <typename T>
+cudaError_t launch_col_fwd(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
+                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
+    if ((L & (L - 1)) == 0) return launch_col_fwd_pow2<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, scale, tw);
+    return launch_col_fwd_smooth<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, scale, tw);
+}
+template <typename T>
+cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
+                           unsigned long long* umax2, Twiddles<T> tw) {
+    if ((L & (L - 1)) == 0) return launch_z_fused_pow2<T>(st, num_sms, L, in, out, MM, batch, umax2, tw);
+    return launch_z_fused_smooth<T>(st, num_sms, L, in, out, MM, batch, umax2, tw);
+}
+#endif  // !NS_FAMILY_SMOOTH
+
+#define NS_FFT_ARGS_COL(T) cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, long, long, long, long
+#define NS_FFT_ARGS_Z(T) cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*, Twiddles<T>
+#ifdef NS_FAMILY_SMOOTH
+#define NS_INSTANTIATE_FFT(T)                                                                   \
+    template cudaError_t launch_col_inv_smooth<T>(NS_FFT_ARGS_COL(T), Twiddles<T>);             \
+    template cudaError_t launch_col_fwd_smooth<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>);          \
+    template cudaError_t launch_z_fused_smooth<T>(NS_FFT_ARGS_Z(T));
+#else
+#define NS_INSTANTIATE_FFT(T)                                                                   \
+    template cudaError_t launch_col_inv_pow2<T>(NS_FFT_ARGS_COL(T), Twiddles<T>);               \
+    template cudaError_t launch_col_fwd_pow2<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>);            \
+    template cudaError_t launch_z_fused_pow2<T>(NS_FFT_ARGS_Z(T));                              \
+    template cudaError_t launch_col_inv<T>(NS_FFT_ARGS_COL(T), Twiddles<T>);                    \
+    template cudaError_t launch_col_fwd<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>);                 \
+    template cudaError_t launch_z_fused<T>(NS_FFT_ARGS_Z(T));                                   \
+    template cudaError_t launch_y2d<T>(NS_FFT_ARGS_Z(T));
+#endif
 
 }  // namespace ns

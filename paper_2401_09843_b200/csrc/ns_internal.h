@@ -56,6 +56,21 @@ template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
                            unsigned long long* umax2, Twiddles<T> tw);
 
+// the same three launchers per kernel family (ns_fft_impl.cuh): L = 2^a / L = 3, 5, 7, 15 times 2^a
+#define NS_DECL_FAMILY(FAM)                                                                                                        \
+    template <typename T>                                                                                                          \
+    cudaError_t launch_col_inv_##FAM(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,    \
+                                     long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw);                     \
+    template <typename T>                                                                                                          \
+    cudaError_t launch_col_fwd_##FAM(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,    \
+                                     long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw);            \
+    template <typename T>                                                                                                          \
+    cudaError_t launch_z_fused_##FAM(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,        \
+                                     unsigned long long* umax2, Twiddles<T> tw);
+NS_DECL_FAMILY(pow2)
+NS_DECL_FAMILY(smooth)
+#undef NS_DECL_FAMILY
+
 // factor carried by the output of launch_z_fused / launch_y2d relative to the plain unnormalised transform (the kernels of
 // kernels_zpair.cuh fold the 1/2 of their Hermitian split into the normalisation of the spectral kernel)
 int z_fused_output_scale(int L);

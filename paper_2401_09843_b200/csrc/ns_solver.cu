@@ -410,8 +410,8 @@ public:
     }
 
     int generic_fft3(cx<T>* W, long cubes, int sign) {
-        const int radix3 = N % 3 == 0 ? 1 : 0;
-        const int m = radix3 ? N / 3 : N;
+        const int radix3 = N % 15 == 0 ? 15 : (N % 3 == 0 ? 3 : (N % 5 == 0 ? 5 : (N % 7 == 0 ? 7 : 1)));   // odd factor of N
+        const int m = N / radix3;
         int log2m = 0;
         while ((1 << log2m) < m) ++log2m;
         const long tiles = cubes * (long)N * N / 8;
@@ -597,11 +597,11 @@ int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dt
     g_create_error.clear();
     if (!out) { g_create_error = "out is NULL"; return NS_ERR_INVALID_ARG; }
     *out = nullptr;
-    // N = 2^a or 3 * 2^a (sizes with small prime factors); a column tile is 128 bytes = 8 (fp64) / 16 (fp32)
-    // complex values of the N/2 stored kz entries
+    // N = p 2^a with p in {1, 3, 5, 7, 15} (sizes with small prime factors); a column tile is 128 bytes = 8 (fp64) /
+    // 16 (fp32) complex values of the N/2 stored kz entries
     const int tile = dtype == NS_F32 ? 16 : 8;
-    if (N < 16 || N > 512 || (N % 2) != 0 || !fft_supported(N / 2) || (N / 2) % tile != 0) {
-        g_create_error = "N must be 2^a or 3 * 2^a with 16 <= N <= 512 (fp32: N/2 a multiple of 16, i.e. N >= 32 and N != 48)";
+    if (N < 16 || N > 640 || (N % 2) != 0 || !fft_supported(N / 2) || (N / 2) % tile != 0) {
+        g_create_error = "N must be p * 2^a with p in {1, 3, 5, 7, 15}, 16 <= N <= 640 and N/2 a multiple of 8 (fp32: of 16)";
         return NS_ERR_INVALID_ARG;
     }
     if (batch < 1) { g_create_error = "batch must be >= 1"; return NS_ERR_INVALID_ARG; }
