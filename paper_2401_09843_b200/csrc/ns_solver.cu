@@ -36,6 +36,7 @@ struct ns_solver {
     virtual int ensemble_moments(void* mean, void* var, ns_memspace ms) = 0;
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
+    virtual int set_pipeline(int groups, int z_sms) = 0;
     virtual int profile(int enable) = 0;
     virtual int profile_read(double* ms, long long* cnt) = 0;
 };
@@ -131,10 +132,22 @@ public:
     size_t nS, nX, nY, nZ;  // complex element counts of state, X, Y, Z
     size_t red_count;
     PassProfiler prof;
+    // two-stream software pipeline over groups of samples (ns_set_pipeline): the fused z kernel (fp64-issue / shared-memory
+    // bound, DRAM a third busy) of one group runs on its own high-priority stream and a subset of the SMs while the column and
+    // spectral passes (DRAM bound, fp64 a third busy) of the other groups run on the solver's stream on the remaining SMs.
+    static constexpr int MAX_GROUPS = 16;
+    int groups = 1, z_sms = 0;
+    cudaStream_t st_z = nullptr;
+    cudaEvent_t ev_inv[MAX_GROUPS] = {}, ev_z[MAX_GROUPS] = {};
 
     Solver(int N_, int batch_, const ns_params& p, cudaStream_t s) : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), prm(p), st(s) {}
     ~Solver() override {
         if (arena) cudaFree(arena);
+        if (st_z) cudaStreamDestroy(st_z);
+        for (int g = 0; g < MAX_GROUPS; ++g) {
+            if (ev_inv[g]) cudaEventDestroy(ev_inv[g]);
+            if (ev_z[g]) cudaEventDestroy(ev_z[g]);
+        }
     }
 
     int fail(int code, const std::string& msg) {
@@ -168,6 +181,24 @@ public:
                 snprintf(buf, sizeof buf, "sample %d: the velocity field is not finite (NaN or inf); the sample is frozen", b);
                 return fail(NS_ERR_NONFINITE, buf);
             }
+        return NS_OK;
+    }
+
+    int set_pipeline(int groups_, int z_sms_) override {
+        if (groups_ < 1 || groups_ > MAX_GROUPS || batch % groups_ != 0) return fail(NS_ERR_INVALID_ARG, "groups must divide batch (1..16)");
+        if (z_sms_ < 0 || z_sms_ > num_sms) return fail(NS_ERR_INVALID_ARG, "z_sms must be in [0, SM count]");
+        NS_CK(cudaStreamSynchronize(st));
+        if (groups_ > 1 && !st_z) {
+            int lo = 0, hi = 0;
+            NS_CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            NS_CK(cudaStreamCreateWithPriority(&st_z, cudaStreamNonBlocking, hi));
+        }
+        for (int g = 0; g < groups_; ++g) {
+            if (!ev_inv[g]) NS_CK(cudaEventCreateWithFlags(&ev_inv[g], cudaEventDisableTiming));
+            if (!ev_z[g]) NS_CK(cudaEventCreateWithFlags(&ev_z[g], cudaEventDisableTiming));
+        }
+        groups = groups_;
+        z_sms = z_sms_ == 0 ? num_sms : z_sms_;
         return NS_OK;
     }
 
@@ -237,43 +268,98 @@ public:
     long long device_bytes() const override { return (long long)arena_bytes; }
 
     // ---------------------------------------------------------------- RHS transform pipeline a1..a6
-    // Uin (internal layout) -> Y = Th [b][5][N][N][H] (unnormalised transforms of the trace-free flux)
-    int transform(const cx<T>* Uin, bool want_umax, int upto = 6) {
+    // Every pass works on the samples [b0, b0 + nb) of the batch; workspaces are indexed by sample, so groups of samples use
+    // disjoint ranges of X / Y / Z within a pass.  X holds 3 (a1 out) or 5 (a5 out) components per sample and Y 3 padded
+    // (a2 out) or 5 truncated (a6 out): a forward pass of one group may overwrite the inverse-pass output of ANOTHER group
+    // (a5 of group g touches the a1 range of groups h > g), which is why stage_transform queues the inverse passes of all
+    // groups before the first forward pass.
+    int pass_inverse(const cx<T>* Uin, int b0, int nb) {
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
         prof.tick(0, st);
-        e = launch_col_inv<T>(st, num_sms, L, Uin, X, NH, (long)batch * 3, NH, NH, (long)N * NH, (long)M * NH, tw());
+        e = launch_col_inv<T>(st, num_sms, L, Uin + (size_t)b0 * 3 * N * NH, X + (size_t)b0 * 3 * M * NH, NH, (long)nb * 3, NH, NH,
+                              (long)N * NH, (long)M * NH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a1 col_inv x");
         ++launches;
         prof.tick(1, st);
-        e = launch_col_inv<T>(st, num_sms, L, X, Y, H, (long)batch * 3 * M, H, H, NH, MH, tw());
+        e = launch_col_inv<T>(st, num_sms, L, X + (size_t)b0 * 3 * M * NH, Y + (size_t)b0 * 3 * M * MH, H, (long)nb * 3 * M, H, H, NH, MH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
         ++launches;
-        prof.tick(2, st);
-        e = launch_z_fused<T>(st, num_sms, L, Y, Z, (long)M * M, batch, want_umax ? umax2 : nullptr, tw());
+        return NS_OK;
+    }
+    int pass_z(cudaStream_t s, int sms, int b0, int nb, bool want_umax) {
+        const long MH = (long)M * H;
+        prof.tick(2, s);
+        cudaError_t e = launch_z_fused<T>(s, sms, L, Y + (size_t)b0 * 3 * M * MH, Z + (size_t)b0 * NS_NFLUX * M * MH, (long)M * M, nb,
+                                          want_umax ? umax2 + b0 : nullptr, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a3+a4 z_fused");
         ++launches;
-        if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
+        return NS_OK;
+    }
+    int pass_forward(int b0, int nb) {
+        const long NH = (long)N * H, MH = (long)M * H;
+        cudaError_t e;
         prof.tick(4, st);
-        e = launch_col_fwd<T>(st, num_sms, L, Z, X, H, (long)batch * NS_NFLUX * M, H, H, MH, NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, num_sms, L, Z + (size_t)b0 * NS_NFLUX * M * MH, X + (size_t)b0 * NS_NFLUX * M * NH, H,
+                              (long)nb * NS_NFLUX * M, H, H, MH, NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a5 col_fwd y");
         ++launches;
         prof.tick(5, st);
-        e = launch_col_fwd<T>(st, num_sms, L, X, Y, NH, (long)batch * NS_NFLUX, NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, num_sms, L, X + (size_t)b0 * NS_NFLUX * M * NH, Y + (size_t)b0 * NS_NFLUX * N * NH, NH, (long)nb * NS_NFLUX,
+                              NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a6 col_fwd x");
         ++launches;
         prof.tick(7, st);
         return NS_OK;
     }
 
-    int spectral(const cx<T>* Us, const cx<T>* Un, cx<T>* out, double alpha, double beta, double gamma, int mode) {
-        const long total = (long)batch * N * N * H;
+    // Uin (internal layout) -> Y = Th [b][5][N][N][H] (unnormalised transforms of the trace-free flux), all samples, one stream
+    int transform(const cx<T>* Uin, bool want_umax, int upto = 6) {
+        int rc;
+        if ((rc = pass_inverse(Uin, 0, batch)) != NS_OK) return rc;
+        if ((rc = pass_z(st, num_sms, 0, batch, want_umax)) != NS_OK) return rc;
+        if (upto <= 3) { prof.tick(-1, st); return NS_OK; }
+        return pass_forward(0, batch);
+    }
+
+    int spectral(const cx<T>* Us, const cx<T>* Un, cx<T>* out, double alpha, double beta, double gamma, int mode, int b0 = 0, int nb = -1) {
+        if (nb < 0) nb = batch;
+        const long plane = (long)N * N * H, total = (long)nb * plane;
         const T scale = (T)(1.0 / ((double)M * M * M * z_fused_output_scale(L)));
         prof.tick(6, st);
-        spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y, Us, Un, out, N, total, dtab, scale, (T)alpha, (T)beta,
-                                                                    (T)gamma, dt_dev, mode);
+        spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y + (size_t)b0 * NS_NFLUX * plane, Us + (size_t)b0 * 3 * plane,
+                                                                    Un ? Un + (size_t)b0 * 3 * plane : nullptr, out + (size_t)b0 * 3 * plane, N,
+                                                                    total, dtab, scale, (T)alpha, (T)beta, (T)gamma, dt_dev + b0, mode);
         NS_LAUNCHED("a7 spectral_kernel");
         prof.tick(-1, st);
+        return NS_OK;
+    }
+
+    // One RK stage = transform + tail (time-step bookkeeping in stage 1, then a7).  With groups > 1 (ns_set_pipeline) and the
+    // per-pass profiler off, the samples are processed in `groups` groups: the inverse passes of all groups are queued on the
+    // solver's stream, each followed by an event that releases the group's z kernel on the z stream (grid limited to z_sms
+    // SMs); the forward passes and the tail of a group wait for its z kernel.  Every kernel sees exactly the data it sees
+    // in the single-stream order, so the result is bit-identical.
+    template <typename Tail>
+    int stage(const cx<T>* Uin, bool want_umax, Tail tail) {
+        int rc;
+        if (groups <= 1 || prof.on) {
+            if ((rc = transform(Uin, want_umax)) != NS_OK) return rc;
+            return tail(0, batch);
+        }
+        const int nb = batch / groups;
+        for (int g = 0; g < groups; ++g) {
+            if ((rc = pass_inverse(Uin, g * nb, nb)) != NS_OK) return rc;
+            NS_CK(cudaEventRecord(ev_inv[g], st));
+            NS_CK(cudaStreamWaitEvent(st_z, ev_inv[g], 0));
+            if ((rc = pass_z(st_z, z_sms, g * nb, nb, want_umax)) != NS_OK) return rc;
+            NS_CK(cudaEventRecord(ev_z[g], st_z));
+        }
+        for (int g = 0; g < groups; ++g) {
+            NS_CK(cudaStreamWaitEvent(st, ev_z[g], 0));
+            if ((rc = pass_forward(g * nb, nb)) != NS_OK) return rc;
+            if ((rc = tail(g * nb, nb)) != NS_OK) return rc;
+        }
         return NS_OK;
     }
 
@@ -282,30 +368,31 @@ public:
     int rk3(DtMode mode, double dt, const double* dts_host, double cfl, double t_end) {
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
         int rc;
-        const unsigned gb = blocks_for(batch, 128);
         // max|u|^2 is a free by-product of a3 in stage 1; besides the CFL step it is what detects a non-finite state
         NS_CK(cudaMemsetAsync(umax2, 0, (size_t)batch * sizeof(unsigned long long), st));
-        if ((rc = transform(U, true)) != NS_OK) return rc;
-        if (mode == DT_UNIFORM) {
-            set_dt_uniform_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, dt, umax2, bad_dev, batch);
-            NS_LAUNCHED("set_dt_uniform");
-        } else if (mode == DT_ARRAY) {
-            NS_CK(cudaMemcpyAsync(scal_dev, dts_host, (size_t)batch * sizeof(double), cudaMemcpyHostToDevice, st));
-            set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, scal_dev, umax2, bad_dev, batch);
-            NS_LAUNCHED("set_dt_array");
-        } else {
-            cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, umax2, bad_dev, cfl, 2.0 * 3.14159265358979323846 / N, t_end, batch);
-            NS_LAUNCHED("cfl_finalize");
-        }
+        if (mode == DT_ARRAY) NS_CK(cudaMemcpyAsync(scal_dev, dts_host, (size_t)batch * sizeof(double), cudaMemcpyHostToDevice, st));
         // eq. (2.6): u1 = u + dt R(u)
-        if ((rc = spectral(U, nullptr, V, 0.0, 1.0, 1.0, 1)) != NS_OK) return rc;
+        rc = stage(U, true, [&](int b0, int nb) -> int {
+            const unsigned gb = blocks_for(nb, 128);
+            if (mode == DT_UNIFORM) {
+                set_dt_uniform_kernel<<<gb, 128, 0, st>>>(dt_dev + b0, t_dev + b0, dt, umax2 + b0, bad_dev + b0, nb);
+                NS_LAUNCHED("set_dt_uniform");
+            } else if (mode == DT_ARRAY) {
+                set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev + b0, t_dev + b0, scal_dev + b0, umax2 + b0, bad_dev + b0, nb);
+                NS_LAUNCHED("set_dt_array");
+            } else {
+                cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev + b0, t_dev + b0, umax2 + b0, bad_dev + b0, cfl, 2.0 * 3.14159265358979323846 / N,
+                                                        t_end, nb);
+                NS_LAUNCHED("cfl_finalize");
+            }
+            return spectral(U, nullptr, V, 0.0, 1.0, 1.0, 1, b0, nb);
+        });
+        if (rc != NS_OK) return rc;
         // u2 = 3/4 u + 1/4 u1 + 1/4 dt R(u1)
-        if ((rc = transform(V, false)) != NS_OK) return rc;
-        if ((rc = spectral(V, U, V, 0.75, 0.25, 0.25, 1)) != NS_OK) return rc;
+        rc = stage(V, false, [&](int b0, int nb) -> int { return spectral(V, U, V, 0.75, 0.25, 0.25, 1, b0, nb); });
+        if (rc != NS_OK) return rc;
         // u+ = 1/3 u + 2/3 u2 + 2/3 dt R(u2)
-        if ((rc = transform(V, false)) != NS_OK) return rc;
-        if ((rc = spectral(V, U, U, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 1)) != NS_OK) return rc;
-        return NS_OK;
+        return stage(V, false, [&](int b0, int nb) -> int { return spectral(V, U, U, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 1, b0, nb); });
     }
 
     int step_uniform(double dt) override {
@@ -654,6 +741,7 @@ double ns_time(const ns_solver* h, int sample) {
     if (!h) return std::numeric_limits<double>::quiet_NaN();
     return const_cast<ns_solver*>(h)->time(sample);
 }
+int ns_set_pipeline(ns_solver* h, int groups, int z_sms) { NS_H(h); return h->set_pipeline(groups, z_sms); }
 int ns_profile(ns_solver* h, int enable) { NS_H(h); return h->profile(enable); }
 int ns_profile_read(ns_solver* h, double* ms, long long* cnt) { NS_H(h); return h->profile_read(ms, cnt); }
 long long ns_kernel_launches(const ns_solver* h) { return h ? h->launches : 0; }

@@ -94,7 +94,7 @@ def test_product_does_not_import_oracle():
 
 def test_sass_is_blackwell_native():
     """The built library carries the sm_100a paths the design names (B200_PROFILING.md 'What proves a Blackwell-native
-    kernel'): TMA bulk copies (UBLKCP) in every fused z kernel, tensor-memory parking (STTM / LDTM after a
+    kernel'): TMA bulk copies (UBLKCP) in every fused z kernel, tensor-map TMA loads (UTMALDG) in the persistent column kernel, tensor-memory parking (STTM / LDTM after a
     tcgen05.alloc) in the long-line kernels, and no cuFFT / cuBLAS dependency.  Static check with cuobjdump / ldd."""
     import shutil
     import subprocess
@@ -110,12 +110,15 @@ def test_sass_is_blackwell_native():
             name = line.split("Function :")[1].strip()
             per_fn[name] = set()
         elif name is not None:
-            for m in ("UBLKCP", "LDTM", "STTM", "UTCATOMSWS", "DFMA"):
+            for m in ("UBLKCP", "UTMALDG", "LDTM", "STTM", "UTCATOMSWS", "DFMA"):
                 if m in line:
                     per_fn[name].add(m)
     z = {k: v for k, v in per_fn.items() if "z_fused" in k or "z_pair" in k or "y2d_kernel" in k}
     assert len(z) >= 12 and all("UBLKCP" in v for v in z.values())
     tm = {k: v for k, v in per_fn.items() if "z_pair" in k or "y2d_kernel" in k or "_tmem_kernel" in k}
     assert len(tm) >= 12 and all({"LDTM", "STTM", "UTCATOMSWS"} <= v for v in tm.values())
+    # the persistent forward column kernel: tensor-map TMA loads (cp.async.bulk.tensor) and twiddles in tensor memory
+    ring = {k: v for k, v in per_fn.items() if "col_fwd_ring_kernel" in k}
+    assert len(ring) >= 1 and all({"UTMALDG", "LDTM", "STTM"} <= v for v in ring.values())
     ldd = subprocess.run(["ldd", binding.LIB_PATH], capture_output=True, text=True).stdout
     assert "cufft" not in ldd.lower() and "cublas" not in ldd.lower()
