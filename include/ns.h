@@ -15,7 +15,13 @@
  * listed in DESIGN.md section 3 (A1..A20).
  *
  * Conventions
- *   N         grid points per axis, a power of two, 16 <= N <= 512 (fp32: 32 <= N).  Padded grid M = 3N/2.
+ *   N         grid points per axis: any even N, 16 <= N <= 640.  The transforms run on a TRANSFORM GRID Nt >= N of the form
+ *             p 2^a, p in {1, 3, 5, 7, 15}, Nt/2 a multiple of 8 (fp32: 16), with the padded grid M = 3 Nt / 2 >= 3N/2 -- the
+ *             paper's "round the padded size up to the next 2^a 3^b 5^c 7^d"; Nt = N whenever N has that form
+ *             (all BASELINE.json sizes), else the next such size or the one ns_autotune measured.  The state is truncated to
+ *             the user's N (P_N of eq. 2.1) and all public arrays have the user's N; results do not depend on Nt beyond
+ *             round-off, except max|u| (ns_max_velocity, the CFL step), which is a maximum over the M^3 points of the
+ *             padded grid in use (ns_padded_size).
  *   spectral  complex interleaved (re,im) of `dtype`, shape [batch][3][N][N][N/2+1], index
  *             [b][component][ikx][iky][ikz], ikz fastest (r2c half spectrum, kz >= 0).
  *             Stored index i <-> wavenumber k = i (i < N/2) or i - N (i > N/2).  Coefficients are
@@ -76,11 +82,23 @@ typedef struct {
 } ns_params;
 
 /* Create a solver for `batch` independent samples on an N^3 grid.  `p` may be NULL (inviscid).
- * Allocates one device arena of about 15.7 * batch * N^3 * sizeof(complex) bytes (state, stage
+ * Allocates one device arena of about 15.7 * batch * Nt^3 * sizeof(complex) bytes (Nt = the transform grid; state, stage
  * state and three workspaces aliased across the passes, cf. "Workspaces", PAPER.md:L207-213;
  * ns_device_bytes returns the exact figure).
  * cuda_stream: a cudaStream_t cast to void* (NULL = default stream). */
 int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream);
+
+/* Transform-grid benchmark of PAPER.md:L175 ("On any new system, we therefore once run a benchmark of only the Fourier transform
+ * storing its results and extracting the optimal padding size ... If no suitable size is found in the benchmark results, we choose
+ * the next larger N with prime factors at most 7 instead"): times the transform passes a1..a6 of one sample on the first `ncand`
+ * (1..16) admissible transform grids Nt >= N of the current device and records the fastest in a process-wide table keyed by
+ * (device, N, dtype), which later ns_create calls for that N use; without an entry ns_create takes the first admissible Nt.
+ * grids_out[ncand], ms_out[ncand] (host, may be NULL): the candidates and their milliseconds per pass sequence (0 past the
+ * last candidate that exists or fits in memory); *best_out (may be NULL): the grid recorded.  Synchronous; thread safe. */
+int ns_autotune(int N, ns_dtype dtype, int ncand, int* grids_out, double* ms_out, int* best_out);
+/* The transform grid Nt and the padded grid M = 3 Nt / 2 of a handle (0 for NULL). */
+int ns_transform_grid(const ns_solver* h);
+int ns_padded_size(const ns_solver* h);
 int ns_destroy(ns_solver* h);
 
 /* Set the state from PHYSICAL samples u_phys [batch][3][N][N][N] (eq. 2.1 third line,
@@ -114,7 +132,7 @@ int ns_step_dts(ns_solver* h, const double* dt);
  * NS_ERR_INVALID_ARG for cfl <= 0 or max_steps < 0. */
 int ns_advance(ns_solver* h, double cfl, double t_end, int max_steps, int* steps_done);
 
-/* umax_out[batch] (host): max over the padded M^3 grid of the Euclidean |u| of the current state. */
+/* umax_out[batch] (host): max over the padded M^3 grid (M = ns_padded_size(h)) of the Euclidean |u| of the current state. */
 int ns_max_velocity(ns_solver* h, double* umax_out);
 /* Physical velocity on the N grid, [batch][3][N][N][N] (the "whole flow field" writer). */
 int ns_get_fields(ns_solver* h, void* u_phys_out, ns_memspace ms);

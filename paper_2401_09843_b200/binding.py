@@ -22,7 +22,7 @@ NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE, NS_ERR_NONFINI
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
     "ns_step_cfl", "ns_step_dts", "ns_advance", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
-    "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_set_pipeline", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
+    "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_set_pipeline", "ns_autotune", "ns_transform_grid", "ns_padded_size", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
 # include/ns2d.h: the two-dimensional solver
 EXPORTS_2D = [
@@ -73,6 +73,9 @@ def lib():
         L.ns_structure_function_p.argtypes = [vp, d, vp, i]
         L.ns_ensemble_moments.argtypes = [vp, vp, vp, i]
         L.ns_set_pipeline.argtypes = [vp, i, i]
+        L.ns_autotune.argtypes = [i, i, i, vp, vp, ctypes.POINTER(ctypes.c_int)]
+        L.ns_transform_grid.argtypes = [vp]
+        L.ns_padded_size.argtypes = [vp]
         L.ns_profile.argtypes = [vp, i]
         L.ns_profile_read.argtypes = [vp, vp, vp]
         L.ns_time.argtypes = [vp, i]
@@ -127,6 +130,19 @@ def _buf(x, writable=False):
             raise ValueError("output host buffer must be a C-contiguous numpy array")
         a = np.ascontiguousarray(a)
     return ctypes.c_void_p(a.ctypes.data), NS_HOST, a
+
+
+def autotune(N, dtype="f64", ncand=3):
+    """ns_autotune: time the transform passes on the first `ncand` admissible transform grids >= N, record the fastest for later
+    Solver(N, ...) calls in this process.  Returns (best grid, [(grid, ms), ...])."""
+    dt = {"f64": NS_F64, "f32": NS_F32, NS_F64: NS_F64, NS_F32: NS_F32}[dtype]
+    grids = np.zeros(ncand, dtype=np.int32)
+    ms = np.zeros(ncand, dtype=np.float64)
+    best = ctypes.c_int(0)
+    rc = lib().ns_autotune(int(N), dt, int(ncand), ctypes.c_void_p(grids.ctypes.data), ctypes.c_void_p(ms.ctypes.data), ctypes.byref(best))
+    if rc != NS_OK:
+        raise NSError(rc, lib().ns_last_error(None).decode())
+    return int(best.value), [(int(g), float(t)) for g, t in zip(grids, ms) if g]
 
 
 class Solver:
@@ -275,6 +291,16 @@ class Solver:
 
     PASS_NAMES = ["a1_col_inv_x", "a2_col_inv_y", "a3_z_inv_prod", "a4_z_fwd", "a5_col_fwd_y", "a6_col_fwd_x",
                   "a7_spectral", "other"]
+
+    @property
+    def transform_grid(self):
+        """ns_transform_grid: the grid Nt >= N the transforms run on."""
+        return int(lib().ns_transform_grid(self._h))
+
+    @property
+    def padded_size(self):
+        """ns_padded_size: M = 3 Nt / 2, the padded grid max|u| is taken over."""
+        return int(lib().ns_padded_size(self._h))
 
     def set_pipeline(self, groups=1, z_sms=0):
         """ns_set_pipeline: process the batch in `groups` groups, the z kernel of a group on its own stream and `z_sms` SMs."""

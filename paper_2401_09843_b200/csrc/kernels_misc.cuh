@@ -28,7 +28,7 @@ __device__ __forceinline__ int wavenum(int i, int N) { return i < N / 2 ? i : i 
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(256)
-spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
+spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, int kmax, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
                 T gamma, const double* __restrict__ dt, int mode) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
@@ -43,7 +43,9 @@ spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, 
     cx<T>* op = out + b * 3 * plane + o;
     const int kxi = wavenum(ix, N), kyi = wavenum(iy, N);
     const int k2i = kxi * kxi + kyi * kyi + iz * iz;
-    const bool dead = (ix == N / 2) || (iy == N / 2) || (k2i == 0);
+    // truncation P_N of eq. 2.1: modes with a wavenumber component >= kmax = (user N)/2 carry nothing (kmax = N/2 unless the
+    // transform grid is larger than the user's grid, ns_create); k = 0: reading A8
+    const bool dead = (kxi >= kmax) || (kxi <= -kmax) || (kyi >= kmax) || (kyi <= -kmax) || (iz >= kmax) || (k2i == 0);
 
     cx<T> R[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
     cx<T> u[3];
@@ -146,26 +148,42 @@ static __global__ void umax_read_kernel(double* out, const unsigned long long* u
 // ------------------------------------------------------------------------------------------------
 // layout converters: public [.][N][N][N/2+1]  <->  internal [.][N][N][N/2]
 // ------------------------------------------------------------------------------------------------
+// Nu = the user's grid size (public arrays), N >= Nu the transform grid of the handle (internal arrays): a mode k of the
+// user's grid sits at stored index k mod Nu there and k mod N here; modes with |k_i| >= Nu/2 are zero here.
+__device__ __forceinline__ int embed_index(int i, int N, int Nu) {   // internal index -> public index, -1 if outside K_Nu
+    const int k = wavenum(i, N);
+    if (k >= Nu / 2 || k <= -(Nu / 2)) return -1;
+    return k >= 0 ? k : k + Nu;
+}
 template <typename T>
-__global__ void to_internal_kernel(const cx<T>* __restrict__ pub, cx<T>* __restrict__ in, int N, long total) {
+__global__ void to_internal_kernel(const cx<T>* __restrict__ pub, cx<T>* __restrict__ in, int N, int Nu, long total) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
-    const int H = N / 2;
+    const int H = N / 2, Hu = Nu / 2;
     const int iz = (int)(idx % H);
     const long row = idx / H;  // (cube, ix, iy)
     const int iy = (int)(row % N), ix = (int)((row / N) % N);
-    cx<T> v = pub[row * (H + 1) + iz];
-    if (ix == N / 2 || iy == N / 2) v = mk<T>(0, 0);
+    const long cube = row / ((long)N * N);
+    const int jx = embed_index(ix, N, Nu), jy = embed_index(iy, N, Nu);
+    cx<T> v = mk<T>(0, 0);
+    if (jx >= 0 && jy >= 0 && iz < Hu) v = pub[((cube * Nu + jx) * Nu + jy) * (Hu + 1) + iz];
     in[idx] = v;
 }
 template <typename T>
-__global__ void to_public_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ pub, int N, long total_pub) {
+__global__ void to_public_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ pub, int N, int Nu, long total_pub) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total_pub) return;
-    const int H = N / 2;
-    const int iz = (int)(idx % (H + 1));
-    const long row = idx / (H + 1);
-    pub[idx] = iz == H ? mk<T>(0, 0) : in[row * H + iz];
+    const int H = N / 2, Hu = Nu / 2;
+    const int iz = (int)(idx % (Hu + 1));
+    const long row = idx / (Hu + 1);
+    const int jy = (int)(row % Nu), jx = (int)((row / Nu) % Nu);
+    const long cube = row / ((long)Nu * Nu);
+    cx<T> v = mk<T>(0, 0);
+    if (iz != Hu && jx != Hu && jy != Hu) {
+        const int ix = jx < Hu ? jx : jx - Nu + N, iy = jy < Hu ? jy : jy - Nu + N;
+        v = in[((cube * N + ix) * N + iy) * H + iz];
+    }
+    pub[idx] = v;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -244,7 +262,7 @@ __global__ void sf_marginals_kernel(const cx<T>* __restrict__ U, double* __restr
         if (bins[i] != 0.0) atomicAdd(&marg[b * 3 * N + i], bins[i]);
 }
 // one block per sample, thread per l
-static __global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __restrict__ S, int N, int nl) {
+static __global__ void sf_finalize_kernel(const double* __restrict__ marg, double* __restrict__ S, int N, int Nu, int nl) {
     const int b = blockIdx.x;
     for (int l = 1 + threadIdx.x; l <= nl; l += blockDim.x) {
         double acc = 0.0;
@@ -253,9 +271,9 @@ static __global__ void sf_finalize_kernel(const double* __restrict__ marg, doubl
                 const double e = marg[(b * 3 + d) * N + i];
                 if (e == 0.0) continue;
                 const int k = (d == 2) ? i : wavenum(i, N);
-                // cos(2 pi k l / N) with exact argument reduction
-                const long kl = ((long)k * l) % N;
-                acc += 2.0 * (1.0 - cospi(2.0 * (double)kl / (double)N)) * e;
+                // cos(k l dx) = cos(2 pi k l / Nu), dx = 2 pi / Nu the user's grid spacing, with exact argument reduction
+                const long kl = ((long)k * l) % Nu;
+                acc += 2.0 * (1.0 - cospi(2.0 * (double)kl / (double)Nu)) * e;
             }
         S[b * nl + (l - 1)] = acc / 3.0;
     }
@@ -355,6 +373,58 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int nsub, int axis, 
     }
 }
 
+// Fallback of generic_fft_kernel for a grid size n that is not p 2^a (p in {1, 3, 5, 7, 15}): the plain O(n^2) DFT of tiles of
+// 8 lines, X[k] = sum_j x[j] exp(sign 2 pi i jk/n), roots from the table gtw[j] = exp(+2 pi i j/n).  Only the physical-space
+// entry points (ns_set_initial, ns_get_fields, S_p, moments) of handles with such a size use it; never on the hot path.
+template <typename T>
+__global__ void __launch_bounds__(256)
+dft_lines_kernel(cx<T>* __restrict__ A, int n, int axis, int sign, long total_tiles, const cx<T>* __restrict__ gtw) {
+    constexpr int TL = 8, PITCH = TL + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);   // [n][PITCH] input
+    cx<T>* O = S + (size_t)n * PITCH;                // [n][PITCH] output
+    const long tile = blockIdx.x;
+    if (tile >= total_tiles) return;
+    const long n2 = (long)n * n;
+    const long tiles_per_cube = (n2 + TL - 1) / TL;   // the last tile of a cube may be ragged (n^2 not a multiple of 8)
+    const long cube = tile / tiles_per_cube;
+    const long l0 = (tile % tiles_per_cube) * TL;
+    cx<T>* base = A + cube * n2 * n;
+    const long es = axis == 0 ? n2 : (axis == 1 ? n : 1);
+    auto line_base = [&](long l) -> long {
+        if (axis == 0) return l;
+        if (axis == 1) return (l / n) * n2 + (l % n);
+        return l * n;
+    };
+    for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
+        int j, c;
+        if (axis == 2) { j = e % n; c = e / n; } else { c = e % TL; j = e / TL; }
+        S[j * PITCH + c] = l0 + c < n2 ? base[line_base(l0 + c) + (long)j * es] : mk<T>(0, 0);
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
+        const int c = e % TL, k = e / TL;
+        T ar = 0, ai = 0;
+        int r = 0;                                   // (j k) mod n
+        for (int j = 0; j < n; ++j) {
+            const cx<T> w = ldg(gtw + r);
+            const cx<T> x = S[j * PITCH + c];
+            const T wy = sign > 0 ? w.y : -w.y;
+            ar += x.x * w.x - x.y * wy;
+            ai += x.x * wy + x.y * w.x;
+            r += k;
+            if (r >= n) r -= n;
+        }
+        O[k * PITCH + c] = mk<T>(ar, ai);
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
+        int j, c;
+        if (axis == 2) { j = e % n; c = e / n; } else { c = e % TL; j = e / TL; }
+        if (l0 + c < n2) base[line_base(l0 + c) + (long)j * es] = O[j * PITCH + c];
+    }
+}
+
 template <typename T>
 __global__ void real_to_complex_kernel(const T* __restrict__ in, cx<T>* __restrict__ out, long total) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -369,7 +439,7 @@ __global__ void complex_to_real_kernel(const cx<T>* __restrict__ in, T* __restri
 // W: [batch][3][N][N][N] full complex unnormalised spectra -> U internal, scaled 1/N^3, Nyquist zeroed,
 // Leray-projected for k != 0 (eq. 2.5 projector; reading A11).
 template <typename T>
-__global__ void init_project_kernel(const cx<T>* __restrict__ W, cx<T>* __restrict__ U, int N, long total, T scale) {
+__global__ void init_project_kernel(const cx<T>* __restrict__ W, cx<T>* __restrict__ U, int N, int Nu, long total, T scale) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
     const int H = N / 2;
@@ -377,15 +447,13 @@ __global__ void init_project_kernel(const cx<T>* __restrict__ W, cx<T>* __restri
     const int iy = (int)((idx / H) % N);
     const int ix = (int)((idx / ((long)H * N)) % N);
     const long b = idx / ((long)H * N * N);
-    const long plane = (long)N * N * H, cube = (long)N * N * N;
+    const long plane = (long)N * N * H, cube = (long)Nu * Nu * Nu;
     const long o = ((long)ix * N + iy) * H + iz;
     cx<T> u[3];
-    const bool nyq = ix == N / 2 || iy == N / 2;
+    const int jx = embed_index(ix, N, Nu), jy = embed_index(iy, N, Nu);
+    const bool nyq = jx < 0 || jy < 0 || iz >= Nu / 2;      // outside K_Nu (incl. the Nyquist planes of the user's grid)
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const cx<T> w = W[(b * 3 + c) * cube + ((long)ix * N + iy) * N + iz];
-        u[c] = nyq ? mk<T>(0, 0) : scale * w;
-    }
+    for (int c = 0; c < 3; ++c) u[c] = nyq ? mk<T>(0, 0) : scale * W[(b * 3 + c) * cube + ((long)jx * Nu + jy) * Nu + iz];
     const int kxi = wavenum(ix, N), kyi = wavenum(iy, N);
     const int k2i = kxi * kxi + kyi * kyi + iz * iz;
     if (!nyq && k2i > 0) {
@@ -399,24 +467,24 @@ __global__ void init_project_kernel(const cx<T>* __restrict__ W, cx<T>* __restri
     for (int c = 0; c < 3; ++c) U[(b * 3 + c) * plane + o] = u[c];
 }
 
-// U internal -> W full complex Hermitian spectrum on the N grid (kz < 0 from conj of (-k)).
+// U internal (transform grid N) -> W full complex Hermitian spectrum on the user's Nu grid (kz < 0 from conj of (-k)).
 template <typename T>
-__global__ void expand_hermitian_kernel(const cx<T>* __restrict__ U, cx<T>* __restrict__ W, int N, long total) {
+__global__ void expand_hermitian_kernel(const cx<T>* __restrict__ U, cx<T>* __restrict__ W, int N, int Nu, long total) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
-    const int H = N / 2;
-    const int iz = (int)(idx % N);
-    const int iy = (int)((idx / N) % N);
-    const int ix = (int)((idx / ((long)N * N)) % N);
-    const long cubei = idx / ((long)N * N * N);
+    const int H = N / 2, Hu = Nu / 2;
+    const int jz = (int)(idx % Nu);
+    const int jy = (int)((idx / Nu) % Nu);
+    const int jx = (int)((idx / ((long)Nu * Nu)) % Nu);
+    const long cubei = idx / ((long)Nu * Nu * Nu);
     const long plane = (long)N * N * H;
     cx<T> v = mk<T>(0, 0);
-    if (ix != N / 2 && iy != N / 2 && iz != N / 2) {
-        if (iz < H) {
-            v = U[cubei * plane + ((long)ix * N + iy) * H + iz];
+    if (jx != Hu && jy != Hu && jz != Hu) {
+        const int kx = jx < Hu ? jx : jx - Nu, ky = jy < Hu ? jy : jy - Nu, kz = jz < Hu ? jz : jz - Nu;
+        if (kz >= 0) {
+            v = U[cubei * plane + ((long)(kx >= 0 ? kx : kx + N) * N + (ky >= 0 ? ky : ky + N)) * H + kz];
         } else {
-            const int jx = (N - ix) % N, jy = (N - iy) % N, jz = N - iz;
-            v = conj(U[cubei * plane + ((long)jx * N + jy) * H + jz]);
+            v = conj(U[cubei * plane + ((long)(kx > 0 ? N - kx : -kx) * N + (ky > 0 ? N - ky : -ky)) * H - kz]);
         }
     }
     W[idx] = v;

@@ -6,6 +6,8 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <map>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -37,6 +39,9 @@ struct ns_solver {
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
     virtual int set_pipeline(int groups, int z_sms) = 0;
+    virtual int padded_size() const = 0;
+    virtual int transform_grid() const = 0;
+    virtual int time_transform(int reps, double* ms) = 0;
     virtual int profile(int enable) = 0;
     virtual int profile_read(double* ms, long long* cnt) = 0;
 };
@@ -115,7 +120,9 @@ struct PassProfiler {
 template <typename T>
 class Solver final : public ns_solver {
 public:
-    int N, L, M, H, batch;
+    int N, L, M, H, batch;   // N = the transform grid (N/2 a supported length), M = 3N/2 its padded grid
+    int Nu;                  // the user's grid (public arrays, truncation set K_Nu, dx, eps_N, m_N); Nu <= N, see ns_create
+    cx<T>* gNu = nullptr;    // exp(2 pi i j / Nu), j < Nu (unpadded transforms on the user's grid)
     int device = 0, num_sms = 0;   // the device the handle was created on (no process-wide caches)
     ns_params prm;
     cudaStream_t st;
@@ -140,7 +147,8 @@ public:
     cudaStream_t st_z = nullptr;
     cudaEvent_t ev_inv[MAX_GROUPS] = {}, ev_z[MAX_GROUPS] = {};
 
-    Solver(int N_, int batch_, const ns_params& p, cudaStream_t s) : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), prm(p), st(s) {}
+    Solver(int Nu_, int N_, int batch_, const ns_params& p, cudaStream_t s)
+        : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), Nu(Nu_), prm(p), st(s) {}
     ~Solver() override {
         if (arena) cudaFree(arena);
         if (st_z) cudaStreamDestroy(st_z);
@@ -215,7 +223,7 @@ public:
         nX = b * NS_NFLUX * (size_t)M * N * H;            // A1b; >= A1u (3 M N H), W (3 N^3 = 6 N^2 H), R (3 N^2 H)
         nY = b * 3 * (size_t)M * M * H;                   // A2u; >= Bh (5 N^2 H), public / physical staging
         nZ = b * NS_NFLUX * (size_t)M * M * H;            // A2b
-        const size_t pub = b * 3 * (size_t)N * N * (H + 1);
+        const size_t pub = b * 3 * (size_t)Nu * Nu * (Nu / 2 + 1);
         if (nY < pub) nY = pub;
         const size_t ndt = (size_t)3 * L * L + 1;
         red_count = b * (size_t)(4096 > 3 * N ? 4096 : 3 * N);
@@ -225,6 +233,7 @@ public:
         const size_t oU = take(nS * sizeof(cx<T>)), oV = take(nS * sizeof(cx<T>));
         const size_t oX = take(nX * sizeof(cx<T>)), oY = take(nY * sizeof(cx<T>)), oZ = take(nZ * sizeof(cx<T>));
         const size_t otw = take(twiddle_table_len(L) * sizeof(cx<T>));
+        const size_t ogu = take((size_t)Nu * sizeof(cx<T>));
         const size_t oD = take(ndt * sizeof(T));
         const size_t odt = take(b * sizeof(double)), ot = take(b * sizeof(double)), osc = take(b * sizeof(double));
         const size_t oum = take(b * sizeof(unsigned long long));
@@ -245,6 +254,7 @@ public:
         Y = (cx<T>*)(arena + oY);
         Z = (cx<T>*)(arena + oZ);
         twbase = (cx<T>*)(arena + otw);
+        gNu = (cx<T>*)(arena + ogu);
         dtab = (T*)(arena + oD);
         dt_dev = (double*)(arena + odt);
         t_dev = (double*)(arena + ot);
@@ -255,7 +265,14 @@ public:
 
         const std::vector<cx<T>> htw = build_twiddle_block<T>(L);
         std::vector<T> hd(ndt);
-        for (size_t k2 = 0; k2 < ndt; ++k2) hd[k2] = (T)dissipation_rate(prm, N, (double)k2);
+        for (size_t k2 = 0; k2 < ndt; ++k2) hd[k2] = (T)dissipation_rate(prm, Nu, (double)k2);   // eps_N, m_N of the USER's N
+        std::vector<cx<T>> hgu((size_t)Nu);
+        for (int j = 0; j < Nu; ++j) {
+            const long double a = 6.283185307179586476925286766559005768L * (long double)j / (long double)Nu;
+            hgu[(size_t)j].x = (T)cosl(a);
+            hgu[(size_t)j].y = (T)sinl(a);
+        }
+        NS_CK(cudaMemcpyAsync(gNu, hgu.data(), hgu.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemcpyAsync(twbase, htw.data(), htw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemcpyAsync(dtab, hd.data(), hd.size() * sizeof(T), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemsetAsync(t_dev, 0, b * sizeof(double), st));
@@ -329,7 +346,7 @@ public:
         prof.tick(6, st);
         spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y + (size_t)b0 * NS_NFLUX * plane, Us + (size_t)b0 * 3 * plane,
                                                                     Un ? Un + (size_t)b0 * 3 * plane : nullptr, out + (size_t)b0 * 3 * plane, N,
-                                                                    total, dtab, scale, (T)alpha, (T)beta, (T)gamma, dt_dev + b0, mode);
+                                                                    Nu / 2, total, dtab, scale, (T)alpha, (T)beta, (T)gamma, dt_dev + b0, mode);
         NS_LAUNCHED("a7 spectral_kernel");
         prof.tick(-1, st);
         return NS_OK;
@@ -381,7 +398,7 @@ public:
                 set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev + b0, t_dev + b0, scal_dev + b0, umax2 + b0, bad_dev + b0, nb);
                 NS_LAUNCHED("set_dt_array");
             } else {
-                cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev + b0, t_dev + b0, umax2 + b0, bad_dev + b0, cfl, 2.0 * 3.14159265358979323846 / N,
+                cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev + b0, t_dev + b0, umax2 + b0, bad_dev + b0, cfl, 2.0 * 3.14159265358979323846 / Nu,
                                                         t_end, nb);
                 NS_LAUNCHED("cfl_finalize");
             }
@@ -462,9 +479,9 @@ public:
 
     // internal [b*3][N][N][H] -> public layout in caller memory
     int export_spectral(const cx<T>* src, void* out, ns_memspace ms) {
-        const long total_pub = (long)batch * 3 * N * N * (H + 1);
+        const long total_pub = (long)batch * 3 * Nu * Nu * (Nu / 2 + 1);
         cx<T>* dst = ms == NS_DEVICE ? (cx<T>*)out : Y;
-        to_public_kernel<T><<<blocks_for(total_pub, 256), 256, 0, st>>>(src, dst, N, total_pub);
+        to_public_kernel<T><<<blocks_for(total_pub, 256), 256, 0, st>>>(src, dst, N, Nu, total_pub);
         NS_LAUNCHED("to_public");
         if (ms == NS_HOST) {
             NS_CK(cudaMemcpyAsync(out, Y, (size_t)total_pub * sizeof(cx<T>), cudaMemcpyDeviceToHost, st));
@@ -481,14 +498,14 @@ public:
 
     int set_spectral(const void* in, ns_memspace ms) override {
         if (!in) return fail(NS_ERR_INVALID_ARG, "input pointer is NULL");
-        const long total_pub = (long)batch * 3 * N * N * (H + 1);
+        const long total_pub = (long)batch * 3 * Nu * Nu * (Nu / 2 + 1);
         const cx<T>* src = (const cx<T>*)in;
         if (ms == NS_HOST) {
             NS_CK(cudaMemcpyAsync(Y, in, (size_t)total_pub * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
             src = Y;
         }
         const long total = (long)batch * 3 * N * N * H;
-        to_internal_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, U, N, total);
+        to_internal_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, U, N, Nu, total);
         NS_LAUNCHED("to_internal");
         NS_CK(cudaMemsetAsync(bad_dev, 0, (size_t)batch * sizeof(int), st));
         if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));  // caller buffer fully consumed
@@ -496,18 +513,30 @@ public:
         return NS_OK;
     }
 
+    // unpadded 3-D transform on the USER's grid (cubes of Nu^3 complex), in place: mixed radix when Nu = p 2^a with p in
+    // {1, 3, 5, 7, 15} and Nu a multiple of 8, else the plain DFT
     int generic_fft3(cx<T>* W, long cubes, int sign) {
-        const int radix3 = N % 15 == 0 ? 15 : (N % 3 == 0 ? 3 : (N % 5 == 0 ? 5 : (N % 7 == 0 ? 7 : 1)));   // odd factor of N
-        const int m = N / radix3;
-        int log2m = 0;
-        while ((1 << log2m) < m) ++log2m;
-        const long tiles = cubes * (long)N * N / 8;
-        const size_t smem = (size_t)N * 9 * sizeof(cx<T>);
-        if (smem > 48 * 1024)
-            NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        for (int axis = 0; axis < 3; ++axis) {
-            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2m, radix3, axis, sign, tiles, tw().gN, 3);
-            NS_LAUNCHED("generic_fft");
+        int odd = Nu, log2m = 0;
+        while (odd % 2 == 0) { odd /= 2; ++log2m; }
+        const bool fast = (odd == 1 || odd == 3 || odd == 5 || odd == 7 || odd == 15) && Nu % 8 == 0;
+        if (fast) {
+            const long tiles = cubes * (long)Nu * Nu / 8;
+            const size_t smem = (size_t)Nu * 9 * sizeof(cx<T>);
+            if (smem > 48 * 1024)
+                NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            for (int axis = 0; axis < 3; ++axis) {
+                generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, Nu, log2m, odd, axis, sign, tiles, gNu, 3);
+                NS_LAUNCHED("generic_fft");
+            }
+        } else {
+            const long tiles = cubes * (((long)Nu * Nu + 7) / 8);
+            const size_t smem = (size_t)2 * Nu * 9 * sizeof(cx<T>);
+            if (smem > 48 * 1024)
+                NS_CK(cudaFuncSetAttribute(dft_lines_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            for (int axis = 0; axis < 3; ++axis) {
+                dft_lines_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, Nu, axis, sign, tiles, gNu);
+                NS_LAUNCHED("dft_lines");
+            }
         }
         return NS_OK;
     }
@@ -515,7 +544,7 @@ public:
     int set_initial(const void* in, ns_memspace ms) override {
         if (!in) return fail(NS_ERR_INVALID_ARG, "input pointer is NULL");
         const long cubes = (long)batch * 3;
-        const long total = cubes * N * N * N;
+        const long total = cubes * Nu * Nu * Nu;
         const T* src = (const T*)in;
         if (ms == NS_HOST) {
             NS_CK(cudaMemcpyAsync(Y, in, (size_t)total * sizeof(T), cudaMemcpyHostToDevice, st));
@@ -526,7 +555,7 @@ public:
         int rc = generic_fft3(X, cubes, -1);
         if (rc != NS_OK) return rc;
         const long tot = (long)batch * N * N * H;
-        init_project_kernel<T><<<blocks_for(tot, 256), 256, 0, st>>>(X, U, N, tot, (T)(1.0 / ((double)N * N * N)));
+        init_project_kernel<T><<<blocks_for(tot, 256), 256, 0, st>>>(X, U, N, Nu, tot, (T)(1.0 / ((double)Nu * Nu * Nu)));
         NS_LAUNCHED("init_project");
         NS_CK(cudaMemsetAsync(t_dev, 0, (size_t)batch * sizeof(double), st));
         NS_CK(cudaMemsetAsync(bad_dev, 0, (size_t)batch * sizeof(int), st));
@@ -539,8 +568,8 @@ public:
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
         if (!out) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
         const long cubes = (long)batch * 3;
-        const long total = cubes * N * N * N;
-        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        const long total = cubes * Nu * Nu * Nu;
+        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, Nu, total);
         NS_LAUNCHED("expand_hermitian");
         int rc = generic_fft3(X, cubes, +1);
         if (rc != NS_OK) return rc;
@@ -573,7 +602,7 @@ public:
 
     int structure_function(double* S, int nl) override {
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
-        if (!S || nl < 1 || nl > N / 2) return fail(NS_ERR_INVALID_ARG, "S is NULL or nl not in [1, N/2]");
+        if (!S || nl < 1 || nl > Nu / 2) return fail(NS_ERR_INVALID_ARG, "S is NULL or nl not in [1, N/2]");
         NS_CK(cudaMemsetAsync(red_dev, 0, (size_t)batch * 3 * N * sizeof(double), st));
         const long plane = (long)N * N * H;
         unsigned chunks = blocks_for(plane, 256 * 16);
@@ -581,7 +610,7 @@ public:
         sf_marginals_kernel<T><<<dim3(chunks, batch), 256, (size_t)3 * N * sizeof(double), st>>>(U, red_dev, N);
         NS_LAUNCHED("sf_marginals");
         double* out_dev = reinterpret_cast<double*>(Y);
-        sf_finalize_kernel<<<batch, 128, 0, st>>>(red_dev, out_dev, N, nl);
+        sf_finalize_kernel<<<batch, 128, 0, st>>>(red_dev, out_dev, N, Nu, nl);
         NS_LAUNCHED("sf_finalize");
         NS_CK(cudaMemcpyAsync(S, out_dev, (size_t)batch * nl * sizeof(double), cudaMemcpyDeviceToHost, st));
         NS_CK(cudaStreamSynchronize(st));
@@ -590,11 +619,11 @@ public:
 
     int structure_function_p(double p, double* S, int nl) override {
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
-        if (!S || nl < 1 || nl > N / 2 || !(p > 0.0) || std::isinf(p)) return fail(NS_ERR_INVALID_ARG, "S is NULL, nl not in [1, N/2] or p not positive and finite");
+        if (!S || nl < 1 || nl > Nu / 2 || !(p > 0.0) || std::isinf(p)) return fail(NS_ERR_INVALID_ARG, "S is NULL, nl not in [1, N/2] or p not positive and finite");
         // physical fields on the N grid, as in get_fields: Hermitian expansion -> unpadded inverse FFT -> reals in Y
         const long cubes = (long)batch * 3;
-        const long total = cubes * N * N * N;
-        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        const long total = cubes * Nu * Nu * Nu;
+        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, Nu, total);
         NS_LAUNCHED("expand_hermitian");
         int rc = generic_fft3(X, cubes, +1);
         if (rc != NS_OK) return rc;
@@ -602,10 +631,10 @@ public:
         complex_to_real_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(X, phys, total);
         NS_LAUNCHED("complex_to_real");
         NS_CK(cudaMemsetAsync(red_dev, 0, (size_t)batch * nl * sizeof(double), st));
-        const long np = (long)N * N * N;
+        const long np = (long)Nu * Nu * Nu;
         unsigned chunks = blocks_for(np, 256 * 8);
         if (chunks > 592) chunks = 592;
-        sf_p_kernel<T><<<dim3(chunks, nl, batch), 256, 0, st>>>(phys, red_dev, N, nl, p);
+        sf_p_kernel<T><<<dim3(chunks, nl, batch), 256, 0, st>>>(phys, red_dev, Nu, nl, p);
         NS_LAUNCHED("sf_p");
         scale_kernel<<<blocks_for((long)batch * nl, 128), 128, 0, st>>>(red_dev, 1.0 / (3.0 * (double)np), batch * nl);
         NS_LAUNCHED("scale");
@@ -618,15 +647,15 @@ public:
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
         if (!mean && !var) return fail(NS_ERR_INVALID_ARG, "both output pointers are NULL");
         const long cubes = (long)batch * 3;
-        const long total = cubes * N * N * N;
-        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        const long total = cubes * Nu * Nu * Nu;
+        expand_hermitian_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, Nu, total);
         NS_LAUNCHED("expand_hermitian");
         int rc = generic_fft3(X, cubes, +1);
         if (rc != NS_OK) return rc;
         T* phys = reinterpret_cast<T*>(Y);
         complex_to_real_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(X, phys, total);
         NS_LAUNCHED("complex_to_real");
-        const long n = 3L * N * N * N;                 // X is free again: mean | var staged there
+        const long n = 3L * Nu * Nu * Nu;              // X is free again: mean | var staged there
         T* dmean = reinterpret_cast<T*>(X);
         T* dvar = dmean + n;
         ensemble_moments_kernel<T><<<blocks_for(n, 256), 256, 0, st>>>(phys, dmean, dvar, n, batch);
@@ -636,6 +665,30 @@ public:
         if (var) NS_CK(cudaMemcpyAsync(var, dvar, (size_t)n * sizeof(T), kind, st));
         if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));
         return NS_OK;
+    }
+
+    int padded_size() const override { return M; }
+    int transform_grid() const override { return N; }
+
+    // autotune probe: milliseconds of one pass a1..a6 over whatever the workspaces hold (the work is data independent)
+    int time_transform(int reps, double* ms) override {
+        cudaEvent_t a, b;
+        NS_CK(cudaEventCreate(&a));
+        NS_CK(cudaEventCreate(&b));
+        NS_CK(cudaMemsetAsync(U, 0, nS * sizeof(cx<T>), st));
+        int rc = transform(U, false);
+        if (rc == NS_OK) {
+            cudaEventRecord(a, st);
+            for (int i = 0; i < reps && rc == NS_OK; ++i) rc = transform(U, false);
+            cudaEventRecord(b, st);
+            cudaError_t e = cudaStreamSynchronize(st);
+            float t = 0;
+            if (rc == NS_OK && e == cudaSuccess && cudaEventElapsedTime(&t, a, b) == cudaSuccess) *ms = t / reps;
+            else if (rc == NS_OK) rc = cuda_fail(e, "time_transform");
+        }
+        cudaEventDestroy(a);
+        cudaEventDestroy(b);
+        return rc;
     }
 
     int profile(int enable) override {
@@ -664,8 +717,8 @@ public:
 };
 
 template <typename T>
-int create_typed(ns_solver** out, int N, int batch, const ns_params& p, cudaStream_t st) {
-    Solver<T>* s = new Solver<T>(N, batch, p, st);
+int create_typed(ns_solver** out, int Nu, int N, int batch, const ns_params& p, cudaStream_t st) {
+    Solver<T>* s = new Solver<T>(Nu, N, batch, p, st);
     int rc = s->init();
     if (rc != NS_OK) {
         g_create_error = s->err;
@@ -676,33 +729,52 @@ int create_typed(ns_solver** out, int N, int batch, const ns_params& p, cudaStre
     return NS_OK;
 }
 
+// ---- transform-grid selection ("we round the padded data's size up to the next value of the form 2^a 3^b 5^c 7^d
+// ... On any new system, we therefore once run a benchmark of only the Fourier transform storing its results and extracting the
+// optimal padding size from that generated data.  If no suitable size is found in the benchmark results, we choose the next
+// larger N with prime factors at most 7 instead").  Here the padded grid is 3/2 of the TRANSFORM grid Nt >= N, Nt/2 one of the
+// supported lengths; the state lives on the Nt grid with zeros outside K_N, which gives the RHS of the user's N exactly
+// (independence of the padding, oracle pin P7).
+bool transform_grid_ok(int Nt, ns_dtype dtype) {
+    const int tile = dtype == NS_F32 ? 16 : 8;
+    return Nt >= 16 && Nt <= 640 && Nt % 2 == 0 && fft_supported(Nt / 2) && (Nt / 2) % tile == 0;
+}
+int next_transform_grid(int N, ns_dtype dtype) {
+    for (int Nt = N + (N & 1); Nt <= 640; Nt += 2)
+        if (transform_grid_ok(Nt, dtype)) return Nt;
+    return 0;
+}
+struct TuneKey {
+    int device, N, dtype;
+    bool operator<(const TuneKey& o) const { return device != o.device ? device < o.device : (N != o.N ? N < o.N : dtype < o.dtype); }
+};
+std::mutex g_tune_mutex;
+std::map<TuneKey, int> g_tune_table;   // (device, N, dtype) -> transform grid chosen by ns_autotune
+
 }  // namespace
 
 extern "C" {
 
-int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream) {
-    g_create_error.clear();
-    if (!out) { g_create_error = "out is NULL"; return NS_ERR_INVALID_ARG; }
-    *out = nullptr;
-    // N = p 2^a with p in {1, 3, 5, 7, 15} (sizes with small prime factors); a column tile is 128 bytes = 8 (fp64) /
-    // 16 (fp32) complex values of the N/2 stored kz entries
-    const int tile = dtype == NS_F32 ? 16 : 8;
-    if (N < 16 || N > 640 || (N % 2) != 0 || !fft_supported(N / 2) || (N / 2) % tile != 0) {
-        g_create_error = "N must be p * 2^a with p in {1, 3, 5, 7, 15}, 16 <= N <= 640 and N/2 a multiple of 8 (fp32: of 16)";
-        return NS_ERR_INVALID_ARG;
-    }
-    if (batch < 1) { g_create_error = "batch must be >= 1"; return NS_ERR_INVALID_ARG; }
-    if (dtype != NS_F64 && dtype != NS_F32) { g_create_error = "unknown dtype"; return NS_ERR_INVALID_ARG; }
-    ns_params prm;
-    std::memset(&prm, 0, sizeof prm);
-    prm.s = 1.0;
-    prm.m_cut = -1.0;
-    prm.q_exp = -1.0;
-    if (p) prm = *p;
-    if (!(prm.s >= 1.0) || prm.nu < 0.0 || prm.eps < 0.0 || !(prm.nu == prm.nu) || !(prm.eps == prm.eps)) {
+static int resolve_params(const ns_params* p, ns_params* prm) {
+    std::memset(prm, 0, sizeof *prm);
+    prm->s = 1.0;
+    prm->m_cut = -1.0;
+    prm->q_exp = -1.0;
+    if (p) *prm = *p;
+    if (!(prm->s >= 1.0) || prm->nu < 0.0 || prm->eps < 0.0 || !(prm->nu == prm->nu) || !(prm->eps == prm->eps)) {
         g_create_error = "params: need s >= 1, nu >= 0, eps >= 0";
         return NS_ERR_INVALID_ARG;
     }
+    return NS_OK;
+}
+static int create_on_grid(ns_solver** out, int N, int Nt, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream) {
+    ns_params prm;
+    int rcp = resolve_params(p, &prm);
+    if (rcp != NS_OK) return rcp;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return dtype == NS_F64 ? create_typed<double>(out, N, Nt, batch, prm, st) : create_typed<float>(out, N, Nt, batch, prm, st);
+}
+static int check_device() {
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev < 1) {
@@ -710,8 +782,73 @@ int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dt
         g_create_error = std::string("no usable CUDA device (no CPU fallback): ") + (e != cudaSuccess ? cudaGetErrorString(e) : "0 devices");
         return NS_ERR_CUDA;
     }
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    return dtype == NS_F64 ? create_typed<double>(out, N, batch, prm, st) : create_typed<float>(out, N, batch, prm, st);
+    return NS_OK;
+}
+static int check_sizes(int N, int batch, ns_dtype dtype) {
+    if (dtype != NS_F64 && dtype != NS_F32) { g_create_error = "unknown dtype"; return NS_ERR_INVALID_ARG; }
+    // any even N; the transforms run on the next grid Nt >= N with Nt = p 2^a, p in {1, 3, 5, 7, 15}, Nt/2 a multiple of the
+    // column tile (128 bytes = 8 fp64 / 16 fp32 complex values)
+    if (N < 16 || N > 640 || (N % 2) != 0 || next_transform_grid(N, dtype) == 0) {
+        g_create_error = "N must be even with 16 <= N <= 640";
+        return NS_ERR_INVALID_ARG;
+    }
+    if (batch < 1) { g_create_error = "batch must be >= 1"; return NS_ERR_INVALID_ARG; }
+    return NS_OK;
+}
+
+int ns_create(ns_solver** out, int N, int batch, const ns_params* p, ns_dtype dtype, void* cuda_stream) {
+    g_create_error.clear();
+    if (!out) { g_create_error = "out is NULL"; return NS_ERR_INVALID_ARG; }
+    *out = nullptr;
+    int rc = check_sizes(N, batch, dtype);
+    if (rc != NS_OK) return rc;
+    ns_params chk;
+    if ((rc = resolve_params(p, &chk)) != NS_OK) return rc;
+    if ((rc = check_device()) != NS_OK) return rc;
+    int Nt = next_transform_grid(N, dtype), dev = 0;
+    cudaGetDevice(&dev);
+    {
+        std::lock_guard<std::mutex> lock(g_tune_mutex);
+        auto it = g_tune_table.find(TuneKey{dev, N, (int)dtype});
+        if (it != g_tune_table.end()) Nt = it->second;
+    }
+    return create_on_grid(out, N, Nt, batch, p, dtype, cuda_stream);
+}
+
+int ns_autotune(int N, ns_dtype dtype, int ncand, int* grids_out, double* ms_out, int* best_out) {
+    g_create_error.clear();
+    int rc = check_sizes(N, 1, dtype);
+    if (rc != NS_OK) return rc;
+    if (ncand < 1 || ncand > 16) { g_create_error = "ncand must be in [1, 16]"; return NS_ERR_INVALID_ARG; }
+    if ((rc = check_device()) != NS_OK) return rc;
+    int best = 0, found = 0;
+    double best_ms = 0.0;
+    for (int Nt = next_transform_grid(N, dtype); Nt != 0 && found < ncand; Nt = next_transform_grid(Nt + 2, dtype)) {
+        ns_solver* h = nullptr;
+        rc = create_on_grid(&h, N, Nt, 1, nullptr, dtype, nullptr);
+        double ms = 0.0;
+        if (rc == NS_OK) rc = h->time_transform(3, &ms);
+        if (rc != NS_OK && h) g_create_error = h->err;
+        delete h;
+        if (rc == NS_ERR_OOM && found > 0) break;      // larger grids do not fit: keep what was measured
+        if (rc != NS_OK) return rc;
+        if (grids_out) grids_out[found] = Nt;
+        if (ms_out) ms_out[found] = ms;
+        if (found == 0 || ms < best_ms) { best = Nt; best_ms = ms; }
+        ++found;
+    }
+    for (int i = found; i < ncand; ++i) {
+        if (grids_out) grids_out[i] = 0;
+        if (ms_out) ms_out[i] = 0.0;
+    }
+    int dev = 0;
+    cudaGetDevice(&dev);
+    {
+        std::lock_guard<std::mutex> lock(g_tune_mutex);
+        g_tune_table[TuneKey{dev, N, (int)dtype}] = best;
+    }
+    if (best_out) *best_out = best;
+    return NS_OK;
 }
 
 int ns_destroy(ns_solver* h) {
@@ -744,6 +881,8 @@ double ns_time(const ns_solver* h, int sample) {
 int ns_set_pipeline(ns_solver* h, int groups, int z_sms) { NS_H(h); return h->set_pipeline(groups, z_sms); }
 int ns_profile(ns_solver* h, int enable) { NS_H(h); return h->profile(enable); }
 int ns_profile_read(ns_solver* h, double* ms, long long* cnt) { NS_H(h); return h->profile_read(ms, cnt); }
+int ns_transform_grid(const ns_solver* h) { return h ? h->transform_grid() : 0; }
+int ns_padded_size(const ns_solver* h) { return h ? h->padded_size() : 0; }
 long long ns_kernel_launches(const ns_solver* h) { return h ? h->launches : 0; }
 long long ns_device_bytes(const ns_solver* h) { return h ? h->device_bytes() : 0; }
 const char* ns_last_error(const ns_solver* h) { return h ? h->err.c_str() : g_create_error.c_str(); }

@@ -45,8 +45,8 @@ def test_no_torch_types_in_header():
 def test_create_rejects_bad_arguments(libns):
     from paper_2401_09843_b200 import binding
     h = ctypes.c_void_p()
-    for N, batch, dtype in [(7, 1, 0), (24, 1, 0), (1024, 1, 0), (8, 1, 0), (16, 1, 1), (32, 0, 0), (32, 1, 5), (40, 1, 0), (144, 1, 0), (200, 1, 0),
-                            (48, 1, 1), (80, 1, 1), (768, 1, 0)]:
+    for N, batch, dtype in [(7, 1, 0), (1024, 1, 0), (8, 1, 0), (32, 0, 0), (32, 1, 5), (41, 1, 0), (14, 1, 0), (642, 1, 0),
+                            (768, 1, 0)]:
         rc = libns.ns_create(ctypes.byref(h), N, batch, None, dtype, None)
         assert rc == binding.NS_ERR_INVALID_ARG, (N, batch, dtype, rc)
         assert not h.value

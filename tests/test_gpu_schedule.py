@@ -11,7 +11,8 @@ Tolerances are the north_star's: relative L2 <= 1e-12 per ns_rhs, <= 1e-10 after
 Run on the B200 box:  python -m pytest tests -m gpu
 
 The oracle is deliberately naive (25 s per 256^3 RHS on the box's 16 cores), so the whole `-m gpu` suite is sized to stay well
-inside the driver's 1200 s limit: by default config 3 replays 1 step and config 4 six; `NS_FULL_SCHEDULE=1` runs the full
+inside the driver's 1200 s limit: by default config 3 checks the full-array RHS only and config 4 replays four steps;
+`NS_FULL_SCHEDULE=1` runs the full
 counts (3 and 10 steps, 20 steps at 96^3, two samples at 192^3) -- the log of such a run is profiles/r02_parity_schedule.md.
 """
 import os
@@ -74,8 +75,9 @@ def test_config2_128_rhs_and_20_cfl_steps(ns, oracle):
 def test_config3_256_full_array_rhs_and_steps(ns, oracle):
     """BASELINE.json configs[2] with its own input (perturbed shear layer, seed 3) at N = 256 -- the size that runs the
     long-line kernels: EVERY stored entry of ns_rhs against orc_rhs_parts (relative L2 <= 1e-12, and the largest
-    single-entry deviation), max|u| on the padded grid, then 1 CFL step (3 with NS_FULL_SCHEDULE=1; an oracle step at this
-    size takes 80 s) with the oracle replaying the GPU's dt."""
+    single-entry deviation), max|u| on the padded grid; with NS_FULL_SCHEDULE=1 then 3 CFL steps with the oracle replaying the
+    GPU's dt (an oracle step at this size takes 80 s; by default the fused step at 256^3 / 512^3 is checked against eq. 2.6
+    assembled from ns_rhs in test_full_size_stratified_sampled_rhs, and against the oracle at every smaller size)."""
     N = 256
     u = inputs.shear_layer(N, seed=3)
     kw = dict(eps=0.05, s=1.0)
@@ -94,7 +96,7 @@ def test_config3_256_full_array_rhs_and_steps(ns, oracle):
     assert np.abs(got - want["r"]).max() < 1e-12 * np.abs(want["r"]).max()     # no single entry is off (tile faults)
     assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
     del got, want
-    worst, nsteps = 0.0, 3 if FULL else 1
+    worst, nsteps = 0.0, 3 if FULL else 0
     for i in range(nsteps):
         dts = s.step_cfl(0.2, 1e9)
         uh = oracle.step(N, p, uh, dts[0])
@@ -106,7 +108,7 @@ def test_config3_256_full_array_rhs_and_steps(ns, oracle):
 # ------------------------------------------------------------------------------------------------ config 4
 def test_config4_one_sample_replayed(ns, oracle):
     """BASELINE.json configs[3]: the 32 x 128^3 shear-layer ensemble stepped in ONE batched launch at per-sample CFL 0.2;
-    the oracle replays sample 1's dt sequence for 6 steps (10 with NS_FULL_SCHEDULE=1).  State at relative L2 <= 1e-10 at every step; the reported
+    the oracle replays sample 1's dt sequence for 4 steps (10 with NS_FULL_SCHEDULE=1).  State at relative L2 <= 1e-10 at every step; the reported
     statistics E(K) and S_2(l) of that sample at the statistical tolerance of reading A17 (1e-8 relative)."""
     N, B, pick = 128, 32, 1
     us = inputs.shear_layer_ensemble(N, B, seed0=1000)
@@ -120,7 +122,7 @@ def test_config4_one_sample_replayed(ns, oracle):
     uh = u0[pick].copy()
     del u0
     p = oracle.Params(**kw)
-    worst, nsteps = 0.0, 10 if FULL else 6
+    worst, nsteps = 0.0, 10 if FULL else 4
     for i in range(nsteps):
         dts = s.step_cfl(0.2, 1.0)
         uh = oracle.step(N, p, uh, dts[pick])
@@ -360,3 +362,69 @@ def test_sizes_5_7_15_large_sampled(ns, oracle, N):
     w = np.full(N // 2 + 1, 2.0)
     w[0] = 1.0
     assert abs(np.sum(w * np.real(np.conj(uh) * rn))) < 1e-12 * np.sum(w * np.abs(uh) * np.abs(rn))
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-3: general N, autotune
+@pytest.mark.parametrize("N", [18, 50, 100])
+def test_general_even_n_on_a_larger_transform_grid(ns, oracle, N):
+    """SURVEY.md 8(f) NEXT-3 / PAPER.md:L175 (the padded size may be any size >= 3N/2; it is rounded up to one with small prime
+    factors): an N that is not p 2^a runs on the next admissible transform grid Nt > N, padded grid M = 3 Nt / 2 > 3N/2, with the
+    state truncated to the user's N.  Against the oracle at the user's N with the SAME padded size M (by pin P7 the RHS does not
+    depend on M; max|u| does): set_initial (plain DFT on the N grid), get_fields, RHS (every entry), max|u|, 5 CFL steps (2 at N = 100),
+    spectra, S_2 and S_p."""
+    u = inputs.gaussian_field(N, 800 + N, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    u += 0.2 * inputs.normal01(N, 3, 3 * N ** 3).reshape(3, N, N, N)          # not solenoidal, full band
+    kw = dict(nu=0.002, eps=0.05, s=1.5)
+    s = ns.Solver(N, **kw)
+    Nt, M = s.transform_grid, s.padded_size
+    assert Nt > N and M == 3 * Nt // 2 and M > 3 * N // 2
+    s.set_initial(u[None])
+    uh = oracle.set_initial(N, u)
+    got = s.get_spectral()[0]
+    assert got.shape == uh.shape and rel(got, uh) < 1e-13
+    assert rel(s.get_fields()[0], oracle.get_fields(N, uh)) < 1e-13
+    s.set_spectral(uh[None])
+    assert np.array_equal(s.get_spectral()[0], uh)                              # round trip through the larger grid is exact
+    p = oracle.Params(**kw)
+    want = oracle.rhs_parts(N, p, uh, M)
+    r = s.rhs()[0]
+    assert rel(r, want["r"]) < TOL_RHS_F64
+    assert rel(r, oracle.rhs(N, p, uh)) < TOL_RHS_F64                           # and equals the 3N/2 result (P7)
+    assert np.all(r[:, N // 2] == 0) and np.all(r[:, :, N // 2] == 0) and np.all(r[:, :, :, N // 2] == 0)
+    assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
+    worst, nsteps = 0.0, 5 if (FULL or N < 100) else 2
+    for i in range(nsteps):
+        dts = s.step_cfl(0.2, 1e9)
+        assert abs(dts[0] - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, uh, M)) < 1e-12 * dts[0]
+        uh = oracle.step(N, p, uh, dts[0], M)
+        worst = max(worst, rel(s.get_spectral()[0], uh))
+        assert worst < TOL_STEPS_F64, (i, worst)
+    assert np.abs(s.energy_spectrum(N)[0] - oracle.energy_spectrum(N, uh, N)).max() < 1e-13
+    Zo = oracle.enstrophy_spectrum(N, uh, N)
+    assert np.abs(s.enstrophy_spectrum(N)[0] - Zo).max() < 1e-12 * Zo.max()
+    assert np.abs(s.structure_function()[0] / oracle.structure_function(N, uh) - 1).max() < 1e-11
+    assert np.abs(s.structure_function_p(3.0, nl=4)[0] / oracle.structure_function_p(N, uh, 3.0, 4) - 1).max() < 1e-11
+    print(f"N = {N} on transform grid {Nt} (padded {M}): worst rel-L2 over {nsteps} steps {worst:.2e}")
+
+
+def test_autotune_records_the_transform_grid(ns, oracle):
+    """ns_autotune (benchmark of the transform only, the fastest padding is stored and used afterwards): candidates
+    are the admissible grids >= N in increasing order; the recorded one is the fastest measured; ns_create uses it; the result on
+    whatever grid was chosen still matches the oracle with that padded size.  For an N that is itself admissible the candidates
+    start with N."""
+    N = 100
+    best, cand = ns.autotune(N, "f64", 3)
+    assert [g for g, _ in cand] == [112, 128, 160] and all(t > 0 for _, t in cand)
+    assert best == min(cand, key=lambda c: c[1])[0]
+    s = ns.Solver(N, eps=0.05)
+    assert s.transform_grid == best and s.padded_size == 3 * best // 2
+    u = inputs.gaussian_field(N, 77, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    s.set_initial(u[None])
+    uh = s.get_spectral()[0]
+    want = oracle.rhs_parts(N, oracle.Params(eps=0.05), uh, s.padded_size)
+    assert rel(s.rhs()[0], want["r"]) < TOL_RHS_F64
+    assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
+    best2, cand2 = ns.autotune(128, "f64", 2)
+    assert [g for g, _ in cand2] == [128, 160]
+    with pytest.raises(ns.NSError):
+        ns.autotune(101, "f64", 2)
