@@ -15,7 +15,7 @@
 //  * the twiddle factors a thread needs (they depend on its position in the team only, not on the tile) are parked once per
 //    CTA in TENSOR MEMORY (tmem.cuh) and fetched four (fp64) at a time instead of 31 L1 loads per thread and tile.
 //
-// Measured (profiles/r02_experiments.md): a5 3.65 -> 3.20 ms, a6 2.67 -> 2.52 ms at 512^3 fp64.  The inverse counterpart and
+// Measured (profiles/r02_experiments.md) at 512^3: fp64 a5 3.65 -> 3.20 ms, a6 2.67 -> 2.52 ms; fp32 1.96 -> 1.84, 1.40 -> 1.24 ms.  The inverse counterpart and
 // the shorter lines (L = 64, 128) were built and measured too and lost against kernels_col.cuh; they are not in the library.
 // Tile, register stages R1 x R2, twiddle tables and the decimated physical order are those of kernels_col.cuh.
 #pragma once

@@ -7,6 +7,7 @@
 // Internal spectral layout: [batch][comp][N][N][H], H = N/2 (the identically-zero kz = N/2 column of the
 // public layout is not stored, so rows are 128-byte aligned).
 #pragma once
+#include <cuda_pipeline.h>
 #include <math_constants.h>
 
 #include "cx.cuh"
@@ -279,6 +280,39 @@ static __global__ void sf_finalize_kernel(const double* __restrict__ marg, doubl
     }
 }
 
+// G consecutive radix-2 DIT levels s .. s+G-1 of the tile in shared memory S[n][9] (8 lines), done in registers: the 2^G
+// elements base + t 2^(s-1) of a block of 2^(s-1+G) (a sub-sequence of length m is a whole number of such blocks).
+template <typename T, int G>
+__device__ __forceinline__ void generic_dit_pass(cx<T>* __restrict__ S, int s, int n, int sign, const cx<T>* __restrict__ gtw) {
+    constexpr int TL = 8, PITCH = TL + 1, R = 1 << G;
+    const int half0 = 1 << (s - 1);
+    const int items = (n >> G) * TL;
+    for (int e = threadIdx.x; e < items; e += blockDim.x) {
+        const int c = e % TL, gi = e / TL;
+        const int o = gi & (half0 - 1);
+        const int base = ((gi >> (s - 1)) << (s - 1 + G)) + o;
+        cx<T> v[R];
+#pragma unroll
+        for (int t = 0; t < R; ++t) v[t] = S[(base + t * half0) * PITCH + c];
+#pragma unroll
+        for (int l = 0; l < G; ++l) {
+            const int dt = 1 << l;
+#pragma unroll
+            for (int t = 0; t < R; ++t) {
+                if (t & dt) continue;
+                const int j = o + (t & (dt - 1)) * half0;                  // position within the half of level s + l
+                cx<T> w = ldg(gtw + (long)j * (n >> (s + l)));              // w_{2^(s+l)}^j from the order-n table
+                if (sign < 0) w = conj(w);
+                const cx<T> a = v[t], bq = cmul(v[t + dt], w);
+                v[t] = a + bq;
+                v[t + dt] = a - bq;
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < R; ++t) S[(base + t * half0) * PITCH + c] = v[t];
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // unpadded N-grid transforms for ns_set_initial / ns_get_fields / the physical-space statistics (NOT on the hot path):
 // a shared-memory FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place, n = 2^a or 3 * 2^a.
@@ -315,27 +349,26 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int nsub, int axis, 
         const cx<T> w = ldg(gtw + j);
         return sign > 0 ? w : conj(w);
     };
-    // load: element j = nsub r + q goes to q m + bitrev_m(r)
+    // load: element j = nsub r + q goes to q m + bitrev_m(r); asynchronous copies (LDGSTS), so that all of a thread's loads
+    // are in flight at once without holding registers
     for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {
         int j, c;
         if (axis == 2) { j = e % n; c = e / n; } else { c = e % TL; j = e / TL; }
         const int q = j % nsub, r = j / nsub;
         const int rr = log2m == 0 ? 0 : (int)(__brev((unsigned)r) >> (32 - log2m));
-        S[(q * m + rr) * PITCH + c] = base[line_base(l0 + c) + (long)j * es];
+        __pipeline_memcpy_async(&S[(q * m + rr) * PITCH + c], &base[line_base(l0 + c) + (long)j * es], sizeof(cx<T>));
     }
+    __pipeline_commit();
+    __pipeline_wait_prior(0);
     __syncthreads();
-    for (int s = 1; s <= log2m; ++s) {
-        const int half = 1 << (s - 1);
-        for (int e = threadIdx.x; e < (n / 2) * TL; e += blockDim.x) {
-            const int c = e % TL, bf = e / TL;
-            const int j = bf & (half - 1);
-            const int i0 = ((bf >> (s - 1)) << s) + j;
-            const cx<T> w = root(j * (n >> s));          // w_{2^s}^j
-            const cx<T> a = S[i0 * PITCH + c];
-            const cx<T> bq = cmul(S[(i0 + half) * PITCH + c], w);
-            S[i0 * PITCH + c] = a + bq;
-            S[(i0 + half) * PITCH + c] = a - bq;
-        }
+    // radix-2 decimation-in-time levels 1..log2m, up to three levels per pass in registers (one barrier and one trip through
+    // shared memory per pass instead of per level)
+    for (int s = 1; s <= log2m;) {
+        const int G = log2m - s + 1 >= 3 ? 3 : log2m - s + 1;
+        if (G == 3) generic_dit_pass<T, 3>(S, s, n, sign, gtw);
+        else if (G == 2) generic_dit_pass<T, 2>(S, s, n, sign, gtw);
+        else generic_dit_pass<T, 1>(S, s, n, sign, gtw);
+        s += G;
         __syncthreads();
     }
     if (nsub == 3) {

@@ -112,7 +112,7 @@ static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, 
     return cudaGetLastError();
 }
 
-// ---- persistent TMA-fed forward column kernel (kernels_colring.cuh), fp64 L = 256
+// ---- persistent TMA-fed forward column kernel (kernels_colring.cuh), L = 256
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link dependency on libcuda)
 typedef CUresult (*ns_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                        const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -142,7 +142,7 @@ static cudaError_t col_tensor_map(CUtensorMap* m, const cx<T>* in, long ncols, l
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
-// stages of the input ring / CTAs per SM: L = 256: 2 x 96 KB, one CTA of 13 warps per SM
+// stages of the input ring / CTAs per SM: L = 256: 2 x 96 KB, one CTA of 13 (fp64) / 25 (fp32) warps per SM
 template <int L> struct RingCfg { static constexpr int STAGES = 2, MINB = 1; };
 
 template <typename T, int L>
@@ -319,12 +319,9 @@ cudaError_t NS_FAM(launch_col_fwd)(cudaStream_t st, int num_sms, int L, const cx
     const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
     const bool pf = col_pf_on(true, L, istride * (long)sizeof(cx<T>));
 #ifndef NS_FAMILY_SMOOTH
-    // fp64 long lines: the persistent TMA-fed kernel (measured: a5 3.65 -> 3.20 ms, a6 2.67 -> 2.52 ms at 512^3)
-    if constexpr (sizeof(T) == 8) {
-        if (L == 256) return col_fwd_ring_L<T, 256>(st, num_sms, in, out, ncols, g, scale, tw);
-    }
+    // long lines: the persistent TMA-fed kernel (measured at 512^3: fp64 a5 3.65 -> 3.20 ms, a6 2.67 -> 2.52 ms; fp32 1.96 -> 1.84, 1.40 -> 1.24)
+    if (L == 256) return col_fwd_ring_L<T, 256>(st, num_sms, in, out, ncols, g, scale, tw);
     if (L == 128) return pf ? col_fwd_tmem_L<T, 128, true>(st, in, out, g, scale, tw) : col_fwd_tmem_L<T, 128, false>(st, in, out, g, scale, tw);
-    if (L == 256) return pf ? col_fwd_tmem_L<T, 256, true>(st, in, out, g, scale, tw) : col_fwd_tmem_L<T, 256, false>(st, in, out, g, scale, tw);
 #endif
 #define CALL(LL) (pf ? col_fwd_L<T, LL, true>(st, in, out, g, scale, tw) : col_fwd_L<T, LL, false>(st, in, out, g, scale, tw))
     NS_DISPATCH_L(L, CALL)
