@@ -18,8 +18,6 @@ SOURCES = ["ns_solver.cu", "ns2d_solver.cu", "ns_fft_f64.cu", "ns_fft_f32.cu", "
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "--fmad=true"]
-# A/B builds (never used for the committed library): NS_BUILD_DEFINES="NS_DEV_SWITCHES ..." adds -D flags
-FLAGS += ["-D" + d for d in os.environ.get("NS_BUILD_DEFINES", "").split()]
 
 
 def _newest_source() -> float:

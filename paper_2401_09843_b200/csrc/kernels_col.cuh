@@ -37,7 +37,7 @@ template <int R1, int R2> struct ColP { static constexpr int value = R1 > R2 ? R
 // L2 prefetch of the input rows of a LATER tile (the one this SM will work on a few CTAs from now), issued while the
 // current tile is in its butterflies: one tile per CTA and blocking loads leave HBM idle during the compute phases
 // (ncu: DRAM 59-70 % busy, stalls = global-load latency); the prefetch keeps requests in flight.  `rows` input rows of
-// 128 bytes; thread `tid` of `nthreads` takes every nthreads-th row.  Measured (profiles/r02_notes.md): it pays for the
+// 128 bytes; thread `tid` of `nthreads` takes every nthreads-th row.  Measured: it pays for the
 // short lines (L = 64: a5 1.68 -> 1.52 ms, a6 1.15 -> 1.01 ms at 32 x 128^3) and loses for L = 256, so PF is a template flag.
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 template <typename T>

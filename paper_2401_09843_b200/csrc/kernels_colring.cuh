@@ -25,8 +25,7 @@
 
 #include "cx.cuh"
 #include "kernels_col.cuh"
-#include "kernels_zfused.cuh"   // mbarrier helpers
-#include "kernels_zfused8.cuh"  // named_bar_sync
+#include "kernels_zfused.cuh"   // mbarrier helpers, named_bar_sync
 #include "tmem.cuh"
 
 namespace ns {

@@ -1,7 +1,7 @@
 // kernels_z.cuh -- mathematics shared by the contiguous-axis (z) kernels: step a3 (pad + inverse c2r +
 // products + max|u|) and step a4 (forward r2c + truncate) of SURVEY.md section 8(a); Algorithm 2 steps 2-5
 // and Algorithm 3 steps 4-5 of the paper (symmetric flux per PAPER.md:L245).
-// The kernels themselves are in kernels_zfused.cuh / kernels_zfused8.cuh (a3 and a4 fused).
+// The kernels themselves are in kernels_zfused.cuh / kernels_zpair.cuh (a3 and a4 fused).
 //
 // Real transforms use the two-for-one trick on the same pruned radix-3 core as kernels_col.cuh:
 //   inverse  z = u_a + i u_b  has spectrum Z[k] = U_a[k] + i U_b[k]; for k < 0, U[k] = conj(U[-k]), so

@@ -40,6 +40,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     } while (!done);
 }
 
+// named barrier among `nthreads` threads of the CTA (a unit / a team), id 1..15
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 // s_q[n] = (a + c w3^{-q}) W^{qn}
 template <typename T>
 __device__ __forceinline__ cx<T> prune3(cx<T> a, cx<T> c, int q, int n, const Twiddles<T>& tw) {

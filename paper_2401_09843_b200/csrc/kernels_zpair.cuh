@@ -29,8 +29,7 @@
 #include <cstdint>
 
 #include "cx.cuh"
-#include "kernels_zfused.cuh"   // mbarrier / bulk-copy helpers, prune3
-#include "kernels_zfused8.cuh"  // named_bar_sync
+#include "kernels_zfused.cuh"   // mbarrier / bulk-copy helpers, named_bar_sync, prune3
 #include "tmem.cuh"
 
 namespace ns {

@@ -4,11 +4,8 @@
 #include "kernels_colring.cuh"
 #include "kernels_z.cuh"
 #include "kernels_zfused.cuh"
-#include "kernels_zfused8.cuh"
 #include "kernels_zpair.cuh"
 #include "kernels_y2d.cuh"
-#include <cstdlib>
-#include <cstring>
 #include "ns_internal.h"
 
 namespace ns {
@@ -185,31 +182,6 @@ static cudaError_t z_fused_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T
     return cudaGetLastError();
 }
 
-// warp-synchronous fused z kernel for L >= 64
-template <int L> struct Z8Cfg;
-template <> struct Z8Cfg<64>  { static constexpr int LPB = 8, MINB = 2; };
-
-template <typename T, int L>
-static cudaError_t z_fused8_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
-                              Twiddles<T> tw) {
-    constexpr int LPB = Z8Cfg<L>::LPB;
-    constexpr int G = L / 8, R3 = G / 8;
-    auto k = z_fused8_kernel<T, L, LPB, Z8Cfg<L>::MINB>;
-    const size_t smem = (size_t)LPB * 3 * (L + Z8Geo<R3>::SZ) * sizeof(cx<T>) + (size_t)LPB * 8 + 8;
-    cudaError_t e = set_smem(k, smem);
-    if (e != cudaSuccess) return e;
-    if ((MM % LPB) != 0) return cudaErrorInvalidValue;
-    const long lines = MM * batch;
-    int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 3 * G * LPB, smem);
-    if (e != cudaSuccess) return e;
-    if (occ < 1) occ = 1;
-    long grid = (long)num_sms * occ;
-    if (grid > lines / LPB) grid = lines / LPB;
-    k<<<(unsigned)grid, 3 * G * LPB, smem, st>>>(in, out, MM, lines, umax2, tw);
-    return cudaGetLastError();
-}
-
 // line-pair fused z kernel (kernels_zpair.cuh), L in {64, 128, 256}: one persistent block of UNITS units per SM slot
 template <typename T, int L>
 static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long MM, long batch, unsigned long long* umax2,
@@ -269,17 +241,11 @@ static cudaError_t z_pair_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>
 
 // L2 prefetch distance of the column passes in tiles (kernels_col.cuh): the CTAs resident on the GPU (2-3 per SM)
 static int col_pf_dist(int num_sms, int L) {
-#ifdef NS_DEV_SWITCHES
-    if (const char* v = getenv("NS_COLPF")) return atoi(v) * num_sms;
-#endif
     return (L <= 64 ? 2 : 1) * num_sms;
 }
-// which passes prefetch: measured per length (profiles/r02_notes.md): it pays up to L = 128; at L = 256 only for the inverse
+// which passes prefetch: measured per length: it pays up to L = 128; at L = 256 only for the inverse
 // pass along y (a2 2.13 -> 1.93 ms at 512^3) -- along x every row of a tile lies in another 2 MB page and the extra requests lose
 static bool col_pf_on(bool fwd, int L, long row_stride_bytes) {
-#ifdef NS_DEV_SWITCHES
-    if (const char* v = getenv(fwd ? "NS_COLPF_FWD" : "NS_COLPF_INV")) return atoi(v) != 0;
-#endif
     if (L <= 128) return true;
     return !fwd && L == 256 && row_stride_bytes < (1L << 16);
 }
@@ -340,12 +306,7 @@ cudaError_t NS_FAM(launch_z_fused)(cudaStream_t st, int num_sms, int L, const cx
     switch (L) {
         case 256: return z_pair_L<T, 256>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 128: return z_pair_L<T, 128>(st, num_sms, in, out, MM, batch, umax2, tw);
-#ifdef NS_DEV_SWITCHES   // A/B builds only (never defined by paper_2401_09843_b200/build.py)
-        case 64: return getenv("NS_Z64") && !strcmp(getenv("NS_Z64"), "8") ? z_fused8_L<T, 64>(st, num_sms, in, out, MM, batch, umax2, tw)
-                                                                            : z_pair_L<T, 64>(st, num_sms, in, out, MM, batch, umax2, tw);
-#else
         case 64: return z_pair_L<T, 64>(st, num_sms, in, out, MM, batch, umax2, tw);
-#endif
         // short lines: block-synchronous kernel
         case 8: return z_fused_L<T, 8>(st, num_sms, in, out, MM, batch, umax2, tw);
         case 16: return z_fused_L<T, 16>(st, num_sms, in, out, MM, batch, umax2, tw);

@@ -19,11 +19,6 @@ struct Twiddles {
     const cx<T>* twB;
     const cx<T>* w3a;
     const cx<T>* w3b;
-    // tables of the 8-values-per-lane z kernel (kernels_zfused8.cuh), G = L/8, R3 = G/8 (L >= 64 only):
-    //   z8A[r1*G + t] = w_L^{r1 t},  z8B[ta*G + t] = w_L^{(t/R3)(R3 ta + t%R3)},  z8C[rA*R3 + tb] = w_G^{rA tb}
-    const cx<T>* z8A;
-    const cx<T>* z8B;
-    const cx<T>* z8C;
     // table of the 16-values-per-lane z kernel (kernels_zpair.cuh), G = L/16 (L >= 64 only):
     //   z16[r1*G + t] = w_L^{r1 t},  r1 < 16, t < G
     const cx<T>* z16;

@@ -8,8 +8,7 @@
 
 namespace ns {
 
-// Block layout (complex entries): twA [0,L) twB [L,2L) w3a [2L,3L) w3b [3L,4L) z8A [4L,5L) z8B [5L,6L)
-// z8C [6L,7L) z16 [7L,8L) gN [8L,10L).
+// Block layout (complex entries): twA [0,L) twB [L,2L) w3a [2L,3L) w3b [3L,4L) (unused [4L,7L)) z16 [7L,8L) gN [8L,10L).
 template <typename T>
 inline std::vector<cx<T>> build_twiddle_block(int L) {
     const long double twopi = 6.283185307179586476925286766559005768L;
@@ -35,16 +34,6 @@ inline std::vector<cx<T>> build_twiddle_block(int L) {
     }
     for (int j = 0; j < 2 * L; ++j) h[(size_t)8 * L + j] = root(j, 2L * L);   // exp(2 pi i j / N), N = 2L
     if (L >= 64 && (L & (L - 1)) == 0) {
-        const int G = L / 8, R3 = G / 8;
-        for (int k = 0; k < 8; ++k)
-            for (int t = 0; t < G; ++t) {
-                h[(size_t)4 * L + (size_t)k * G + t] = root((long)k * t, L);
-                h[(size_t)5 * L + (size_t)k * G + t] = root((long)(t / R3) * (R3 * k + t % R3), L);
-            }
-        for (int rA = 0; rA < 8; ++rA)
-            for (int tb = 0; tb < R3; ++tb) h[(size_t)6 * L + (size_t)rA * R3 + tb] = root((long)rA * tb, G);
-    }
-    if (L >= 64 && (L & (L - 1)) == 0) {
         const int G = L / 16;
         for (int r1 = 0; r1 < 16; ++r1)
             for (int t = 0; t < G; ++t) h[(size_t)7 * L + (size_t)r1 * G + t] = root((long)r1 * t, L);
@@ -59,9 +48,6 @@ inline Twiddles<T> make_twiddles(const cx<T>* base, int L) {
     t.twB = base + L;
     t.w3a = base + 2 * (size_t)L;
     t.w3b = base + 3 * (size_t)L;
-    t.z8A = base + 4 * (size_t)L;
-    t.z8B = base + 5 * (size_t)L;
-    t.z8C = base + 6 * (size_t)L;
     t.z16 = base + 7 * (size_t)L;
     t.gN = base + 8 * (size_t)L;
     return t;
