@@ -28,7 +28,7 @@ __device__ __forceinline__ int wavenum(int i, int N) { return i < N / 2 ? i : i 
 //   not __restrict__; every thread reads its own entries of Us / Un before it writes the same entries of out.
 // ------------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, int kmax, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
                 T gamma, const double* __restrict__ dt, int mode) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -49,9 +49,15 @@ spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, 
     const bool dead = (kxi >= kmax) || (kxi <= -kmax) || (kyi >= kmax) || (kyi <= -kmax) || (iz >= kmax) || (k2i == 0);
 
     cx<T> R[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
-    cx<T> u[3];
+    cx<T> u[3], un3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) u[c] = us[c * plane];
+    // the second state of stages 2, 3 is fetched together with everything else (one round trip to HBM instead of two)
+    const cx<T>* un = (mode != 0 && Un) ? Un + b * 3 * plane + o : nullptr;
+    if (un) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) un3[c] = un[c * plane];
+    }
     if (!dead) {
         const cx<T>* bp = Bh + b * NS_NFLUX * plane + o;
         const cx<T> B11 = ldg(bp), B12 = ldg(bp + plane), B13 = ldg(bp + 2 * plane), B22 = ldg(bp + 3 * plane),
@@ -81,12 +87,11 @@ spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, 
         return;
     }
     const T dtb = (T)dt[b];
-    const cx<T>* un = Un ? Un + b * 3 * plane + o : nullptr;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         cx<T> r;
         if (un) {
-            const cx<T> n = un[c * plane];
+            const cx<T> n = un3[c];
             if (dtb == (T)0) r = n;
             else r = mk<T>(alpha * n.x + beta * u[c].x + gamma * dtb * R[c].x, alpha * n.y + beta * u[c].y + gamma * dtb * R[c].y);
         } else {

@@ -137,6 +137,7 @@ public:
     unsigned long long* umax2 = nullptr;
     int* bad_dev = nullptr;   // per-sample flag: non-finite state seen (kernels_misc.cuh)
     size_t nS, nX, nY, nZ;  // complex element counts of state, X, Y, Z
+    long XS = 0;            // pitch of one px row of X (a1 out / a5 out), complex elements
     size_t red_count;
     PassProfiler prof;
     // two-stream software pipeline over groups of samples (ns_set_pipeline): the fused z kernel (fp64-issue / shared-memory
@@ -220,7 +221,8 @@ public:
         nS = b * 3 * N * N * H;
         // Workspaces shared by all passes: X <- a1 out / a5 out / unpadded-FFT cube / R,
         // Y <- a2 out / a6 out (B_hat) / host staging, Z <- fused-z out.
-        nX = b * NS_NFLUX * (size_t)M * N * H;            // A1b; >= A1u (3 M N H), W (3 N^3 = 6 N^2 H), R (3 N^2 H)
+        XS = (long)N * H;                                 // row (px) pitch of the X workspace (padding it was measured: no gain)
+        nX = b * NS_NFLUX * (size_t)M * XS;               // A1b; >= A1u (3 M N H), W (3 N^3 = 6 N^2 H), R (3 N^2 H)
         nY = b * 3 * (size_t)M * M * H;                   // A2u; >= Bh (5 N^2 H), public / physical staging
         nZ = b * NS_NFLUX * (size_t)M * M * H;            // A2b
         const size_t pub = b * 3 * (size_t)Nu * Nu * (Nu / 2 + 1);
@@ -294,12 +296,12 @@ public:
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
         prof.tick(0, st);
-        e = launch_col_inv<T>(st, num_sms, L, Uin + (size_t)b0 * 3 * N * NH, X + (size_t)b0 * 3 * M * NH, NH, (long)nb * 3, NH, NH,
-                              (long)N * NH, (long)M * NH, tw());
+        e = launch_col_inv<T>(st, num_sms, L, Uin + (size_t)b0 * 3 * N * NH, X + (size_t)b0 * 3 * M * XS, NH, (long)nb * 3, NH, XS,
+                              (long)N * NH, (long)M * XS, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a1 col_inv x");
         ++launches;
         prof.tick(1, st);
-        e = launch_col_inv<T>(st, num_sms, L, X + (size_t)b0 * 3 * M * NH, Y + (size_t)b0 * 3 * M * MH, H, (long)nb * 3 * M, H, H, NH, MH, tw());
+        e = launch_col_inv<T>(st, num_sms, L, X + (size_t)b0 * 3 * M * XS, Y + (size_t)b0 * 3 * M * MH, H, (long)nb * 3 * M, H, H, XS, MH, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a2 col_inv y");
         ++launches;
         return NS_OK;
@@ -317,13 +319,13 @@ public:
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
         prof.tick(4, st);
-        e = launch_col_fwd<T>(st, num_sms, L, Z + (size_t)b0 * NS_NFLUX * M * MH, X + (size_t)b0 * NS_NFLUX * M * NH, H,
-                              (long)nb * NS_NFLUX * M, H, H, MH, NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, num_sms, L, Z + (size_t)b0 * NS_NFLUX * M * MH, X + (size_t)b0 * NS_NFLUX * M * XS, H,
+                              (long)nb * NS_NFLUX * M, H, H, MH, XS, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a5 col_fwd y");
         ++launches;
         prof.tick(5, st);
-        e = launch_col_fwd<T>(st, num_sms, L, X + (size_t)b0 * NS_NFLUX * M * NH, Y + (size_t)b0 * NS_NFLUX * N * NH, NH, (long)nb * NS_NFLUX,
-                              NH, NH, (long)M * NH, (long)N * NH, (T)1, tw());
+        e = launch_col_fwd<T>(st, num_sms, L, X + (size_t)b0 * NS_NFLUX * M * XS, Y + (size_t)b0 * NS_NFLUX * N * NH, NH, (long)nb * NS_NFLUX,
+                              XS, NH, (long)M * XS, (long)N * NH, (T)1, tw());
         if (e != cudaSuccess) return cuda_fail(e, "a6 col_fwd x");
         ++launches;
         prof.tick(7, st);
