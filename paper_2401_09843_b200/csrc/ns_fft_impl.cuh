@@ -48,7 +48,7 @@ template <int L> struct Cfg {
         return L == 24 ? 8 : (L % 3 == 0 ? (L >= 192 ? 2 : 4) : 192 / (3 * P));
     }
     // target CTAs per SM of the fused z kernel (bounds its registers)
-    static constexpr int minbf() { return 2; }
+    static constexpr int minbf() { return (L >= 160 && (L & (L - 1)) != 0) ? 4 : 2; }
 };
 
 template <typename K>
