@@ -161,16 +161,6 @@ int ns_ensemble_moments(ns_solver* h, void* mean_out, void* var_out, ns_memspace
 
 /* Simulation time of one sample; NaN if `sample` is out of range. */
 double ns_time(const ns_solver* h, int sample);
-/* Two-stream software pipeline over groups of samples (Algorithm 1: the samples of an ensemble are
- * independent).  With groups > 1 every RK stage processes the batch in `groups` groups of batch / groups samples: the fused
- * z kernel (a3 + a4; bound by fp64 issue and shared memory, HBM a third busy) of one group runs on an internal high-priority
- * stream with its persistent grid limited to `z_sms` SMs, while the column and spectral passes (HBM bound) of the other
- * groups run on the handle's stream on the remaining SMs.  Results are bit-identical to groups = 1.  groups must divide
- * batch (1..16); z_sms = 0 means all SMs.  Default after ns_create: groups = 1 (one stream, the order a1..a7).  All work is
- * still ordered on the handle's stream as seen from outside.  The per-pass profiler (ns_profile) forces groups = 1 while
- * enabled.  Synchronises the stream. */
-int ns_set_pipeline(ns_solver* h, int groups, int z_sms);
-
 /* Per-pass timing with CUDA events recorded on the solver's stream between the kernels of the RHS
  * (measurement aid for bench.py; adds one event record per kernel when enabled).  ns_profile(h, 1)
  * synchronises, clears the accumulators and enables; ns_profile(h, 0) disables.  ns_profile_read

@@ -22,7 +22,7 @@ NS_OK, NS_ERR_INVALID_ARG, NS_ERR_OOM, NS_ERR_CUDA, NS_ERR_STATE, NS_ERR_NONFINI
 EXPORTS = [
     "ns_create", "ns_destroy", "ns_set_initial", "ns_set_spectral", "ns_get_spectral", "ns_rhs", "ns_step",
     "ns_step_cfl", "ns_step_dts", "ns_advance", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
-    "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_set_pipeline", "ns_autotune", "ns_transform_grid", "ns_padded_size", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
+    "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_autotune", "ns_transform_grid", "ns_padded_size", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
 # include/ns2d.h: the two-dimensional solver
 EXPORTS_2D = [
@@ -72,7 +72,6 @@ def lib():
         L.ns_structure_function.argtypes = [vp, vp, i]
         L.ns_structure_function_p.argtypes = [vp, d, vp, i]
         L.ns_ensemble_moments.argtypes = [vp, vp, vp, i]
-        L.ns_set_pipeline.argtypes = [vp, i, i]
         L.ns_autotune.argtypes = [i, i, i, vp, vp, ctypes.POINTER(ctypes.c_int)]
         L.ns_transform_grid.argtypes = [vp]
         L.ns_padded_size.argtypes = [vp]
@@ -301,10 +300,6 @@ class Solver:
     def padded_size(self):
         """ns_padded_size: M = 3 Nt / 2, the padded grid max|u| is taken over."""
         return int(lib().ns_padded_size(self._h))
-
-    def set_pipeline(self, groups=1, z_sms=0):
-        """ns_set_pipeline: process the batch in `groups` groups, the z kernel of a group on its own stream and `z_sms` SMs."""
-        self._check(lib().ns_set_pipeline(self._h, int(groups), int(z_sms)))
 
     def profile(self, enable=True):
         self._check(lib().ns_profile(self._h, 1 if enable else 0))

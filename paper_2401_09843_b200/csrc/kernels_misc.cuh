@@ -320,7 +320,7 @@ __device__ __forceinline__ void generic_dit_pass(cx<T>* __restrict__ S, int s, i
 
 // ------------------------------------------------------------------------------------------------
 // unpadded N-grid transforms for ns_set_initial / ns_get_fields / the physical-space statistics (NOT on the hot path):
-// a shared-memory FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place, n = 2^a or 3 * 2^a.
+// a shared-memory FFT on tiles of 8 lines of a full complex [cubes][n][n][n] array, in place, n = p 2^a with p in {1, 3, 5, 7, 15}.
 //   axis 0: element stride n*n, axis 1: n, axis 2: 1.  dim = 2: the same on [planes][n][n] (axes 1 and 2).
 // n = p m, p in {3, 5, 7, 15}: the p decimated sequences x[p r + q] are transformed by radix-2 stages (m = 2^a) and combined by
 // one radix-p stage, X[k + m t] = sum_q w_n^{q (k + m t)} F_q[k].  Twiddles come from the table gtw[j] = exp(+2 pi i j / n).

@@ -38,7 +38,6 @@ struct ns_solver {
     virtual int ensemble_moments(void* mean, void* var, ns_memspace ms) = 0;
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
-    virtual int set_pipeline(int groups, int z_sms) = 0;
     virtual int padded_size() const = 0;
     virtual int transform_grid() const = 0;
     virtual int time_transform(int reps, double* ms) = 0;
@@ -140,23 +139,10 @@ public:
     long XS = 0;            // pitch of one px row of X (a1 out / a5 out), complex elements
     size_t red_count;
     PassProfiler prof;
-    // two-stream software pipeline over groups of samples (ns_set_pipeline): the fused z kernel (fp64-issue / shared-memory
-    // bound, DRAM a third busy) of one group runs on its own high-priority stream and a subset of the SMs while the column and
-    // spectral passes (DRAM bound, fp64 a third busy) of the other groups run on the solver's stream on the remaining SMs.
-    static constexpr int MAX_GROUPS = 16;
-    int groups = 1, z_sms = 0;
-    cudaStream_t st_z = nullptr;
-    cudaEvent_t ev_inv[MAX_GROUPS] = {}, ev_z[MAX_GROUPS] = {};
-
     Solver(int Nu_, int N_, int batch_, const ns_params& p, cudaStream_t s)
         : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), Nu(Nu_), prm(p), st(s) {}
     ~Solver() override {
         if (arena) cudaFree(arena);
-        if (st_z) cudaStreamDestroy(st_z);
-        for (int g = 0; g < MAX_GROUPS; ++g) {
-            if (ev_inv[g]) cudaEventDestroy(ev_inv[g]);
-            if (ev_z[g]) cudaEventDestroy(ev_z[g]);
-        }
     }
 
     int fail(int code, const std::string& msg) {
@@ -190,24 +176,6 @@ public:
                 snprintf(buf, sizeof buf, "sample %d: the velocity field is not finite (NaN or inf); the sample is frozen", b);
                 return fail(NS_ERR_NONFINITE, buf);
             }
-        return NS_OK;
-    }
-
-    int set_pipeline(int groups_, int z_sms_) override {
-        if (groups_ < 1 || groups_ > MAX_GROUPS || batch % groups_ != 0) return fail(NS_ERR_INVALID_ARG, "groups must divide batch (1..16)");
-        if (z_sms_ < 0 || z_sms_ > num_sms) return fail(NS_ERR_INVALID_ARG, "z_sms must be in [0, SM count]");
-        NS_CK(cudaStreamSynchronize(st));
-        if (groups_ > 1 && !st_z) {
-            int lo = 0, hi = 0;
-            NS_CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-            NS_CK(cudaStreamCreateWithPriority(&st_z, cudaStreamNonBlocking, hi));
-        }
-        for (int g = 0; g < groups_; ++g) {
-            if (!ev_inv[g]) NS_CK(cudaEventCreateWithFlags(&ev_inv[g], cudaEventDisableTiming));
-            if (!ev_z[g]) NS_CK(cudaEventCreateWithFlags(&ev_z[g], cudaEventDisableTiming));
-        }
-        groups = groups_;
-        z_sms = z_sms_ == 0 ? num_sms : z_sms_;
         return NS_OK;
     }
 
@@ -289,9 +257,7 @@ public:
     // ---------------------------------------------------------------- RHS transform pipeline a1..a6
     // Every pass works on the samples [b0, b0 + nb) of the batch; workspaces are indexed by sample, so groups of samples use
     // disjoint ranges of X / Y / Z within a pass.  X holds 3 (a1 out) or 5 (a5 out) components per sample and Y 3 padded
-    // (a2 out) or 5 truncated (a6 out): a forward pass of one group may overwrite the inverse-pass output of ANOTHER group
-    // (a5 of group g touches the a1 range of groups h > g), which is why stage_transform queues the inverse passes of all
-    // groups before the first forward pass.
+    // (a2 out) or 5 truncated (a6 out).
     int pass_inverse(const cx<T>* Uin, int b0, int nb) {
         const long NH = (long)N * H, MH = (long)M * H;
         cudaError_t e;
@@ -354,32 +320,13 @@ public:
         return NS_OK;
     }
 
-    // One RK stage = transform + tail (time-step bookkeeping in stage 1, then a7).  With groups > 1 (ns_set_pipeline) and the
-    // per-pass profiler off, the samples are processed in `groups` groups: the inverse passes of all groups are queued on the
-    // solver's stream, each followed by an event that releases the group's z kernel on the z stream (grid limited to z_sms
-    // SMs); the forward passes and the tail of a group wait for its z kernel.  Every kernel sees exactly the data it sees
-    // in the single-stream order, so the result is bit-identical.
+    // One RK stage = transform + tail (time-step bookkeeping in stage 1, then a7).  A two-stream variant that ran the z kernel of
+    // one group of samples beside the column passes of the others was measured and gained nothing (profiles/r02_experiments.md).
     template <typename Tail>
     int stage(const cx<T>* Uin, bool want_umax, Tail tail) {
-        int rc;
-        if (groups <= 1 || prof.on) {
-            if ((rc = transform(Uin, want_umax)) != NS_OK) return rc;
-            return tail(0, batch);
-        }
-        const int nb = batch / groups;
-        for (int g = 0; g < groups; ++g) {
-            if ((rc = pass_inverse(Uin, g * nb, nb)) != NS_OK) return rc;
-            NS_CK(cudaEventRecord(ev_inv[g], st));
-            NS_CK(cudaStreamWaitEvent(st_z, ev_inv[g], 0));
-            if ((rc = pass_z(st_z, z_sms, g * nb, nb, want_umax)) != NS_OK) return rc;
-            NS_CK(cudaEventRecord(ev_z[g], st_z));
-        }
-        for (int g = 0; g < groups; ++g) {
-            NS_CK(cudaStreamWaitEvent(st, ev_z[g], 0));
-            if ((rc = pass_forward(g * nb, nb)) != NS_OK) return rc;
-            if ((rc = tail(g * nb, nb)) != NS_OK) return rc;
-        }
-        return NS_OK;
+        int rc = transform(Uin, want_umax);
+        if (rc != NS_OK) return rc;
+        return tail(0, batch);
     }
 
     // dt_dev / t_dev must have been set before the first spectral() of the step (stream order)
@@ -880,7 +827,6 @@ double ns_time(const ns_solver* h, int sample) {
     if (!h) return std::numeric_limits<double>::quiet_NaN();
     return const_cast<ns_solver*>(h)->time(sample);
 }
-int ns_set_pipeline(ns_solver* h, int groups, int z_sms) { NS_H(h); return h->set_pipeline(groups, z_sms); }
 int ns_profile(ns_solver* h, int enable) { NS_H(h); return h->profile(enable); }
 int ns_profile_read(ns_solver* h, double* ms, long long* cnt) { NS_H(h); return h->profile_read(ms, cnt); }
 int ns_transform_grid(const ns_solver* h) { return h ? h->transform_grid() : 0; }

@@ -219,36 +219,6 @@ def test_two_handles_on_two_streams(ns):
     assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1])
 
 
-def test_pipeline_groups_bit_identical(ns):
-    """ns_set_pipeline: the two-stream software pipeline over groups of samples (z kernel of one group on its own stream and a
-    subset of the SMs, column / spectral passes of the other groups on the handle's stream) gives bit for bit the state of the
-    single-stream order, for CFL steps, uniform steps and replayed steps; a second handle stays independent; bad arguments."""
-    N, B = 64, 8
-    us = np.stack([field(N, 900 + i) * (1.0 + 0.1 * i) for i in range(B)])
-    kw = dict(nu=0.002, eps=0.05, s=1.0)
-    ref = ns.Solver(N, batch=B, **kw)
-    ref.set_initial(us)
-    dts = [ref.step_cfl(0.2, 1e9) for _ in range(3)]
-    ref.step(1e-3)
-    want = ref.get_spectral()
-    for groups, z_sms in [(2, 0), (4, 100), (8, 64)]:
-        s = ns.Solver(N, batch=B, **kw)
-        s.set_pipeline(groups, z_sms)
-        s.set_initial(us)
-        for i in range(3):
-            got_dt = s.step_cfl(0.2, 1e9) if i != 1 else (s.step_dts(dts[1]), dts[1])[1]
-            assert np.array_equal(got_dt, dts[i])
-        s.step(1e-3)
-        assert np.array_equal(s.get_spectral(), want), (groups, z_sms)
-        assert np.array_equal(s.rhs(), ref.rhs())
-        for b in range(B):
-            assert s.time(b) == ref.time(b)
-    with pytest.raises(ns.NSError):
-        ref.set_pipeline(3, 0)          # does not divide the batch
-    with pytest.raises(ns.NSError):
-        ref.set_pipeline(2, 100000)
-
-
 def test_advance_to_t_end(ns):
     """ns_advance == the host loop over ns_step_cfl it replaces, bit for bit, with every sample ending at t_end."""
     N, B, t_end = 32, 3, 0.05
