@@ -26,6 +26,15 @@ def k53_512():
 
 
 @pytest.fixture(scope="session")
+def k53_512_hat(k53_512):
+    """The spectral state of k53_512 by the numpy restatement of set_initial (tests/_sampling.py): the common input of the CUDA
+    path and the oracle at 512^3 -- no oracle input comes from the CUDA path."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from _sampling import spectral_state
+    return spectral_state(k53_512)
+
+
+@pytest.fixture(scope="session")
 def oracle2d():
     from oracle import ns2d_oracle
     return ns2d_oracle

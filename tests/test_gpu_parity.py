@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 from paper_2401_09843_b200 import inputs
+from _sampling import spectral_state
 
 pytestmark = pytest.mark.gpu
 
@@ -318,11 +319,11 @@ def test_config4_ensemble_two_samples(ns, oracle):
     Zs = s.enstrophy_spectrum(N)
     S = s.structure_function()
     for i in (31,):     # sample 1 is replayed for several steps in tests/test_gpu_schedule.py
-        uh = oracle.set_initial(N, us[i])
+        uh = oracle.set_initial(N, us[i])       # the oracle works on ITS OWN initial state (no input from the CUDA path)
         assert rel(u0[i], uh) < 1e-13
-        assert rel(r0[i], oracle.rhs(N, p, u0[i])) < TOL_RHS_F64
-        assert abs(dts[i] - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, u0[i])) < 1e-12 * dts[i]
-        un = oracle.step(N, p, u0[i], dts[i])
+        assert rel(r0[i], oracle.rhs(N, p, uh)) < TOL_RHS_F64
+        assert abs(dts[i] - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, uh)) < 1e-12 * dts[i]
+        un = oracle.step(N, p, uh, dts[i])
         assert rel(got[i], un) < TOL_STEPS_F64
         assert np.abs(E[i] - oracle.energy_spectrum(N, un, N)).max() < 1e-13
         Zo = oracle.enstrophy_spectrum(N, un, N)
@@ -425,16 +426,16 @@ def test_fp32_rhs_parity_128(ns, oracle):
 
 
 @pytest.mark.parametrize("N", [256, 512])
-def test_fp32_full_size_sampled(ns, oracle, k53_512, N):
+def test_fp32_full_size_sampled(ns, oracle, k53_512, k53_512_hat, N):
     """fp32 at the sizes that run the long-line kernels (L = 128, 256: 16 values per lane, tensor-memory parking):
     ns_rhs at sampled wavenumbers against the oracle's direct truncated convolution, the whole array against the
     fp64 CUDA result (itself checked against the oracle in test_full_size_sampled_rhs_and_step), and one RK3 step."""
     u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5) if N == 256 else k53_512
+    uh = spectral_state(u) if N == 256 else k53_512_hat        # numpy restatement of set_initial: the common input
     kw = dict(eps=0.05, s=1.0)
     s64 = ns.Solver(N, **kw)
-    s64.set_initial(u[None])
+    s64.set_spectral(uh[None])
     del u
-    uh = s64.get_spectral()[0]
     r64 = s64.rhs()[0]
     dt = 0.2 * (2 * np.pi / N) / s64.max_velocity()[0]
     s64.step(dt)

@@ -22,7 +22,7 @@ import numpy as np
 import pytest
 
 from paper_2401_09843_b200 import inputs
-from _sampling import stratified_modes
+from _sampling import spectral_state, stratified_modes
 
 pytestmark = pytest.mark.gpu
 
@@ -117,10 +117,7 @@ def test_config4_one_sample_replayed(ns, oracle):
     s.set_initial(us)
     uh = oracle.set_initial(N, us[pick])
     del us
-    u0 = s.get_spectral()
-    assert rel(u0[pick], uh) < 1e-13
-    uh = u0[pick].copy()
-    del u0
+    assert rel(s.get_spectral()[pick], uh) < 1e-13      # the oracle keeps ITS OWN initial state (no input from the CUDA path)
     p = oracle.Params(**kw)
     worst, nsteps = 0.0, 10 if FULL else 4
     for i in range(nsteps):
@@ -140,18 +137,20 @@ def test_config4_one_sample_replayed(ns, oracle):
 
 # ------------------------------------------------------------------------------------------------ config 5
 @pytest.mark.parametrize("N", [256, 512])
-def test_full_size_stratified_sampled_rhs(ns, oracle, k53_512, N):
+def test_full_size_stratified_sampled_rhs(ns, oracle, k53_512, k53_512_hat, N):
     """256^3 and 512^3 (configs[4] input), same launch configuration as bench.py: ns_rhs at >= 512 stratified sampled
     wavenumbers against the oracle's direct truncated convolution sum (orc_rhs_at_modes): relative L2 over the sample
     <= 1e-12 and every single sampled entry within 1e-12 of max|R|; then, on the WHOLE array, the energy identity P4
     of the inviscid RHS (a statement about every entry of the transforms: any aliasing or tile fault breaks it), the
     masks, and the fused RK3 step against eq. 2.6 assembled on the host from ns_rhs evaluations (pins the axpy of a7)."""
     u = inputs.gaussian_field(N, 256, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5) if N == 256 else k53_512
+    uh = spectral_state(u) if N == 256 else k53_512_hat        # numpy restatement of set_initial: the common input
     kw = dict(eps=0.05, s=1.0)
     s = ns.Solver(N, **kw)
     s.set_initial(u[None])
     del u
-    uh = s.get_spectral()[0]
+    assert rel(s.get_spectral()[0], uh) < 1e-13                # ns_set_initial at full size, every entry
+    s.set_spectral(uh[None])
     r = s.rhs()[0]
     del s
     rmax = np.abs(r).max()
@@ -234,10 +233,12 @@ def test_sizes_3x2a_192_full_and_384_sampled(ns, oracle):
     N = 192
     us = np.stack([inputs.taylor_green_3d_perturbed(N, 31), inputs.gaussian_field(N, 392, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)])
     kw = dict(eps=0.05, s=1.5)
+    uh = np.stack([spectral_state(u) for u in us])
     s = ns.Solver(N, batch=2, **kw)
     s.set_initial(us)
     del us
-    uh = s.get_spectral()
+    assert rel(s.get_spectral(), uh) < 1e-13
+    s.set_spectral(uh)
     r = s.rhs()
     um = s.max_velocity()
     for b in range(2) if FULL else (1,):
@@ -247,11 +248,13 @@ def test_sizes_3x2a_192_full_and_384_sampled(ns, oracle):
     del s, r, uh
     N = 384
     u = inputs.gaussian_field(N, 384, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    uh = spectral_state(u)
     kw = dict(eps=0.05, s=1.0)
     s = ns.Solver(N, **kw)
     s.set_initial(u[None])
     del u
-    uh = s.get_spectral()[0]
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    s.set_spectral(uh[None])
     r = s.rhs()[0]
     del s
     rmax = np.abs(r).max()
@@ -309,11 +312,13 @@ def test_sizes_5_7_15_full_array_rhs(ns, oracle, N):
     default run covers by sampled wavenumbers below): every stored entry of ns_rhs and max|u| against orc_rhs_parts; fp32
     (where N/2 is a multiple of 16) against the fp64 result."""
     u = inputs.taylor_green_3d_perturbed(N, 40 + N) + 0.3 * inputs.gaussian_field(N, 700 + N, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
+    uh = spectral_state(u)
     kw = dict(eps=0.05, s=1.5)
     s = ns.Solver(N, **kw)
     s.set_initial(u[None])
     del u
-    uh = s.get_spectral()[0]
+    assert rel(s.get_spectral()[0], uh) < 1e-13
+    s.set_spectral(uh[None])
     r = s.rhs()[0]
     want = oracle.rhs_parts(N, oracle.Params(**kw), uh)
     assert rel(r, want["r"]) < TOL_RHS_F64
@@ -331,18 +336,21 @@ def test_sizes_5_7_15_large_sampled(ns, oracle, N):
     """L = 112 = 14 x 8, 120 = 15 x 8 and the long-line members of the families (L = 160 = 10 x 16, 224 = 14 x 16, 240 = 15 x 16,
     320 = 20 x 16): stratified sampled
     wavenumbers of ns_rhs against the direct truncated convolution (relative L2 over the sample <= 1e-12), the masks, and the
-    energy identity P4 of the inviscid RHS on the whole array.  Full-band input: white noise on a shear profile, projected by
-    ns_set_initial (the state handed to the oracle is what ns_get_spectral returns)."""
+    energy identity P4 of the inviscid RHS on the whole array.  Full-band input: white noise on a shear profile; its spectral state
+    by the numpy restatement of set_initial is the common input of both sides (and ns_set_initial is checked against it)."""
     rng = np.random.default_rng(N)
     x = 2 * np.pi * np.arange(N) / N
     u = 0.3 * rng.standard_normal((3, N, N, N))
     u[0] += np.sin(x)[None, :, None] + 0.5 * np.cos(3 * x)[None, None, :]
     u[2] += np.cos(2 * x)[:, None, None]
+    uh = spectral_state(u)                # numpy restatement of set_initial: the common input of both sides
     kw = dict(eps=0.05, s=1.0)
     s = ns.Solver(N, **kw)
-    s.set_initial(u[None])
+    if N < 640:
+        s.set_initial(u[None])
+        assert rel(s.get_spectral()[0], uh) < 1e-13
     del u
-    uh = s.get_spectral()[0]
+    s.set_spectral(uh[None])
     r = s.rhs()[0]
     del s
     rmax = np.abs(r).max()
@@ -419,8 +427,8 @@ def test_autotune_records_the_transform_grid(ns, oracle):
     s = ns.Solver(N, eps=0.05)
     assert s.transform_grid == best and s.padded_size == 3 * best // 2
     u = inputs.gaussian_field(N, 77, lambda k: 1.0 / (1.0 + k) ** 2, e_tot=0.5)
-    s.set_initial(u[None])
-    uh = s.get_spectral()[0]
+    uh = spectral_state(u)
+    s.set_spectral(uh[None])
     want = oracle.rhs_parts(N, oracle.Params(eps=0.05), uh, s.padded_size)
     assert rel(s.rhs()[0], want["r"]) < TOL_RHS_F64
     assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
