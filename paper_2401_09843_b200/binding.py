@@ -24,6 +24,11 @@ EXPORTS = [
     "ns_step_cfl", "ns_step_dts", "ns_advance", "ns_max_velocity", "ns_get_fields", "ns_energy_spectrum", "ns_enstrophy_spectrum",
     "ns_structure_function", "ns_structure_function_p", "ns_ensemble_moments", "ns_autotune", "ns_transform_grid", "ns_padded_size", "ns_profile", "ns_profile_read", "ns_time", "ns_kernel_launches", "ns_device_bytes", "ns_last_error",
 ]
+# include/ns_mg.h: one sample over several devices
+EXPORTS_MG = [
+    "ns_mg_create", "ns_mg_destroy", "ns_mg_set_spectral", "ns_mg_get_spectral", "ns_mg_rhs", "ns_mg_step", "ns_mg_step_cfl",
+    "ns_mg_max_velocity", "ns_mg_time", "ns_mg_exchange_bytes", "ns_mg_kernel_launches", "ns_mg_device_bytes", "ns_mg_last_error",
+]
 # include/ns2d.h: the two-dimensional solver
 EXPORTS_2D = [
     "ns2d_create", "ns2d_destroy", "ns2d_set_initial", "ns2d_set_spectral", "ns2d_get_spectral", "ns2d_rhs", "ns2d_step", "ns2d_step_cfl",
@@ -107,6 +112,21 @@ def lib():
         L.ns2d_device_bytes.restype = ctypes.c_longlong
         L.ns2d_last_error.argtypes = [vp]
         L.ns2d_last_error.restype = ctypes.c_char_p
+        # include/ns_mg.h
+        L.ns_mg_create.argtypes = [ctypes.POINTER(vp), i, i, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ns_params), i]
+        L.ns_mg_destroy.argtypes = [vp]
+        for name in ("ns_mg_set_spectral", "ns_mg_get_spectral", "ns_mg_rhs"):
+            getattr(L, name).argtypes = [vp, vp]
+        L.ns_mg_max_velocity.argtypes = [vp, ctypes.POINTER(d)]
+        L.ns_mg_step.argtypes = [vp, d]
+        L.ns_mg_step_cfl.argtypes = [vp, d, d, ctypes.POINTER(d)]
+        L.ns_mg_time.argtypes = [vp]
+        L.ns_mg_time.restype = d
+        for name in ("ns_mg_exchange_bytes", "ns_mg_kernel_launches", "ns_mg_device_bytes"):
+            getattr(L, name).argtypes = [vp]
+            getattr(L, name).restype = ctypes.c_longlong
+        L.ns_mg_last_error.argtypes = [vp]
+        L.ns_mg_last_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -451,3 +471,74 @@ class Solver2D:
 
     def device_bytes(self):
         return int(lib().ns2d_device_bytes(self._h))
+
+
+class SolverMG:
+    """One sample over several devices (include/ns_mg.h): ky / px slab decomposition driven by one process.  `devices` may name
+    the same GPU more than once (the ranks then share it).  Spectral arrays are host numpy arrays [3][N][N][N/2+1]."""
+
+    def __init__(self, N, devices, nu=0.0, eps=0.0, s=1.0, m_cut=-1.0, q_exp=-1.0, q_sharp=0, dtype="f64"):
+        self.N, self.devices = int(N), [int(x) for x in devices]
+        self.dtype = {"f64": NS_F64, "f32": NS_F32, NS_F64: NS_F64, NS_F32: NS_F32}[dtype]
+        self.cplx = np.complex128 if self.dtype == NS_F64 else np.complex64
+        self.spectral_shape = (3, self.N, self.N, self.N // 2 + 1)
+        p = ns_params(nu, eps, s, m_cut, q_exp, q_sharp)
+        dev = (ctypes.c_int * len(self.devices))(*self.devices)
+        h = ctypes.c_void_p()
+        rc = lib().ns_mg_create(ctypes.byref(h), self.N, len(self.devices), dev, ctypes.byref(p), self.dtype)
+        if rc != NS_OK:
+            raise NSError(rc, lib().ns_mg_last_error(None).decode())
+        self._h = h
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().ns_mg_destroy(self._h)
+            self._h = None
+
+    def _check(self, rc):
+        if rc != NS_OK:
+            raise NSError(rc, lib().ns_mg_last_error(self._h).decode())
+
+    def _host(self, a):
+        a = np.ascontiguousarray(a, dtype=self.cplx)
+        assert a.shape == self.spectral_shape, (a.shape, self.spectral_shape)
+        return a
+
+    def set_spectral(self, u_hat):
+        a = self._host(u_hat)
+        self._check(lib().ns_mg_set_spectral(self._h, ctypes.c_void_p(a.ctypes.data)))
+
+    def get_spectral(self):
+        out = np.empty(self.spectral_shape, dtype=self.cplx)
+        self._check(lib().ns_mg_get_spectral(self._h, ctypes.c_void_p(out.ctypes.data)))
+        return out
+
+    def rhs(self):
+        out = np.empty(self.spectral_shape, dtype=self.cplx)
+        self._check(lib().ns_mg_rhs(self._h, ctypes.c_void_p(out.ctypes.data)))
+        return out
+
+    def step(self, dt):
+        self._check(lib().ns_mg_step(self._h, float(dt)))
+
+    def step_cfl(self, cfl, t_end, return_dt=True):
+        dt = ctypes.c_double(0.0)
+        self._check(lib().ns_mg_step_cfl(self._h, float(cfl), float(t_end), ctypes.byref(dt) if return_dt else None))
+        return dt.value if return_dt else None
+
+    def max_velocity(self):
+        v = ctypes.c_double(0.0)
+        self._check(lib().ns_mg_max_velocity(self._h, ctypes.byref(v)))
+        return v.value
+
+    def time(self):
+        return float(lib().ns_mg_time(self._h))
+
+    def exchange_bytes(self):
+        return int(lib().ns_mg_exchange_bytes(self._h))
+
+    def kernel_launches(self):
+        return int(lib().ns_mg_kernel_launches(self._h))
+
+    def device_bytes(self):
+        return int(lib().ns_mg_device_bytes(self._h))

@@ -30,19 +30,21 @@ __device__ __forceinline__ int wavenum(int i, int N) { return i < N / 2 ? i : i 
 template <typename T>
 __global__ void __launch_bounds__(256, 4)
 spectral_kernel(const cx<T>* __restrict__ Bh, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, int kmax, long total, const T* __restrict__ dtab, T scale, T alpha, T beta,
-                T gamma, const double* __restrict__ dt, int mode) {
+                T gamma, const double* __restrict__ dt, int mode, int Nyl, int iy0) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
+    // arrays [b][comp][N (kx)][Nyl (ky)][H]: the ky rows iy0 .. iy0 + Nyl - 1 of the grid (Nyl = N, iy0 = 0 except in the
+    // ky-slabs of the multi-device solver, ns_mg.h)
     const int H = N / 2;
     const int iz = (int)(idx % H);
-    const int iy = (int)((idx / H) % N);
-    const int ix = (int)((idx / ((long)H * N)) % N);
-    const long b = idx / ((long)H * N * N);
-    const long plane = (long)N * N * H;
-    const long o = ((long)ix * N + iy) * H + iz;
+    const int iyl = (int)((idx / H) % Nyl);
+    const int ix = (int)((idx / ((long)H * Nyl)) % N);
+    const long b = idx / ((long)H * Nyl * N);
+    const long plane = (long)N * Nyl * H;
+    const long o = ((long)ix * Nyl + iyl) * H + iz;
     const cx<T>* us = Us + b * 3 * plane + o;
     cx<T>* op = out + b * 3 * plane + o;
-    const int kxi = wavenum(ix, N), kyi = wavenum(iy, N);
+    const int kxi = wavenum(ix, N), kyi = wavenum(iy0 + iyl, N);
     const int k2i = kxi * kxi + kyi * kyi + iz * iz;
     // truncation P_N of eq. 2.1: modes with a wavenumber component >= kmax = (user N)/2 carry nothing (kmax = N/2 unless the
     // transform grid is larger than the user's grid, ns_create); k = 0: reading A8

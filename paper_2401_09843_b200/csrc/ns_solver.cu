@@ -314,7 +314,7 @@ public:
         prof.tick(6, st);
         spectral_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y + (size_t)b0 * NS_NFLUX * plane, Us + (size_t)b0 * 3 * plane,
                                                                     Un ? Un + (size_t)b0 * 3 * plane : nullptr, out + (size_t)b0 * 3 * plane, N,
-                                                                    Nu / 2, total, dtab, scale, (T)alpha, (T)beta, (T)gamma, dt_dev + b0, mode);
+                                                                    Nu / 2, total, dtab, scale, (T)alpha, (T)beta, (T)gamma, dt_dev + b0, mode, N, 0);
         NS_LAUNCHED("a7 spectral_kernel");
         prof.tick(-1, st);
         return NS_OK;

@@ -29,6 +29,11 @@ def test_header_symbols_exported(libns):
     for s in syms:
         assert hasattr(libns, s), f"libns.so does not export {s}"
     assert sorted(binding.EXPORTS) == syms
+    syms3 = declared_symbols("ns_mg.h", "ns_mg_")
+    assert len(syms3) >= 12
+    for s in syms3:
+        assert hasattr(libns, s), f"libns.so does not export {s}"
+    assert sorted(binding.EXPORTS_MG) == syms3
     syms2 = declared_symbols("ns2d.h", "ns2d_")
     assert len(syms2) >= 15
     for s in syms2:
