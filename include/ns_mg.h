@@ -6,22 +6,24 @@
  * is transformed; Algorithm 3; the transpose moves only partially padded data).  Its design -- MPI ranks, host-staged
  * MPI_Alltoall -- is prior art; here one process drives the P devices ("cuFFT can only distribute over multiple GPUs given they
  * are managed by the same process", L177, is the model that fits one NVLink node), each device has its own stream, and the
- * transpose is a set of strided device-to-device copies over NVLink peer access, ordered by events: no host staging, no host
- * synchronisation inside a step.
+ * transpose is FUSED into the transform pass that produces the data: the kernel stores every output row straight into the
+ * memory of the device that owns it (peer stores over NVLink, overlapped with the butterflies of the next tile), ordered
+ * between the devices' streams by events: no separate transpose pass, no host staging, no host synchronisation inside a step.
  *
  * Decomposition (P devices, rank r = position in the device list; Nyl = N/P, Ml = M/P, M = 3N/2):
  *   spectral side   rank r owns the ky rows [r Nyl, (r+1) Nyl) of every array [comp][kx][ky][kz]: a1 (inverse x pass), a6 (forward
  *                   x pass), a7 (spectral / RK kernel) and the state live here;
  *   physical side   rank r owns the px planes [r Ml, (r+1) Ml) of [comp][px][ky][kz]: a2 (y pass), a3+a4 (fused z kernel: padded
  *                   physical data never leaves the SM) and a5 run here;
- *   exchange A      after a1: block (px in slab s, ky in slab r) of 3 components goes from rank r to rank s   (3 M N H / P^2 per pair)
- *   exchange B      after a5: block (px in slab r, ky in slab s) of the 5 trace-free flux components goes back (5 M N H / P^2 per pair)
+ *   exchange A      inside a1: block (px in slab s, ky in slab r) of 3 components is stored by rank r into rank s   (3 M N H / P^2 per pair)
+ *   exchange B      inside a5: block (px in slab r, ky in slab s) of the 5 trace-free flux components goes back     (5 M N H / P^2 per pair)
  * The kernels are the ones of ns.h (same launchers, sub-ranges by pointer / stride); max|u| for the CFL step is reduced over the
  * devices by peer copies of P scalars.  Results equal those of ns.h on one device to round-off (the arithmetic per line is
  * identical; only the order of the max reduction differs, which is exact).
  *
  * Conventions: those of ns.h (layouts, normalisation, Nyquist planes, ns_params, ns_dtype, ns_status).  Restrictions: batch = 1;
- * N a power of two in [32, 512] with N/P and M/P multiples of 8 (fp32: 16) ... (M/P) M / 2 a multiple of 32; the state is set and
+ * N a transform grid of ns.h (p 2^a, p in {1, 3, 5, 7, 15}, 32 <= N <= 640, N/2 a multiple of 8, fp32: 16) with N and 3N/2
+ * divisible by P; a decomposition whose slabs the pass kernels cannot tile is rejected by ns_mg_create; the state is set and
  * read in SPECTRAL form in host memory (physical-space entry points stay with ns.h).  The device list may name the same device
  * more than once: the P ranks then share that GPU, which is how the decomposition is tested on a single-GPU machine.
  */

@@ -30,7 +30,23 @@ struct ColArgs {
     int tiles_per_slab;       // column tiles per slab (columns / TC)
     long total_tiles;         // slabs * tiles_per_slab
     int pf_dist;              // tiles ahead to prefetch into L2 (kernels instantiated with PF): about the CTAs resident on the GPU
+    // Output split over several destinations (multi-device solver, ns_mg.h: the slab exchange fused into the pass -- the rows of
+    // the transformed axis are stored straight into the memory of the device that owns them, over NVLink peer access).
+    // split_rows = 0: plain output.  Otherwise output row n goes to destination n / split_rows, row n % split_rows of the array
+    // at peer[destination] (same slab / column offsets and row stride as the plain output); peer is a table in DEVICE memory
+    // (a dynamically indexed kernel-parameter array would be copied to local memory in every thread).
+    int split_rows;
+    const unsigned long long* peer;
 };
+
+// address of output row `row` of the tile whose plain output base is `op` (= out + slab offset + column)
+// (SPLIT is a template flag of the kernels: the plain path compiles to exactly the single-device code)
+template <bool SPLIT, typename T>
+__device__ __forceinline__ cx<T>* col_row(cx<T>* out, cx<T>* op, const ColArgs& g, int row) {
+    if constexpr (!SPLIT) return op + (long)row * g.ostride;
+    const int dst = row / g.split_rows;
+    return reinterpret_cast<cx<T>*>(__ldg(g.peer + dst)) + (op - out) + (long)(row - dst * g.split_rows) * g.ostride;
+}
 
 template <int R1, int R2> struct ColP { static constexpr int value = R1 > R2 ? R1 : R2; };
 
@@ -52,7 +68,7 @@ __device__ __forceinline__ void col_prefetch_tile(const cx<T>* __restrict__ in, 
 // ------------------------------------------------------------------------------------------------
 // inverse (spectral rows [0,2L) -> physical rows [0,3L)), exp(+i...)
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R1, int R2, int TC, int TPB, bool PF>
+template <typename T, int L, int R1, int R2, int TC, int TPB, bool PF, bool SPLIT>
 __global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
 col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
                Twiddles<T> tw) {
@@ -126,7 +142,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
             for (int n2 = 0; n2 < R2; ++n2) y[n2] = Et[buf * EBUF + (size_t)(i * R2 + n2) * TC + c];
             fft_reg<R2, +1, T>(y);
 #pragma unroll
-            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[outpos<R2>(r2)];
+            for (int r2 = 0; r2 < R2; ++r2) *col_row<SPLIT>(out, op, g, q * L + i + R1 * r2) = y[outpos<R2>(r2)];
         }
         buf ^= 1;
     }
@@ -135,7 +151,7 @@ col_inv_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 // ------------------------------------------------------------------------------------------------
 // forward (physical rows [0,3L) -> spectral rows [0,2L), truncated), exp(-i...), output * scale
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R1, int R2, int TC, int TPB, bool PF>
+template <typename T, int L, int R1, int R2, int TC, int TPB, bool PF, bool SPLIT>
 __global__ void __launch_bounds__(TC* ColP<R1, R2>::value* TPB)
 col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale,
                Twiddles<T> tw) {
@@ -214,8 +230,8 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
                     const cx<T> A = F0[n1] + S;
                     // C = F0 - S/2 + i (sqrt3/2) D
                     const cx<T> C = mk<T>(F0[n1].x - (T)0.5 * S.x - h3 * D.y, F0[n1].y - (T)0.5 * S.y + h3 * D.x);
-                    op[(long)n * g.ostride] = scale * A;
-                    op[(long)(L + n) * g.ostride] = (n == 0) ? mk<T>(0, 0) : scale * C;
+                    *col_row<SPLIT>(out, op, g, n) = scale * A;
+                    *col_row<SPLIT>(out, op, g, L + n) = (n == 0) ? mk<T>(0, 0) : scale * C;
                 }
             }
         }
@@ -230,7 +246,7 @@ col_fwd_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g,
 // thread and a third of the shared memory, which is what bounded the kernel at two CTAs (8 warps) per SM.
 // One tile per CTA; CTAs of 4 (fp64) or 8 (fp32) warps; warp w uses TMEM lanes 32 (w % 4), columns of set w / 4.
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R2, int TC, int MINB, bool PF>
+template <typename T, int L, int R2, int TC, int MINB, bool PF, bool SPLIT>
 __global__ void __launch_bounds__(TC * 16, MINB)
 col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, T scale, Twiddles<T> tw) {
     constexpr int R1 = 16;
@@ -320,8 +336,8 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
                         const cx<T> A = f0 + S;
                         // C = F0 - S/2 + i (sqrt3/2) D
                         const cx<T> C = mk<T>(f0.x - (T)0.5 * S.x - h3 * D.y, f0.y - (T)0.5 * S.y + h3 * D.x);
-                        op[(long)n * g.ostride] = scale * A;
-                        op[(long)(L + n) * g.ostride] = (n == 0) ? mk<T>(0, 0) : scale * C;
+                        *col_row<SPLIT>(out, op, g, n) = scale * A;
+                        *col_row<SPLIT>(out, op, g, L + n) = (n == 0) ? mk<T>(0, 0) : scale * C;
                     }
                 }
             }
@@ -339,7 +355,7 @@ col_fwd_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
 // fits on the SM (the register-resident version needs 254 registers; ncu: 1.9 warps per scheduler, stalls
 // dominated by the global loads).  Thread layout and TMEM window as in col_fwd_tmem_kernel.
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R2, int TC, int MINB, bool PF>
+template <typename T, int L, int R2, int TC, int MINB, bool PF, bool SPLIT>
 __global__ void __launch_bounds__(TC * 16, MINB)
 col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColArgs g, Twiddles<T> tw) {
     constexpr int R1 = 16;
@@ -431,7 +447,7 @@ col_inv_tmem_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, ColAr
             for (int n2 = 0; n2 < R2; ++n2) y[n2] = E[buf * EBUF + (size_t)(i * R2 + n2) * TC + c];
             fft_reg<R2, +1, T>(y);
 #pragma unroll
-            for (int r2 = 0; r2 < R2; ++r2) op[(long)(q * L + i + R1 * r2) * g.ostride] = y[outpos<R2>(r2)];
+            for (int r2 = 0; r2 < R2; ++r2) *col_row<SPLIT>(out, op, g, q * L + i + R1 * r2) = y[outpos<R2>(r2)];
         }
         buf ^= 1;
     }

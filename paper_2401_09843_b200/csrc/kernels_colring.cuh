@@ -81,7 +81,7 @@ __device__ __forceinline__ void ring_park(uint32_t base, Gen gen) {
 // ------------------------------------------------------------------------------------------------
 // forward: physical rows [0,3L) -> spectral rows [0,2L), truncated, output * scale
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int R1, int R2, int TC, int STAGES, int MINB>
+template <typename T, int L, int R1, int R2, int TC, int STAGES, int MINB, bool SPLIT>
 __global__ void __launch_bounds__(3 * TC * ColP<R1, R2>::value + 32, MINB)
 col_fwd_ring_kernel(const __grid_constant__ CUtensorMap tmap, cx<T>* __restrict__ out, ColArgs g, T scale, Twiddles<T> tw) {
     using Geo = ColRingGeo<T, L, R1, R2, TC, STAGES>;
@@ -199,8 +199,8 @@ col_fwd_ring_kernel(const __grid_constant__ CUtensorMap tmap, cx<T>* __restrict_
             // C = F0 - S/2 + i (sqrt3/2) D
             const cx<T> Cc = mk<T>(f0.x - (T)0.5 * S.x - h3 * D.y, f0.y - (T)0.5 * S.y + h3 * D.x);
             cx<T>* op = ob + (e % TC);
-            stg_stream(op + (long)n * g.ostride, scale * A);
-            stg_stream(op + (long)(L + n) * g.ostride, (n == 0) ? mk<T>(0, 0) : scale * Cc);
+            stg_stream(col_row<SPLIT>(out, op, g, n), scale * A);
+            stg_stream(col_row<SPLIT>(out, op, g, L + n), (n == 0) ? mk<T>(0, 0) : scale * Cc);
         }
         named_bar_sync(BAR_ALL, 3 * TT);          // combine read: the stage goes back to the producer
         if (threadIdx.x == 0) mbar_arrive(empty + s);

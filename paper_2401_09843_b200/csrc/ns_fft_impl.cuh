@@ -57,11 +57,11 @@ static cudaError_t set_smem(K kernel, size_t bytes) {
     return cudaSuccess;
 }
 
-template <typename T, int L, bool PF>
+template <typename T, int L, bool PF, bool SPLIT = false>
 static cudaError_t col_inv_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, Twiddles<T> tw) {
     using C = Cfg<L>;
     constexpr int TC = tile_cols<T>(), TPB = C::template tpb<T>();
-    auto k = col_inv_kernel<T, L, C::R1, C::R2, TC, TPB, PF>;
+    auto k = col_inv_kernel<T, L, C::R1, C::R2, TC, TPB, PF, SPLIT>;
     const size_t smem = (size_t)2 * TPB * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -70,11 +70,11 @@ static cudaError_t col_inv_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
     return cudaGetLastError();
 }
 
-template <typename T, int L, bool PF>
+template <typename T, int L, bool PF, bool SPLIT = false>
 static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
     using C = Cfg<L>;
     constexpr int TC = tile_cols<T>(), TPB = C::template tpb<T>();
-    auto k = col_fwd_kernel<T, L, C::R1, C::R2, TC, TPB, PF>;
+    auto k = col_fwd_kernel<T, L, C::R1, C::R2, TC, TPB, PF, SPLIT>;
     const size_t smem = (size_t)3 * TPB * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -84,11 +84,11 @@ static cudaError_t col_fwd_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColAr
 }
 
 // long lines (L = 128, 256): inverse pass with its inputs parked in tensor memory
-template <typename T, int L, bool PF>
+template <typename T, int L, bool PF, bool SPLIT = false>
 static cudaError_t col_inv_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, Twiddles<T> tw) {
     constexpr int TC = tile_cols<T>(), R2 = L / 16;
     constexpr int MINB = sizeof(T) == 8 ? 3 : 2;
-    auto k = col_inv_tmem_kernel<T, L, R2, TC, MINB, PF>;
+    auto k = col_inv_tmem_kernel<T, L, R2, TC, MINB, PF, SPLIT>;
     const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -97,11 +97,11 @@ static cudaError_t col_inv_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, 
 }
 
 // long lines (L = 128, 256): forward pass with F_0 / G_1 parked in tensor memory
-template <typename T, int L, bool PF>
+template <typename T, int L, bool PF, bool SPLIT = false>
 static cudaError_t col_fwd_tmem_L(cudaStream_t st, const cx<T>* in, cx<T>* out, ColArgs g, T scale, Twiddles<T> tw) {
     constexpr int TC = tile_cols<T>(), R2 = L / 16;
     constexpr int MINB = sizeof(T) == 8 ? 3 : 2;
-    auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB, PF>;
+    auto k = col_fwd_tmem_kernel<T, L, R2, TC, MINB, PF, SPLIT>;
     const size_t smem = (size_t)2 * L * TC * sizeof(cx<T>);
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
@@ -142,12 +142,12 @@ static cudaError_t col_tensor_map(CUtensorMap* m, const cx<T>* in, long ncols, l
 // stages of the input ring / CTAs per SM: L = 256: 2 x 96 KB, one CTA of 13 (fp64) / 25 (fp32) warps per SM
 template <int L> struct RingCfg { static constexpr int STAGES = 2, MINB = 1; };
 
-template <typename T, int L>
+template <typename T, int L, bool SPLIT = false>
 static cudaError_t col_fwd_ring_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T>* out, long ncols, ColArgs g, T scale, Twiddles<T> tw) {
     using C = Cfg<L>;
     constexpr int TC = tile_cols<T>(), STAGES = RingCfg<L>::STAGES;
     using Geo = ColRingGeo<T, L, C::R1, C::R2, TC, STAGES>;
-    auto k = col_fwd_ring_kernel<T, L, C::R1, C::R2, TC, STAGES, RingCfg<L>::MINB>;
+    auto k = col_fwd_ring_kernel<T, L, C::R1, C::R2, TC, STAGES, RingCfg<L>::MINB, SPLIT>;
     CUtensorMap m;
     cudaError_t e = col_tensor_map<T>(&m, in, ncols, 3 * L, g, L);
     if (e != cudaSuccess) return e;
@@ -251,8 +251,11 @@ static bool col_pf_on(bool fwd, int L, long row_stride_bytes) {
 }
 
 template <typename T>
-static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab, int pf_dist) {
+static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride, long in_slab, long out_slab, int pf_dist,
+                             const ColSplit* split) {
     ColArgs g;
+    g.split_rows = split ? split->rows : 0;
+    g.peer = split ? split->peer : nullptr;
     g.istride = istride;
     g.ostride = ostride;
     g.in_slab = in_slab;
@@ -265,11 +268,19 @@ static ColArgs make_col_args(long ncols, long nslabs, long istride, long ostride
 
 template <typename T>
 cudaError_t NS_FAM(launch_col_inv)(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
-                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
+                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw, const ColSplit* split) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
-    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
+    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L), split);
     // measured (profiles/): parking pays at L = 128 (0.264 -> 0.216 ms at 256^3); at L = 256 the register kernel is faster
     const bool pf = col_pf_on(false, L, istride * (long)sizeof(cx<T>));
+    if (split) {      // multi-device solver: output rows stored to their owners (no L2 prefetch variant)
+#ifndef NS_FAMILY_SMOOTH
+        if (L == 128) return col_inv_tmem_L<T, 128, false, true>(st, in, out, g, tw);
+#endif
+#define CALL(LL) col_inv_L<T, LL, false, true>(st, in, out, g, tw)
+        NS_DISPATCH_L(L, CALL)
+#undef CALL
+    }
 #ifndef NS_FAMILY_SMOOTH
     if (L == 128) return pf ? col_inv_tmem_L<T, 128, true>(st, in, out, g, tw) : col_inv_tmem_L<T, 128, false>(st, in, out, g, tw);
 #endif
@@ -280,10 +291,19 @@ cudaError_t NS_FAM(launch_col_inv)(cudaStream_t st, int num_sms, int L, const cx
 
 template <typename T>
 cudaError_t NS_FAM(launch_col_fwd)(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
-                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
+                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw, const ColSplit* split) {
     if (ncols % tile_cols<T>() != 0) return cudaErrorInvalidValue;
-    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L));
+    const ColArgs g = make_col_args<T>(ncols, nslabs, istride, ostride, in_slab, out_slab, col_pf_dist(num_sms, L), split);
     const bool pf = col_pf_on(true, L, istride * (long)sizeof(cx<T>));
+    if (split) {      // multi-device solver: output rows stored to their owners
+#ifndef NS_FAMILY_SMOOTH
+        if (L == 256) return col_fwd_ring_L<T, 256, true>(st, num_sms, in, out, ncols, g, scale, tw);
+        if (L == 128) return col_fwd_tmem_L<T, 128, false, true>(st, in, out, g, scale, tw);
+#endif
+#define CALL(LL) col_fwd_L<T, LL, false, true>(st, in, out, g, scale, tw)
+        NS_DISPATCH_L(L, CALL)
+#undef CALL
+    }
 #ifndef NS_FAMILY_SMOOTH
     // long lines: the persistent TMA-fed kernel (measured at 512^3: fp64 a5 3.65 -> 3.20 ms, a6 2.67 -> 2.52 ms; fp32 1.96 -> 1.84, 1.40 -> 1.24)
     if (L == 256) return col_fwd_ring_L<T, 256>(st, num_sms, in, out, ncols, g, scale, tw);
@@ -349,15 +369,15 @@ cudaError_t launch_y2d(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<
 // the public launchers route by family (defined once, in the pow2 translation unit)
 template <typename T>
 cudaError_t launch_col_inv(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
-                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw) {
-    if ((L & (L - 1)) == 0) return launch_col_inv_pow2<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, tw);
-    return launch_col_inv_smooth<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, tw);
+                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw, const ColSplit* split) {
+    if ((L & (L - 1)) == 0) return launch_col_inv_pow2<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, tw, split);
+    return launch_col_inv_smooth<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, tw, split);
 }
 template <typename T>
 cudaError_t launch_col_fwd(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
-                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw) {
-    if ((L & (L - 1)) == 0) return launch_col_fwd_pow2<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, scale, tw);
-    return launch_col_fwd_smooth<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, scale, tw);
+                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw, const ColSplit* split) {
+    if ((L & (L - 1)) == 0) return launch_col_fwd_pow2<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, scale, tw, split);
+    return launch_col_fwd_smooth<T>(st, num_sms, L, in, out, ncols, nslabs, istride, ostride, in_slab, out_slab, scale, tw, split);
 }
 template <typename T>
 cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,
@@ -371,16 +391,16 @@ cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in,
 #define NS_FFT_ARGS_Z(T) cudaStream_t, int, int, const cx<T>*, cx<T>*, long, long, unsigned long long*, Twiddles<T>
 #ifdef NS_FAMILY_SMOOTH
 #define NS_INSTANTIATE_FFT(T)                                                                   \
-    template cudaError_t launch_col_inv_smooth<T>(NS_FFT_ARGS_COL(T), Twiddles<T>);             \
-    template cudaError_t launch_col_fwd_smooth<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>);          \
+    template cudaError_t launch_col_inv_smooth<T>(NS_FFT_ARGS_COL(T), Twiddles<T>, const ColSplit*);             \
+    template cudaError_t launch_col_fwd_smooth<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>, const ColSplit*);          \
     template cudaError_t launch_z_fused_smooth<T>(NS_FFT_ARGS_Z(T));
 #else
 #define NS_INSTANTIATE_FFT(T)                                                                   \
-    template cudaError_t launch_col_inv_pow2<T>(NS_FFT_ARGS_COL(T), Twiddles<T>);               \
-    template cudaError_t launch_col_fwd_pow2<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>);            \
+    template cudaError_t launch_col_inv_pow2<T>(NS_FFT_ARGS_COL(T), Twiddles<T>, const ColSplit*);               \
+    template cudaError_t launch_col_fwd_pow2<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>, const ColSplit*);            \
     template cudaError_t launch_z_fused_pow2<T>(NS_FFT_ARGS_Z(T));                              \
-    template cudaError_t launch_col_inv<T>(NS_FFT_ARGS_COL(T), Twiddles<T>);                    \
-    template cudaError_t launch_col_fwd<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>);                 \
+    template cudaError_t launch_col_inv<T>(NS_FFT_ARGS_COL(T), Twiddles<T>, const ColSplit*);                    \
+    template cudaError_t launch_col_fwd<T>(NS_FFT_ARGS_COL(T), T, Twiddles<T>, const ColSplit*);                 \
     template cudaError_t launch_z_fused<T>(NS_FFT_ARGS_Z(T));                                   \
     template cudaError_t launch_y2d<T>(NS_FFT_ARGS_Z(T));
 #endif

@@ -37,14 +37,23 @@ bool fft_supported(int L);
 // columns per tile of the strided passes (128 bytes per row)
 template <typename T> constexpr int tile_cols() { return 128 / (2 * (int)sizeof(T)); }
 
+// Output of a strided-axis pass split over several destinations (multi-device solver): output row n is stored to row
+// n % rows of the array at peer[n / rows]; `peer` is a table IN DEVICE MEMORY of the launching device holding the destination
+// base addresses (device pointers, possibly of other devices with peer access enabled); `base` = peer[0], the address the
+// plain-output offsets are taken against.
+struct ColSplit {
+    int rows;
+    const unsigned long long* peer;
+};
+
 // Strided-axis passes.  `ncols` contiguous columns per slab (multiple of tile_cols<T>()), `nslabs` slabs.
 // Input rows [0,2L) -> output rows [0,3L) (inverse) or the reverse (forward, output multiplied by scale).
 template <typename T>
 cudaError_t launch_col_inv(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
-                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw);
+                           long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw, const ColSplit* split = nullptr);
 template <typename T>
 cudaError_t launch_col_fwd(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,
-                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw);
+                           long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw, const ColSplit* split = nullptr);
 // fused a3+a4 (kernels_zpair.cuh; kernels_zfused.cuh for L <= 32): in [batch][3][MM][L] -> out [batch][NS_NFLUX][MM][L];
 // persistent grid sized from num_sms (the SM count of the solver's device) and the CTAs per SM.  umax2 may be NULL.
 template <typename T>
@@ -55,10 +64,12 @@ cudaError_t launch_z_fused(cudaStream_t st, int num_sms, int L, const cx<T>* in,
 #define NS_DECL_FAMILY(FAM)                                                                                                        \
     template <typename T>                                                                                                          \
     cudaError_t launch_col_inv_##FAM(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,    \
-                                     long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw);                     \
+                                     long istride, long ostride, long in_slab, long out_slab, Twiddles<T> tw,                     \
+                                     const ColSplit* split);                                                                       \
     template <typename T>                                                                                                          \
     cudaError_t launch_col_fwd_##FAM(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long ncols, long nslabs,    \
-                                     long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw);            \
+                                     long istride, long ostride, long in_slab, long out_slab, T scale, Twiddles<T> tw,            \
+                                     const ColSplit* split);                                                                       \
     template <typename T>                                                                                                          \
     cudaError_t launch_z_fused_##FAM(cudaStream_t st, int num_sms, int L, const cx<T>* in, cx<T>* out, long MM, long batch,        \
                                      unsigned long long* umax2, Twiddles<T> tw);

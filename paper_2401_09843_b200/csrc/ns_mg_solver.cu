@@ -1,6 +1,7 @@
 // ns_mg_solver.cu -- host side of the multi-device solver (include/ns_mg.h): one sample distributed over P
-// devices by slabs (Algorithm 3), one process driving all of them.  Launch sequences and the slab
-// exchanges only; every arithmetic step runs in the kernels of ns.h's path (same launchers, sub-ranges by pointer / stride).
+// devices by slabs (Algorithm 3), one process driving all of them.  Launch sequences and event ordering
+// only; every arithmetic step runs in the kernels of ns.h's path (same launchers, sub-ranges by pointer / stride) and the slab
+// exchanges are peer stores of those kernels (ColSplit in kernels_col.cuh).
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -107,8 +108,9 @@ struct MgRank {
     T* dtab = nullptr;
     double *dt_dev = nullptr, *t_dev = nullptr;
     unsigned long long *umax2 = nullptr, *um_all = nullptr;
+    unsigned long long* ptab = nullptr;   // [1 + NS_NFLUX][P] destination base addresses of the fused exchanges (a1; a5 per component)
     int* bad = nullptr;
-    cudaEvent_t e1 = nullptr, e5 = nullptr, eB = nullptr, ez = nullptr;
+    cudaEvent_t e1 = nullptr, e2 = nullptr, e5 = nullptr, e6 = nullptr, ez = nullptr;
     std::vector<void*> allocs;
 };
 
@@ -127,7 +129,7 @@ public:
             cudaSetDevice(r.dev);
             if (r.st) cudaStreamSynchronize(r.st);
             for (void* p : r.allocs) cudaFree(p);
-            cudaEvent_t evs[4] = {r.e1, r.e5, r.eB, r.ez};
+            cudaEvent_t evs[5] = {r.e1, r.e2, r.e5, r.e6, r.ez};
             for (cudaEvent_t e : evs)
                 if (e) cudaEventDestroy(e);
             if (r.st) cudaStreamDestroy(r.st);
@@ -195,20 +197,36 @@ public:
             MG_CK(cudaStreamCreateWithFlags(&k.st, cudaStreamNonBlocking));
             int rc;
             if ((rc = alloc(k, &k.U, 3 * sl)) || (rc = alloc(k, &k.V, 3 * sl)) || (rc = alloc(k, &k.R, 3 * sl)) ||
-                (rc = alloc(k, &k.X, NS_NFLUX * (size_t)M * Nyl * H)) || (rc = alloc(k, &k.Tt, NS_NFLUX * pl)) ||
+                (rc = alloc(k, &k.X, NS_NFLUX * (size_t)M * Nyl * H)) || (rc = alloc(k, &k.Tt, 3 * pl)) ||
                 (rc = alloc(k, &k.Y, 3 * pm)) || (rc = alloc(k, &k.Z, NS_NFLUX * pm)) || (rc = alloc(k, &k.B, NS_NFLUX * sl)) ||
                 (rc = alloc(k, &k.pub, (size_t)3 * N * N * (H + 1))) || (rc = alloc(k, &k.twbase, htw.size())) ||
                 (rc = alloc(k, &k.dtab, ndt)) || (rc = alloc(k, &k.dt_dev, 1)) || (rc = alloc(k, &k.t_dev, 1)) ||
-                (rc = alloc(k, &k.umax2, 1)) || (rc = alloc(k, &k.um_all, (size_t)P)) || (rc = alloc(k, &k.bad, 1)))
+                (rc = alloc(k, &k.umax2, 1)) || (rc = alloc(k, &k.um_all, (size_t)P)) || (rc = alloc(k, &k.bad, 1)) ||
+                (rc = alloc(k, &k.ptab, (size_t)(1 + NS_NFLUX) * P)))
                 return rc;
             MG_CK(cudaMemcpyAsync(k.twbase, htw.data(), htw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, k.st));
             MG_CK(cudaMemcpyAsync(k.dtab, hd.data(), hd.size() * sizeof(T), cudaMemcpyHostToDevice, k.st));
             MG_CK(cudaMemsetAsync(k.t_dev, 0, sizeof(double), k.st));
             MG_CK(cudaMemsetAsync(k.dt_dev, 0, sizeof(double), k.st));
             MG_CK(cudaMemsetAsync(k.bad, 0, sizeof(int), k.st));
-            cudaEvent_t* evs[4] = {&k.e1, &k.e5, &k.eB, &k.ez};
+            cudaEvent_t* evs[5] = {&k.e1, &k.e2, &k.e5, &k.e6, &k.ez};
             for (cudaEvent_t* e : evs) MG_CK(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
             MG_CK(cudaStreamSynchronize(k.st));
+        }
+        // destination tables of the fused exchanges (all ranks' buffers exist now)
+        const size_t ncs = (size_t)Nyl * H;
+        for (int r = 0; r < P; ++r) {
+            MgRank<T>& k = rk[(size_t)r];
+            std::vector<unsigned long long> h((size_t)(1 + NS_NFLUX) * P);
+            for (int s = 0; s < P; ++s) {
+                // a1 of rank r: output row px -> plane px % Ml of Tt_s [3][Ml][N][H], at this rank's ky rows
+                h[(size_t)s] = (unsigned long long)(rk[(size_t)s].Tt + (size_t)r * Nyl * H);
+                // a5 of rank r, component c: output row ky -> row ky % Nyl of X_s [5][M][Nyl][H], at this rank's px planes
+                for (int c = 0; c < NS_NFLUX; ++c)
+                    h[(size_t)(1 + c) * P + s] = (unsigned long long)(rk[(size_t)s].X + ((size_t)c * M + (size_t)r * Ml) * ncs);
+            }
+            MG_CK(cudaSetDevice(k.dev));
+            MG_CK(cudaMemcpy(k.ptab, h.data(), h.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice));
         }
         return NS_OK;
     }
@@ -225,51 +243,53 @@ public:
         return NS_OK;
     }
 
-    // ---------------------------------------------------------------- a1 | exchange A | a2, a3+a4, a5 | exchange B | a6
+    // ---------------------------------------------------------------- a1 (+ exchange A) | a2, a3+a4, a5 (+ exchange B) | a6
     // which = 0: transform the state U, 1: the stage state V.  Result: rank r's B = Th [5][N][Nyl][H].
+    // Both exchanges are FUSED into the producing pass: a1 of rank r stores output row px straight into Tt of the rank that owns
+    // that px plane, a5 of rank s stores output row ky straight into X of the rank that owns that ky row (ColSplit: peer
+    // stores over NVLink, overlapped with the butterflies of the next tile); no separate transpose / copy pass exists.
+    // Ordering between the rank streams by events: e1 (a1 done), e2 (a2 done: Tt consumed), e5 (a5 done), e6 (a6 done: X consumed).
     int transform(int which, bool want_umax) {
         const long nc = (long)Nyl * H;      // contiguous columns of a ky slab row
-        const size_t sz = sizeof(cx<T>);
         for (int r = 0; r < P; ++r) {
             MgRank<T>& k = rk[(size_t)r];
             MG_CK(cudaSetDevice(k.dev));
-            MG_LAUNCH(launch_col_inv<T>(k.st, k.num_sms, L, which ? k.V : k.U, k.X, nc, 3, nc, nc, (long)N * nc, (long)M * nc, tw(k)),
-                      "a1 col_inv x");
+            for (int s = 0; s < P; ++s) MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)s].e2, 0));   // Tt_s of the previous pass consumed
+            ColSplit sp;
+            sp.rows = Ml;                   // output row px -> rank px / Ml, plane px % Ml of Tt [3][Ml][N][H], at this rank's ky rows
+            sp.peer = k.ptab;
+            MG_LAUNCH(launch_col_inv<T>(k.st, k.num_sms, L, which ? k.V : k.U, rk[0].Tt + (size_t)r * Nyl * H, nc, 3, nc, (long)N * H, (long)N * nc,
+                                        (long)Ml * N * H, tw(k), &sp),
+                      "a1 col_inv x + exchange A");
             MG_CK(cudaEventRecord(k.e1, k.st));
         }
         for (int s = 0; s < P; ++s) {       // physical side of rank s
             MgRank<T>& k = rk[(size_t)s];
             MG_CK(cudaSetDevice(k.dev));
-            for (int r = 0; r < P; ++r) {
-                MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)r].e1, 0));   // a1 of rank r done
-                MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)r].eB, 0));   // rank r no longer reads this rank's Tt (previous exchange B)
-            }
-            // exchange A (pull): block (px in slab s, ky in slab r) of X_r -> Tt_s [3][Ml][N][H]
-            for (int r = 0; r < P; ++r)
-                for (int c = 0; c < 3; ++c)
-                    MG_CK(cudaMemcpy2DAsync(k.Tt + ((size_t)c * Ml * N + (size_t)r * Nyl) * H, (size_t)N * H * sz,
-                                            rk[(size_t)r].X + ((size_t)c * M + (size_t)s * Ml) * nc, (size_t)nc * sz, (size_t)nc * sz, (size_t)Ml,
-                                            cudaMemcpyDefault, k.st));
+            for (int r = 0; r < P; ++r) MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)r].e1, 0));   // every rank's a1 has stored into Tt_s
             MG_LAUNCH(launch_col_inv<T>(k.st, k.num_sms, L, k.Tt, k.Y, H, (long)3 * Ml, H, H, (long)N * H, (long)M * H, tw(k)), "a2 col_inv y");
+            MG_CK(cudaEventRecord(k.e2, k.st));
             MG_LAUNCH(launch_z_fused<T>(k.st, k.num_sms, L, k.Y, k.Z, (long)Ml * M, 1, want_umax ? k.umax2 : nullptr, tw(k)), "a3+a4 z_fused");
             if (want_umax) MG_CK(cudaEventRecord(k.ez, k.st));
-            MG_LAUNCH(launch_col_fwd<T>(k.st, k.num_sms, L, k.Z, k.Tt, H, (long)NS_NFLUX * Ml, H, H, (long)M * H, (long)N * H, (T)1, tw(k)),
-                      "a5 col_fwd y");
+            for (int r = 0; r < P; ++r) MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)r].e6, 0));   // X_r of the previous pass consumed
+            for (int c = 0; c < NS_NFLUX; ++c) {
+                ColSplit sp;
+                sp.rows = Nyl;              // output row ky -> rank ky / Nyl, row ky % Nyl of X [5][M][Nyl][H], at this rank's px planes
+                sp.peer = k.ptab + (size_t)(1 + c) * P;
+                MG_LAUNCH(launch_col_fwd<T>(k.st, k.num_sms, L, k.Z + (size_t)c * Ml * M * H, rk[0].X + ((size_t)c * M + (size_t)s * Ml) * nc, H,
+                                            (long)Ml, H, H, (long)M * H,
+                                            nc, (T)1, tw(k), &sp),
+                          "a5 col_fwd y + exchange B");
+            }
             MG_CK(cudaEventRecord(k.e5, k.st));
         }
         for (int r = 0; r < P; ++r) {       // spectral side of rank r
             MgRank<T>& k = rk[(size_t)r];
             MG_CK(cudaSetDevice(k.dev));
-            for (int s = 0; s < P; ++s) MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)s].e5, 0));
-            // exchange B (pull): block (px in slab s, ky in slab r) of Tt_s [5][Ml][N][H] -> X_r [5][M][Nyl][H]
-            for (int s = 0; s < P; ++s)
-                for (int c = 0; c < NS_NFLUX; ++c)
-                    MG_CK(cudaMemcpy2DAsync(k.X + ((size_t)c * M + (size_t)s * Ml) * nc, (size_t)nc * sz,
-                                            rk[(size_t)s].Tt + ((size_t)c * Ml * N + (size_t)r * Nyl) * H, (size_t)N * H * sz, (size_t)nc * sz,
-                                            (size_t)Ml, cudaMemcpyDefault, k.st));
-            MG_CK(cudaEventRecord(k.eB, k.st));
+            for (int s = 0; s < P; ++s) MG_CK(cudaStreamWaitEvent(k.st, rk[(size_t)s].e5, 0));   // every rank's a5 has stored into X_r
             MG_LAUNCH(launch_col_fwd<T>(k.st, k.num_sms, L, k.X, k.B, nc, NS_NFLUX, nc, nc, (long)M * nc, (long)N * nc, (T)1, tw(k)),
                       "a6 col_fwd x");
+            MG_CK(cudaEventRecord(k.e6, k.st));
         }
         return NS_OK;
     }
