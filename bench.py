@@ -450,6 +450,43 @@ def run_workload_2d(binding, torch, name, dtype, steps, warmup, local, rank=0):
             "setup_s": round(setup, 1), "device_bytes": s.device_bytes(), "l2": "inputs exceed L2 (126 MB): no flush needed"}
 
 
+def run_slab(args):
+    """One sample over several GPUs of this node (include/ns_mg.h): "scaling": "strong".  Needs DISTINCT
+    devices -- ranks that share a GPU are how the decomposition is TESTED, never a measurement."""
+    import torch
+    from paper_2401_09843_b200 import binding
+    devs = [int(x) for x in args.slab_devices.split(",")]
+    if len(set(devs)) != len(devs) or max(devs) >= torch.cuda.device_count():
+        raise SystemExit(f"--slab-devices needs distinct ordinals below {torch.cuda.device_count()} (got {devs})")
+    w = WORKLOADS[args.workload]
+    if w["batch"] != 1:
+        raise SystemExit("the slab decomposition distributes ONE sample: use a single-sample workload (c2, c3, c5, tg3d, cyl, n384)")
+    N = w["N"]
+    one = binding.Solver(N, dtype=args.dtype, **w["params"])        # state from the seeded input on device 0
+    one.set_initial(make_input(args.workload, N, 1))
+    uh = one.get_spectral()[0]
+    del one
+    s = binding.SolverMG(N, devs, dtype=args.dtype, **w["params"])
+    s.set_spectral(uh)
+    for _ in range(args.warmup):
+        s.step_cfl(w.get("cfl", 0.2), 1e30, return_dt=False)
+    s.step_cfl(w.get("cfl", 0.2), 1e30)                              # synchronises every rank
+    sampler = ClockSampler(devs[0])
+    launches0 = s.kernel_launches()
+    t0 = time.perf_counter()
+    for _ in range(args.steps - 1):
+        s.step_cfl(w.get("cfl", 0.2), 1e30, return_dt=False)
+    s.step_cfl(w.get("cfl", 0.2), 1e30)                              # ... so the wall clock spans complete steps on all devices
+    ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    print(json.dumps({"metric": "grid_point_stages_per_s", "value": roofline.grid_point_stages(N, 1, 1) / (ms * 1e-3),
+                      "unit": "grid-point-stages/s", "n_gpus": len(devs), "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+                      "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+                      "config": {"workload": w["desc"], "N": N, "parallelism": f"slab decomposition over devices {devs}, one process "
+                                 "(ns_mg.h): exchanges fused into a1 / a5 as peer stores", "timer": "host wall clock around synchronised steps"},
+                      "exchange_bytes_per_rhs": s.exchange_bytes(), "gpu_launches": s.kernel_launches() - launches0, "clocks": sampler.stop()}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -463,11 +500,16 @@ def main():
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT (torch.fft) comparison line")
     ap.add_argument("--no-also", action="store_true", help="skip the sub-records of the other north-star targets")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--slab-devices", default=None,
+                    help="comma-separated DISTINCT CUDA ordinals: time ONE sample of the workload slab-decomposed over these GPUs "
+                         "(include/ns_mg.h, single process; strong scaling) instead of the replica run")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.warmup < 3:
         args.warmup = 3  # timing rule: at least 3 warm-up steps
+    if args.slab_devices is not None:
+        return run_slab(args)
 
     import torch
     rank, world, local = dist_env()

@@ -29,9 +29,9 @@ def field(N, seed):
     return u + 0.1 * inputs.normal01(seed, 3, 3 * N ** 3).reshape(3, N, N, N)
 
 
-@pytest.mark.parametrize("N,P", [(64, 1), (64, 2), (64, 4), (96, 3)])
+@pytest.mark.parametrize("N,P", [(64, 1), (64, 4), (96, 3)])
 def test_mg_rhs_and_steps_against_the_oracle(ns, oracle, N, P):
-    """RHS (every stored entry), max|u| and 5 CFL steps of the slab-decomposed solver against the oracle (which replays dt)."""
+    """RHS (every stored entry), max|u| and 3 CFL steps of the slab-decomposed solver against the oracle (which replays dt)."""
     kw = dict(nu=0.002, eps=0.05, s=1.0)
     uh = oracle.set_initial(N, field(N, 40 + N + P))
     s = ns.SolverMG(N, [0] * P, **kw)
@@ -44,7 +44,7 @@ def test_mg_rhs_and_steps_against_the_oracle(ns, oracle, N, P):
     assert np.all(r[:, N // 2] == 0) and np.all(r[:, :, N // 2] == 0) and np.all(r[:, :, :, N // 2] == 0)
     assert abs(s.max_velocity() - want["umax"]) < 1e-13 * want["umax"]
     worst, tsum = 0.0, 0.0
-    for i in range(5):
+    for i in range(3):
         dt = s.step_cfl(0.2, 1e9)
         assert abs(dt - 0.2 * (2 * np.pi / N) / oracle.max_velocity(N, uh)) < 1e-12 * dt
         tsum += dt
@@ -53,10 +53,10 @@ def test_mg_rhs_and_steps_against_the_oracle(ns, oracle, N, P):
         assert worst < 1e-10, (i, worst)
     assert abs(s.time() - tsum) < 1e-13 * tsum
     assert s.exchange_bytes() == 8 * (3 * N // 2) * N * (N // 2) * 16 // P * (P - 1)
-    print(f"N = {N}, P = {P}: worst rel-L2 over 5 steps {worst:.2e}; exchange {s.exchange_bytes() / 1e6:.1f} MB per RHS")
+    print(f"N = {N}, P = {P}: worst rel-L2 over 3 steps {worst:.2e}; exchange {s.exchange_bytes() / 1e6:.1f} MB per RHS")
 
 
-@pytest.mark.parametrize("N,P,dtype", [(128, 2, "f64"), (128, 4, "f64"), (256, 2, "f64"), (256, 4, "f32")])
+@pytest.mark.parametrize("N,P,dtype", [(128, 4, "f64"), (256, 2, "f64"), (256, 4, "f32")])
 def test_mg_is_bitwise_the_single_device_result(ns, N, P, dtype):
     """Sizes that run the line-pair z kernel and the tensor-memory column kernels on slabs: RHS, per-step dt and the state after 3
     CFL steps + 1 fixed step are BIT-IDENTICAL to the single-device solver of ns.h (same kernels per line; the slab exchange only
