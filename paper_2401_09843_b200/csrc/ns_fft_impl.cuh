@@ -7,6 +7,9 @@
 #include "kernels_zpair.cuh"
 #include "kernels_y2d.cuh"
 #include "ns_internal.h"
+#include <map>
+#include <mutex>
+#include <utility>
 
 namespace ns {
 
@@ -51,9 +54,44 @@ template <int L> struct Cfg {
     static constexpr int minbf() { return (L >= 160 && (L & (L - 1)) != 0) ? 4 : 2; }
 };
 
+// Function attributes and occupancy are properties of (kernel, device): they are set / queried once per pair and remembered, not
+// on every launch (one RK3 step is 19 launches; at 32^3 the step is launch bound).  Thread safe.
+struct KernelSetup {
+    size_t smem = 0;      // MaxDynamicSharedMemorySize already granted
+    int occ = 0;          // CTAs per SM from the occupancy query (0 = not asked yet)
+    bool carveout = false;
+};
+static std::mutex& kernel_setup_mutex() {
+    static std::mutex m;
+    return m;
+}
+static KernelSetup& kernel_setup(const void* fn) {      // call with kernel_setup_mutex() held
+    static std::map<std::pair<const void*, int>, KernelSetup> table;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return table[std::make_pair(fn, dev)];
+}
 template <typename K>
 static cudaError_t set_smem(K kernel, size_t bytes) {
-    if (bytes > 48 * 1024) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    std::lock_guard<std::mutex> lock(kernel_setup_mutex());
+    KernelSetup& ks = kernel_setup((const void*)kernel);
+    if (ks.smem >= bytes) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) ks.smem = bytes;
+    return e;
+}
+template <typename K>
+static cudaError_t occupancy(K kernel, int threads, size_t smem, int* occ) {
+    std::lock_guard<std::mutex> lock(kernel_setup_mutex());
+    KernelSetup& ks = kernel_setup((const void*)kernel);
+    if (ks.occ == 0) {
+        int o = 0;
+        const cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kernel, threads, smem);
+        if (e != cudaSuccess) return e;
+        ks.occ = o < 1 ? 1 : o;
+    }
+    *occ = ks.occ;
     return cudaSuccess;
 }
 
@@ -153,7 +191,7 @@ static cudaError_t col_fwd_ring_L(cudaStream_t st, int num_sms, const cx<T>* in,
     if (e != cudaSuccess) return e;
     if ((e = set_smem(k, Geo::FWD_BYTES)) != cudaSuccess) return e;
     int occ = 0;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, Geo::NT, Geo::FWD_BYTES)) != cudaSuccess) return e;
+    if ((e = occupancy(k, Geo::NT, Geo::FWD_BYTES, &occ)) != cudaSuccess) return e;
     long grid = (long)num_sms * (occ < 1 ? 1 : occ);
     if (grid > g.total_tiles) grid = g.total_tiles;
     k<<<(unsigned)grid, Geo::NT, Geo::FWD_BYTES, st>>>(m, out, g, scale, tw);
@@ -168,12 +206,19 @@ static cudaError_t z_fused_L(cudaStream_t st, int num_sms, const cx<T>* in, cx<T
     const size_t smem = (size_t)LPB * (3 * L + 3 * C::R1 * (C::R2 + 1)) * sizeof(cx<T>) + 16;
     cudaError_t e = set_smem(k, smem);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
+    {
+        std::lock_guard<std::mutex> lock(kernel_setup_mutex());
+        KernelSetup& ks = kernel_setup((const void*)k);
+        if (!ks.carveout) {
+            e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+            if (e != cudaSuccess) return e;
+            ks.carveout = true;
+        }
+    }
     if ((MM % LPB) != 0) return cudaErrorInvalidValue;
     const long tiles = MM * batch / LPB;
     int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 3 * C::P * LPB, smem);
+    e = occupancy(k, 3 * C::P * LPB, smem, &occ);
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
     long grid = (long)num_sms * occ;
