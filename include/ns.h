@@ -46,7 +46,9 @@
  *             by the next call that synchronises anyway: ns_step_cfl with dt_out, ns_step_dts,
  *             ns_advance (which stops instead of running to max_steps) and ns_max_velocity (which
  *             still fills umax_out, +inf or NaN for that sample).  Setting a new state clears the mark.
- *   threads   no global state; handles are independent; one handle must not be used concurrently.
+ *   threads   handles are independent; one handle must not be used concurrently.  The only process-wide state is read-mostly and
+ *             mutex-protected: the ns_autotune table (device, N, dtype) -> transform grid, and the per-(kernel, device) record
+ *             of function attributes already set.
  */
 #ifndef NS_H_
 #define NS_H_
