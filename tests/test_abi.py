@@ -64,6 +64,13 @@ def test_create_rejects_bad_arguments(libns):
     for N, batch, dtype in [(64, 1, 0), (96, 1, 0), (1024, 1, 0), (256, 0, 0), (256, 1, 7)]:
         assert libns.ns2d_create(ctypes.byref(h), N, batch, None, dtype, None) == binding.NS_ERR_INVALID_ARG and not h.value
     assert libns.ns2d_destroy(None) == binding.NS_ERR_INVALID_ARG and libns.ns2d_step(None, 0.1) == binding.NS_ERR_INVALID_ARG
+    # ns_mg.h: decomposition checks come before any device is touched
+    dev = (ctypes.c_int * 4)(0, 0, 0, 0)
+    for N, P, dtype in [(64, 0, 0), (64, 17, 0), (64, 3, 0), (50, 2, 0), (16, 2, 0), (64, 2, 9), (80, 2, 1)]:
+        assert libns.ns_mg_create(ctypes.byref(h), N, P, dev, None, dtype) == binding.NS_ERR_INVALID_ARG, (N, P, dtype)
+        assert not h.value and len(libns.ns_mg_last_error(None)) > 0
+    assert libns.ns_mg_create(ctypes.byref(h), 64, 2, None, None, 0) == binding.NS_ERR_INVALID_ARG
+    assert libns.ns_mg_destroy(None) == binding.NS_ERR_INVALID_ARG and libns.ns_mg_step(None, 0.1) == binding.NS_ERR_INVALID_ARG
 
 
 def test_no_cpu_fallback(libns):
@@ -79,6 +86,10 @@ def test_no_cpu_fallback(libns):
     with pytest.raises(binding.NSError):
         binding.Solver(32, stream=0)
     assert libns.ns2d_create(ctypes.byref(h), 256, 4, None, 0, None) == binding.NS_ERR_CUDA
+    dev = (ctypes.c_int * 2)(0, 0)
+    assert libns.ns_mg_create(ctypes.byref(h), 64, 2, dev, None, 0) == binding.NS_ERR_CUDA
+    with pytest.raises(binding.NSError):
+        binding.SolverMG(64, [0, 0])
     with pytest.raises(binding.NSError):
         binding.Solver2D(256, stream=0)
 
