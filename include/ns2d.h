@@ -8,7 +8,10 @@
  * ensembles (Algorithm 1, L82-90) are the leading `batch` index -- in two dimensions typically a very large one.
  *
  * Conventions (those of ns.h unless stated)
- *   N         grid points per axis: 128, 256 or 512.  Padded grid M = 3N/2.
+ *   N         grid points per axis: any even N, 16 <= N <= 512.  The transforms run on the transform grid Nt = 128, 256 or 512
+ *             (the smallest >= N; ns2d_transform_grid) with the padded grid M = 3 Nt / 2 >= 3N/2 (the padded size
+ *             is rounded up to one the transforms are fast for); the state is truncated to the user's N and all public arrays have
+ *             the user's N, exactly as in ns.h; max|u| is a maximum over the M^2 points of the padded grid in use.
  *   spectral  complex interleaved of `dtype`, shape [batch][2][N][N/2+1], index [b][component][ikx][iky], iky >= 0 fastest (r2c
  *             half spectrum along y); normalised coefficients; entries with an index == N/2 are zero (reading A3).
  *   physical  reals of `dtype`, shape [batch][2][N][N], index [b][component][ix][iy], x_j = 2 pi j / N.
@@ -61,6 +64,7 @@ double ns2d_time(const ns2d_solver* h, int sample);
 /* Per-pass timing as ns_profile; the 4 passes are {b1 x inverse, b2 fused y (inverse + flux + forward), b3 x forward, b4 spectral}. */
 int ns2d_profile(ns2d_solver* h, int enable);
 int ns2d_profile_read(ns2d_solver* h, double* ms_out /*[4]*/, long long* count_out /*[4]*/);
+int ns2d_transform_grid(const ns2d_solver* h);   /* Nt; the padded grid is 3 Nt / 2 */
 long long ns2d_kernel_launches(const ns2d_solver* h);
 long long ns2d_device_bytes(const ns2d_solver* h);
 const char* ns2d_last_error(const ns2d_solver* h);

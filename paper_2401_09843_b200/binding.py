@@ -33,7 +33,7 @@ EXPORTS_MG = [
 EXPORTS_2D = [
     "ns2d_create", "ns2d_destroy", "ns2d_set_initial", "ns2d_set_spectral", "ns2d_get_spectral", "ns2d_rhs", "ns2d_step", "ns2d_step_cfl",
     "ns2d_step_dts", "ns2d_advance", "ns2d_max_velocity", "ns2d_get_fields", "ns2d_energy_spectrum", "ns2d_enstrophy_spectrum", "ns2d_time",
-    "ns2d_profile", "ns2d_profile_read", "ns2d_kernel_launches", "ns2d_device_bytes", "ns2d_last_error",
+    "ns2d_profile", "ns2d_profile_read", "ns2d_transform_grid", "ns2d_kernel_launches", "ns2d_device_bytes", "ns2d_last_error",
 ]
 
 
@@ -106,6 +106,7 @@ def lib():
         L.ns2d_time.restype = d
         L.ns2d_profile.argtypes = [vp, i]
         L.ns2d_profile_read.argtypes = [vp, vp, vp]
+        L.ns2d_transform_grid.argtypes = [vp]
         L.ns2d_kernel_launches.argtypes = [vp]
         L.ns2d_kernel_launches.restype = ctypes.c_longlong
         L.ns2d_device_bytes.argtypes = [vp]
@@ -453,6 +454,15 @@ class Solver2D:
         Z = np.empty((self.batch, int(nbins)), dtype=np.float64)
         self._check(lib().ns2d_enstrophy_spectrum(self._h, ctypes.c_void_p(Z.ctypes.data), int(nbins)))
         return Z
+
+    @property
+    def transform_grid(self):
+        """ns2d_transform_grid: the grid Nt >= N the transforms run on."""
+        return int(lib().ns2d_transform_grid(self._h))
+
+    @property
+    def padded_size(self):
+        return 3 * self.transform_grid // 2
 
     def profile(self, enable=True):
         self._check(lib().ns2d_profile(self._h, 1 if enable else 0))

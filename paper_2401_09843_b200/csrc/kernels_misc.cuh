@@ -418,22 +418,24 @@ generic_fft_kernel(cx<T>* __restrict__ A, int n, int log2m, int nsub, int axis, 
 // entry points (ns_set_initial, ns_get_fields, S_p, moments) of handles with such a size use it; never on the hot path.
 template <typename T>
 __global__ void __launch_bounds__(256)
-dft_lines_kernel(cx<T>* __restrict__ A, int n, int axis, int sign, long total_tiles, const cx<T>* __restrict__ gtw) {
+dft_lines_kernel(cx<T>* __restrict__ A, int n, int axis, int sign, long total_tiles, const cx<T>* __restrict__ gtw, int dim) {
     constexpr int TL = 8, PITCH = TL + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);   // [n][PITCH] input
     cx<T>* O = S + (size_t)n * PITCH;                // [n][PITCH] output
     const long tile = blockIdx.x;
     if (tile >= total_tiles) return;
-    const long n2 = (long)n * n;
-    const long tiles_per_cube = (n2 + TL - 1) / TL;   // the last tile of a cube may be ragged (n^2 not a multiple of 8)
+    // dim = 3: cubes [n][n][n], n^2 lines per cube and axis; dim = 2: planes [n][n] (axes 1 and 2 only), n lines per plane
+    const long nn = (long)n * n;
+    const long n2 = dim == 3 ? nn : n;                // lines per cube / plane
+    const long tiles_per_cube = (n2 + TL - 1) / TL;   // the last tile may be ragged (line count not a multiple of 8)
     const long cube = tile / tiles_per_cube;
     const long l0 = (tile % tiles_per_cube) * TL;
-    cx<T>* base = A + cube * n2 * n;
-    const long es = axis == 0 ? n2 : (axis == 1 ? n : 1);
+    cx<T>* base = A + cube * (dim == 3 ? nn * n : nn);
+    const long es = axis == 0 ? nn : (axis == 1 ? n : 1);
     auto line_base = [&](long l) -> long {
         if (axis == 0) return l;
-        if (axis == 1) return (l / n) * n2 + (l % n);
+        if (axis == 1) return dim == 3 ? (l / n) * nn + (l % n) : l;
         return l * n;
     };
     for (int e = threadIdx.x; e < n * TL; e += blockDim.x) {

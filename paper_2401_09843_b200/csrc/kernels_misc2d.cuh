@@ -16,7 +16,7 @@ namespace ns {
 //   In-place contract as spectral_kernel: out may alias Us or Un.
 template <typename T>
 __global__ void __launch_bounds__(256)
-spectral2d_kernel(const cx<T>* __restrict__ Th, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, long total,
+spectral2d_kernel(const cx<T>* __restrict__ Th, const cx<T>* Us, const cx<T>* Un, cx<T>* out, int N, int kmax, long total,
                   const T* __restrict__ dtab, T scale, T alpha, T beta, T gamma, const double* __restrict__ dt, int mode) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
@@ -30,7 +30,8 @@ spectral2d_kernel(const cx<T>* __restrict__ Th, const cx<T>* Us, const cx<T>* Un
     cx<T>* op = out + b * 2 * plane + o;
     const int kxi = wavenum(ix, N);
     const int k2i = kxi * kxi + iy * iy;
-    const bool dead = (ix == N / 2) || (k2i == 0);
+    // P_N of the user's grid: modes with a component >= kmax = (user N)/2 carry nothing (kmax = N/2 unless the transform grid is larger)
+    const bool dead = (kxi >= kmax) || (kxi <= -kmax) || (iy >= kmax) || (k2i == 0);
     cx<T> R[2] = {mk<T>(0, 0), mk<T>(0, 0)};
     const cx<T> u0 = us[0], u1 = us[plane];
     if (!dead) {
@@ -66,45 +67,56 @@ spectral2d_kernel(const cx<T>* __restrict__ Th, const cx<T>* Us, const cx<T>* Un
     }
 }
 
-// public [.][N][N/2+1] <-> internal [.][N][N/2]
+// public [.][Nu][Nu/2+1] (the user's grid) <-> internal [.][N][N/2] (the transform grid N >= Nu; modes outside K_Nu are zero)
+__device__ __forceinline__ int embed_index2d(int i, int N, int Nu) {   // internal index -> public index, -1 if outside K_Nu
+    const int k = wavenum(i, N);
+    if (k >= Nu / 2 || k <= -(Nu / 2)) return -1;
+    return k >= 0 ? k : k + Nu;
+}
 template <typename T>
-__global__ void to_internal2d_kernel(const cx<T>* __restrict__ pub, cx<T>* __restrict__ in, int N, long total) {
+__global__ void to_internal2d_kernel(const cx<T>* __restrict__ pub, cx<T>* __restrict__ in, int N, int Nu, long total) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
-    const int H = N / 2;
+    const int H = N / 2, Hu = Nu / 2;
     const int iy = (int)(idx % H);
     const long row = idx / H;  // (plane, ix)
-    cx<T> v = pub[row * (H + 1) + iy];
-    if ((int)(row % N) == N / 2) v = mk<T>(0, 0);
+    const int ix = (int)(row % N);
+    const long pl = row / N;
+    const int jx = embed_index2d(ix, N, Nu);
+    cx<T> v = mk<T>(0, 0);
+    if (jx >= 0 && iy < Hu) v = pub[(pl * Nu + jx) * (Hu + 1) + iy];
     in[idx] = v;
 }
 template <typename T>
-__global__ void to_public2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ pub, int N, long total_pub) {
+__global__ void to_public2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ pub, int N, int Nu, long total_pub) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total_pub) return;
-    const int H = N / 2;
-    const int iy = (int)(idx % (H + 1));
-    const long row = idx / (H + 1);
-    pub[idx] = iy == H ? mk<T>(0, 0) : in[row * H + iy];
+    const int H = N / 2, Hu = Nu / 2;
+    const int iy = (int)(idx % (Hu + 1));
+    const long row = idx / (Hu + 1);
+    const int jx = (int)(row % Nu);
+    const long pl = row / Nu;
+    cx<T> v = mk<T>(0, 0);
+    if (iy != Hu && jx != Hu) v = in[(pl * N + (jx < Hu ? jx : jx - Nu + N)) * H + iy];
+    pub[idx] = v;
 }
 
-// W: [batch][2][N][N] full complex unnormalised spectra -> U internal, scaled, Nyquist lines zeroed, Leray-projected (k != 0)
+// W: [batch][2][Nu][Nu] full complex unnormalised spectra on the user's grid -> U internal, scaled, Nyquist lines zeroed,
+// Leray-projected (k != 0)
 template <typename T>
-__global__ void init_project2d_kernel(const cx<T>* __restrict__ W, cx<T>* __restrict__ U, int N, long total, T scale) {
+__global__ void init_project2d_kernel(const cx<T>* __restrict__ W, cx<T>* __restrict__ U, int N, int Nu, long total, T scale) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
     const int H = N / 2;
     const int iy = (int)(idx % H);
     const int ix = (int)((idx / H) % N);
     const long b = idx / ((long)H * N);
-    const long plane = (long)N * H, sq = (long)N * N;
-    const bool nyq = ix == N / 2;
+    const long plane = (long)N * H, sq = (long)Nu * Nu;
+    const int jx = embed_index2d(ix, N, Nu);
+    const bool nyq = jx < 0 || iy >= Nu / 2;
     cx<T> u[2];
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
-        const cx<T> w = W[(b * 2 + c) * sq + (long)ix * N + iy];
-        u[c] = nyq ? mk<T>(0, 0) : scale * w;
-    }
+    for (int c = 0; c < 2; ++c) u[c] = nyq ? mk<T>(0, 0) : scale * W[(b * 2 + c) * sq + (long)jx * Nu + iy];
     const int kxi = wavenum(ix, N);
     const int k2i = kxi * kxi + iy * iy;
     if (!nyq && k2i > 0) {
@@ -117,20 +129,21 @@ __global__ void init_project2d_kernel(const cx<T>* __restrict__ W, cx<T>* __rest
     U[(b * 2 + 1) * plane + (long)ix * H + iy] = u[1];
 }
 
-// U internal -> W full complex Hermitian spectrum on the N grid (ky < 0 from conj of (-k))
+// U internal -> W full complex Hermitian spectrum on the user's Nu grid (ky < 0 from conj of (-k))
 template <typename T>
-__global__ void expand_hermitian2d_kernel(const cx<T>* __restrict__ U, cx<T>* __restrict__ W, int N, long total) {
+__global__ void expand_hermitian2d_kernel(const cx<T>* __restrict__ U, cx<T>* __restrict__ W, int N, int Nu, long total) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
-    const int H = N / 2;
-    const int iy = (int)(idx % N);
-    const int ix = (int)((idx / N) % N);
-    const long pl = idx / ((long)N * N);
+    const int H = N / 2, Hu = Nu / 2;
+    const int jy = (int)(idx % Nu);
+    const int jx = (int)((idx / Nu) % Nu);
+    const long pl = idx / ((long)Nu * Nu);
     const long plane = (long)N * H;
     cx<T> v = mk<T>(0, 0);
-    if (ix != N / 2 && iy != N / 2) {
-        if (iy < H) v = U[pl * plane + (long)ix * H + iy];
-        else v = conj(U[pl * plane + (long)((N - ix) % N) * H + (N - iy)]);
+    if (jx != Hu && jy != Hu) {
+        const int kx = jx < Hu ? jx : jx - Nu, ky = jy < Hu ? jy : jy - Nu;
+        if (ky >= 0) v = U[pl * plane + (long)(kx >= 0 ? kx : kx + N) * H + ky];
+        else v = conj(U[pl * plane + (long)(kx > 0 ? N - kx : -kx) * H - ky]);
     }
     W[idx] = v;
 }

@@ -31,6 +31,7 @@ struct ns2d_solver {
     virtual int spectrum(double* E, int nbins, bool enstrophy) = 0;
     virtual double time(int sample) = 0;
     virtual long long device_bytes() const = 0;
+    virtual int transform_grid() const = 0;
     virtual int profile(int enable) = 0;
     virtual int profile_read(double* ms, long long* cnt) = 0;
 };
@@ -59,7 +60,9 @@ enum { DT_UNIFORM = 0, DT_ARRAY = 1, DT_CFL = 2 };
 template <typename T>
 class Solver2D final : public ns2d_solver {
 public:
-    int N, L, M, H, batch;
+    int N, L, M, H, batch;   // N = the transform grid (128, 256 or 512), M = 3N/2 its padded grid
+    int Nu;                  // the user's grid (public arrays, truncation set, dx, eps_N, m_N); Nu <= N
+    cx<T>* gNu = nullptr;    // exp(2 pi i j / Nu), j < Nu
     int device = 0, num_sms = 0;
     ns_params prm;
     cudaStream_t st;
@@ -80,7 +83,8 @@ public:
     double pms[4] = {0, 0, 0, 0};
     long long pcnt[4] = {0, 0, 0, 0};
 
-    Solver2D(int N_, int batch_, const ns_params& p, cudaStream_t s) : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), prm(p), st(s) {}
+    Solver2D(int Nu_, int N_, int batch_, const ns_params& p, cudaStream_t s)
+        : N(N_), L(N_ / 2), M(3 * N_ / 2), H(N_ / 2), batch(batch_), Nu(Nu_), prm(p), st(s) {}
     ~Solver2D() override {
         for (cudaEvent_t e : ev) cudaEventDestroy(e);
         if (arena) cudaFree(arena);
@@ -125,6 +129,7 @@ public:
         const size_t oU = take(nS * sizeof(cx<T>)), oV = take(nS * sizeof(cx<T>));
         const size_t oX = take(nX * sizeof(cx<T>)), oY = take(nY * sizeof(cx<T>)), oZ = take(nZ * sizeof(cx<T>));
         const size_t otw = take(twiddle_table_len(L) * sizeof(cx<T>));
+        const size_t ogu = take((size_t)Nu * sizeof(cx<T>));
         const size_t oD = take(ndt * sizeof(T));
         const size_t odt = take(b * sizeof(double)), ot = take(b * sizeof(double)), osc = take(b * sizeof(double));
         const size_t oum = take(b * sizeof(unsigned long long)), obad = take(b * sizeof(int));
@@ -140,6 +145,7 @@ public:
         if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc");
         U = (cx<T>*)(arena + oU); V = (cx<T>*)(arena + oV); X = (cx<T>*)(arena + oX); Y = (cx<T>*)(arena + oY); Z = (cx<T>*)(arena + oZ);
         twbase = (cx<T>*)(arena + otw);
+        gNu = (cx<T>*)(arena + ogu);
         dtab = (T*)(arena + oD);
         dt_dev = (double*)(arena + odt); t_dev = (double*)(arena + ot); scal_dev = (double*)(arena + osc);
         umax2 = (unsigned long long*)(arena + oum);
@@ -147,7 +153,14 @@ public:
         red_dev = (double*)(arena + ored);
         const std::vector<cx<T>> htw = build_twiddle_block<T>(L);
         std::vector<T> hd(ndt);
-        for (size_t k2 = 0; k2 < ndt; ++k2) hd[k2] = (T)dissipation_rate2d(prm, N, (double)k2);
+        for (size_t k2 = 0; k2 < ndt; ++k2) hd[k2] = (T)dissipation_rate2d(prm, Nu, (double)k2);   // eps_N, m_N of the USER's N
+        std::vector<cx<T>> hgu((size_t)Nu);
+        for (int j = 0; j < Nu; ++j) {
+            const long double a = 6.283185307179586476925286766559005768L * (long double)j / (long double)Nu;
+            hgu[(size_t)j].x = (T)cosl(a);
+            hgu[(size_t)j].y = (T)sinl(a);
+        }
+        NS_CK(cudaMemcpyAsync(gNu, hgu.data(), hgu.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemcpyAsync(twbase, htw.data(), htw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemcpyAsync(dtab, hd.data(), hd.size() * sizeof(T), cudaMemcpyHostToDevice, st));
         NS_CK(cudaMemsetAsync(t_dev, 0, b * sizeof(double), st));
@@ -157,6 +170,7 @@ public:
         return NS_OK;
     }
     long long device_bytes() const override { return (long long)arena_bytes; }
+    int transform_grid() const override { return N; }
 
     int check_finite() {
         std::vector<int> bad((size_t)batch);
@@ -195,7 +209,7 @@ public:
         const long total = (long)batch * N * H;
         const T scale = (T)(1.0 / ((double)M * M * z_fused_output_scale(L)));
         tick(3);
-        spectral2d_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y, Us, Un, out, N, total, dtab, scale, (T)alpha, (T)beta, (T)gamma,
+        spectral2d_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(Y, Us, Un, out, N, Nu / 2, total, dtab, scale, (T)alpha, (T)beta, (T)gamma,
                                                                       dt_dev, mode);
         NS_LAUNCHED("b4 spectral2d_kernel");
         tick(-1);
@@ -216,7 +230,7 @@ public:
             set_dt_array_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, scal_dev, umax2, bad_dev, batch);
             NS_LAUNCHED("set_dt_array");
         } else {
-            cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, umax2, bad_dev, cfl, 2.0 * 3.14159265358979323846 / N, t_end, batch);
+            cfl_finalize_kernel<<<gb, 128, 0, st>>>(dt_dev, t_dev, umax2, bad_dev, cfl, 2.0 * 3.14159265358979323846 / Nu, t_end, batch);
             NS_LAUNCHED("cfl_finalize");
         }
         if ((rc = spectral(U, nullptr, V, 0.0, 1.0, 1.0, 1)) != NS_OK) return rc;                       // u1 = u + dt R(u)
@@ -276,9 +290,9 @@ public:
     }
 
     int export_spectral(const cx<T>* src, void* out, ns_memspace ms) {
-        const long total_pub = (long)batch * 2 * N * (H + 1);
+        const long total_pub = (long)batch * 2 * Nu * (Nu / 2 + 1);
         cx<T>* dst = ms == NS_DEVICE ? (cx<T>*)out : Y;
-        to_public2d_kernel<T><<<blocks_for(total_pub, 256), 256, 0, st>>>(src, dst, N, total_pub);
+        to_public2d_kernel<T><<<blocks_for(total_pub, 256), 256, 0, st>>>(src, dst, N, Nu, total_pub);
         NS_LAUNCHED("to_public2d");
         if (ms == NS_HOST) {
             NS_CK(cudaMemcpyAsync(out, Y, (size_t)total_pub * sizeof(cx<T>), cudaMemcpyDeviceToHost, st));
@@ -301,14 +315,14 @@ public:
     }
     int set_spectral(const void* in, ns_memspace ms) override {
         if (!in) return fail(NS_ERR_INVALID_ARG, "input pointer is NULL");
-        const long total_pub = (long)batch * 2 * N * (H + 1);
+        const long total_pub = (long)batch * 2 * Nu * (Nu / 2 + 1);
         const cx<T>* src = (const cx<T>*)in;
         if (ms == NS_HOST) {
             NS_CK(cudaMemcpyAsync(Y, in, (size_t)total_pub * sizeof(cx<T>), cudaMemcpyHostToDevice, st));
             src = Y;
         }
         const long total = (long)batch * 2 * N * H;
-        to_internal2d_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, U, N, total);
+        to_internal2d_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(src, U, N, Nu, total);
         NS_LAUNCHED("to_internal2d");
         NS_CK(cudaMemsetAsync(bad_dev, 0, (size_t)batch * sizeof(int), st));
         if (ms == NS_HOST) NS_CK(cudaStreamSynchronize(st));
@@ -316,23 +330,37 @@ public:
         return NS_OK;
     }
 
+    // unpadded 2-D transform on the USER's grid (planes of Nu^2 complex), in place: mixed radix when Nu = p 2^a with p in
+    // {1, 3, 5, 7, 15} and Nu a multiple of 8, else the plain DFT
     int generic_fft2(cx<T>* W, long planes, int sign) {
-        int log2n = 0;
-        while ((1 << log2n) < N) ++log2n;
-        const long tiles = planes * (long)N / 8;
-        const size_t smem = (size_t)N * 9 * sizeof(cx<T>);
-        if (smem > 48 * 1024)
-            NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        for (int axis = 1; axis < 3; ++axis) {
-            generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, N, log2n, 1, axis, sign, tiles, tw().gN, 2);
-            NS_LAUNCHED("generic_fft 2d");
+        int odd = Nu, log2m = 0;
+        while (odd % 2 == 0) { odd /= 2; ++log2m; }
+        const bool fast = (odd == 1 || odd == 3 || odd == 5 || odd == 7 || odd == 15) && Nu % 8 == 0;
+        if (fast) {
+            const long tiles = planes * (long)Nu / 8;
+            const size_t smem = (size_t)Nu * 9 * sizeof(cx<T>);
+            if (smem > 48 * 1024)
+                NS_CK(cudaFuncSetAttribute(generic_fft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            for (int axis = 1; axis < 3; ++axis) {
+                generic_fft_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, Nu, log2m, odd, axis, sign, tiles, gNu, 2);
+                NS_LAUNCHED("generic_fft 2d");
+            }
+        } else {
+            const long tiles = planes * (((long)Nu + 7) / 8);
+            const size_t smem = (size_t)2 * Nu * 9 * sizeof(cx<T>);
+            if (smem > 48 * 1024)
+                NS_CK(cudaFuncSetAttribute(dft_lines_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            for (int axis = 1; axis < 3; ++axis) {
+                dft_lines_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, Nu, axis, sign, tiles, gNu, 2);
+                NS_LAUNCHED("dft_lines 2d");
+            }
         }
         return NS_OK;
     }
     int set_initial(const void* in, ns_memspace ms) override {
         if (!in) return fail(NS_ERR_INVALID_ARG, "input pointer is NULL");
         const long planes = (long)batch * 2;
-        const long total = planes * N * N;
+        const long total = planes * Nu * Nu;
         const T* src = (const T*)in;
         if (ms == NS_HOST) {
             NS_CK(cudaMemcpyAsync(Y, in, (size_t)total * sizeof(T), cudaMemcpyHostToDevice, st));
@@ -343,7 +371,7 @@ public:
         int rc = generic_fft2(X, planes, -1);
         if (rc != NS_OK) return rc;
         const long tot = (long)batch * N * H;
-        init_project2d_kernel<T><<<blocks_for(tot, 256), 256, 0, st>>>(X, U, N, tot, (T)(1.0 / ((double)N * N)));
+        init_project2d_kernel<T><<<blocks_for(tot, 256), 256, 0, st>>>(X, U, N, Nu, tot, (T)(1.0 / ((double)Nu * Nu)));
         NS_LAUNCHED("init_project2d");
         NS_CK(cudaMemsetAsync(t_dev, 0, (size_t)batch * sizeof(double), st));
         NS_CK(cudaMemsetAsync(bad_dev, 0, (size_t)batch * sizeof(int), st));
@@ -355,8 +383,8 @@ public:
         if (!has_state) return fail(NS_ERR_STATE, "no initial state set");
         if (!out) return fail(NS_ERR_INVALID_ARG, "output pointer is NULL");
         const long planes = (long)batch * 2;
-        const long total = planes * N * N;
-        expand_hermitian2d_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, total);
+        const long total = planes * Nu * Nu;
+        expand_hermitian2d_kernel<T><<<blocks_for(total, 256), 256, 0, st>>>(U, X, N, Nu, total);
         NS_LAUNCHED("expand_hermitian2d");
         int rc = generic_fft2(X, planes, +1);
         if (rc != NS_OK) return rc;
@@ -424,8 +452,8 @@ public:
 };
 
 template <typename T>
-int create_typed2d(ns2d_solver** out, int N, int batch, const ns_params& p, cudaStream_t st) {
-    Solver2D<T>* s = new Solver2D<T>(N, batch, p, st);
+int create_typed2d(ns2d_solver** out, int Nu, int N, int batch, const ns_params& p, cudaStream_t st) {
+    Solver2D<T>* s = new Solver2D<T>(Nu, N, batch, p, st);
     int rc = s->init();
     if (rc != NS_OK) {
         g_create_error2d = s->err;
@@ -444,9 +472,12 @@ int ns2d_create(ns2d_solver** out, int N, int batch, const ns_params* p, ns_dtyp
     g_create_error2d.clear();
     if (!out) { g_create_error2d = "out is NULL"; return NS_ERR_INVALID_ARG; }
     *out = nullptr;
-    if (N != 128 && N != 256 && N != 512) { g_create_error2d = "N must be 128, 256 or 512"; return NS_ERR_INVALID_ARG; }
+    // any even N up to 512; the transforms run on the next transform grid Nt in {128, 256, 512} (the padded size is
+    // rounded up to one the transforms are fast for), the state truncated to the user's N -- as ns.h
+    if (N < 16 || N > 512 || (N % 2) != 0) { g_create_error2d = "N must be even with 16 <= N <= 512"; return NS_ERR_INVALID_ARG; }
+    const int Nt = N <= 128 ? 128 : (N <= 256 ? 256 : 512);
     if (batch < 1) { g_create_error2d = "batch must be >= 1"; return NS_ERR_INVALID_ARG; }
-    if ((long)batch * (3 * N / 2) >= (1L << 31)) { g_create_error2d = "batch too large"; return NS_ERR_INVALID_ARG; }
+    if ((long)batch * (3 * Nt / 2) >= (1L << 31)) { g_create_error2d = "batch too large"; return NS_ERR_INVALID_ARG; }
     if (dtype != NS_F64 && dtype != NS_F32) { g_create_error2d = "unknown dtype"; return NS_ERR_INVALID_ARG; }
     ns_params prm;
     std::memset(&prm, 0, sizeof prm);
@@ -466,7 +497,7 @@ int ns2d_create(ns2d_solver** out, int N, int batch, const ns_params* p, ns_dtyp
         return NS_ERR_CUDA;
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    return dtype == NS_F64 ? create_typed2d<double>(out, N, batch, prm, st) : create_typed2d<float>(out, N, batch, prm, st);
+    return dtype == NS_F64 ? create_typed2d<double>(out, N, Nt, batch, prm, st) : create_typed2d<float>(out, N, Nt, batch, prm, st);
 }
 int ns2d_destroy(ns2d_solver* h) {
     if (!h) return NS_ERR_INVALID_ARG;
@@ -492,6 +523,7 @@ double ns2d_time(const ns2d_solver* h, int sample) {
 }
 int ns2d_profile(ns2d_solver* h, int enable) { NS2_H(h); return h->profile(enable); }
 int ns2d_profile_read(ns2d_solver* h, double* ms, long long* cnt) { NS2_H(h); return h->profile_read(ms, cnt); }
+int ns2d_transform_grid(const ns2d_solver* h) { return h ? h->transform_grid() : 0; }
 long long ns2d_kernel_launches(const ns2d_solver* h) { return h ? h->launches : 0; }
 long long ns2d_device_bytes(const ns2d_solver* h) { return h ? h->device_bytes() : 0; }
 const char* ns2d_last_error(const ns2d_solver* h) { return h ? h->err.c_str() : g_create_error2d.c_str(); }

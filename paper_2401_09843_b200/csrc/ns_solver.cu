@@ -483,7 +483,7 @@ public:
             if (smem > 48 * 1024)
                 NS_CK(cudaFuncSetAttribute(dft_lines_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             for (int axis = 0; axis < 3; ++axis) {
-                dft_lines_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, Nu, axis, sign, tiles, gNu);
+                dft_lines_kernel<T><<<(unsigned)tiles, 256, smem, st>>>(W, Nu, axis, sign, tiles, gNu, 3);
                 NS_LAUNCHED("dft_lines");
             }
         }

@@ -166,3 +166,38 @@ def test_2d_fp32_and_errors(ns, oracle2d):
     t.step(1e-3)
     assert t.kernel_launches() - n0 == 1 + 3 * 4 + 1      # to_internal + 3 stages x (b1, b2, b3, b4) + dt setup
     assert t.device_bytes() > 0
+
+
+@pytest.mark.parametrize("N", [48, 100, 200])
+def test_2d_general_even_n_on_a_larger_transform_grid(ns, oracle2d, N):
+    """An N that is not 128 / 256 / 512 runs on the next of those as transform grid (padded grid 3 Nt / 2 > 3N/2), the
+    state truncated to the user's N: against the 2-D oracle at the user's N with the SAME padded size -- set_initial (mixed-radix or
+    plain DFT on the N grid), get_fields, RHS (every entry; also against M = 3N/2), max|u|, CFL steps, spectra."""
+    u = field2(N, 600 + N) + 0.2 * inputs.normal01(N, 9, 2 * N * N).reshape(2, N, N)
+    kw = dict(nu=0.001, eps=0.05, s=1.5)
+    s = ns.Solver2D(N, batch=1, **kw)
+    Nt, M = s.transform_grid, s.padded_size
+    assert Nt in (128, 256) and Nt > N and M > 3 * N // 2
+    s.set_initial(u[None])
+    uh = oracle2d.set_initial(N, u)
+    got = s.get_spectral()[0]
+    assert got.shape == uh.shape and rel(got, uh) < 1e-13
+    assert rel(s.get_fields()[0], oracle2d.get_fields(N, uh)) < 1e-13
+    s.set_spectral(uh[None])
+    assert np.array_equal(s.get_spectral()[0], uh)
+    p = oracle2d.Params(**kw)
+    want = oracle2d.rhs_parts(N, p, uh, M)
+    r = s.rhs()[0]
+    assert rel(r, want["r"]) < TOL_RHS_F64
+    assert rel(r, oracle2d.rhs(N, p, uh)) < TOL_RHS_F64
+    assert np.all(r[:, N // 2] == 0) and np.all(r[:, :, N // 2] == 0)
+    assert abs(s.max_velocity()[0] - want["umax"]) < 1e-13 * want["umax"]
+    worst = 0.0
+    for i in range(4):
+        dts = s.step_cfl(0.2, 1e9)
+        assert abs(dts[0] - 0.2 * (2 * np.pi / N) / oracle2d.max_velocity(N, uh, M)) < 1e-12 * dts[0]
+        uh = oracle2d.step(N, p, uh, dts[0], M)
+        worst = max(worst, rel(s.get_spectral()[0], uh))
+        assert worst < TOL_STEPS_F64, (i, worst)
+    assert np.abs(s.energy_spectrum(N)[0] - oracle2d.energy_spectrum(N, uh, N)).max() < 1e-13
+    print(f"2-D N = {N} on transform grid {Nt}: worst rel-L2 over 4 steps {worst:.2e}")
