@@ -30,9 +30,6 @@
 
 namespace ns {
 
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 // box of the 3-D tensor (2 * columns scalars, rows, slabs) at (c0, c1, c2) -> shared memory, completion on `bar`
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
     asm volatile(

@@ -43,7 +43,7 @@ template <typename T, int L> struct ZPGeo {
     // odd lane groups are shifted by 4 elements (64 B) when G = 4 so that the two groups of a quarter warp hit disjoint banks
     static constexpr int LGPITCH = 2 * SLOT + (G == 4 ? 4 : 0);
     static constexpr int IN_UNIT = PL * LGPITCH;                         // input ring of one unit, complex elements
-    static constexpr size_t UNIT_BYTES = (size_t)(IN_UNIT + 3 * REGION) * sizeof(cx<T>) + (size_t)PL * 2 * sizeof(uint64_t);
+    static constexpr size_t UNIT_BYTES = (size_t)(IN_UNIT + 3 * REGION) * sizeof(cx<T>) + (size_t)(PL * 2 + 2) * sizeof(uint64_t);
     static constexpr uint32_t C16 = 16 * sizeof(T) / 4;                  // TMEM columns of 16 scalars
     static constexpr uint32_t WCOLS = 4 * C16;                           // TMEM columns per warp: 4 fields
     static constexpr uint32_t TWCOLS = 4 * C16;                          // the thread's 16 inter-stage + 16 radix-3 twiddles (complex)
@@ -66,11 +66,17 @@ template <int G> __host__ __device__ constexpr int zp_unperm(int i) {
 // Sw: the warp's exchange region (16 rows x 32 columns, XOR-swizzled: element (row, col) at row*32 + (col ^ (row & 7))).
 // ttw: tensor-memory address of the thread's inter-stage twiddles w_L^{r1 t}, r1 = 0..15 (they depend on the lane only, so
 // the warps that share a TMEM lane quarter share them; fetched a few at a time they cost neither registers nor L1).
+// cdone / cparity (optional): mbarrier phase to wait for before the exchange region is overwritten -- the phase the three q
+// warps of the unit complete when they have finished READING the regions in the combine of the previous forward job.  The
+// wait sits after the register-only first stage, so a warp that left the combine early has its input formation and a radix-16
+// stage to do before it can block (the combine is split unevenly over the warps on purpose, zp_combine_store).
 template <typename T, int L>
-__device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int t, int lgcol, uint32_t ttw) {
+__device__ __forceinline__ void zp_transform(cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int t, int lgcol, uint32_t ttw,
+                                             uint64_t* cdone = nullptr, uint32_t cparity = 0) {
     constexpr int G = ZPGeo<T, L>::G, Hc = ZPGeo<T, L>::Hc;
     constexpr int CH = tmem_cx_chunk<T>();
     fft_reg<16, +1, T>(v);
+    if (cdone != nullptr) mbar_wait(cdone, cparity);
 #pragma unroll
     for (int ch = 0; ch < 16 / CH; ++ch) {
         T wr[CH], wi[CH];
@@ -273,7 +279,8 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
     unsigned char* ubase = smem_raw + (size_t)unit * Geo::UNIT_BYTES;
     cx<T>* In = reinterpret_cast<cx<T>*>(ubase);                       // [PL] x (2 slots x 2 lines x L), pitch LGPITCH
     cx<T>* Ex = In + Geo::IN_UNIT;                                      // [3][REGION]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(Ex + 3 * REGION);      // [PL][2]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Ex + 3 * REGION);      // [PL][2] input ring, then [1] combine-done
+    uint64_t* cdone = bars + 2 * PL;
     cx<T>* Sw = Ex + q * REGION;
     const cx<T>* Ulg = In + (size_t)lg * Geo::LGPITCH;
     uint64_t* bar_lg = bars + lg * 2;
@@ -298,6 +305,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
 
     if (threadIdx.x % 96 == 0) {
         for (int k = 0; k < 2 * PL; ++k) mbar_init(bars + k, 1);
+        mbar_init(cdone, 3);            // one arrival per q warp
         mbar_fence_init();
     }
     if (warp == 0) tmem_alloc(&tslot, NCOLS);
@@ -321,6 +329,7 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
         for (int k = 0; k < 2; ++k) issue(pair, k, k);
     }
 
+    unsigned nfwd = 0;      // forward jobs this warp has completed = phases of cdone it has arrived on
     for (int it = 0; pair < total_pairs; pair += stride, ++it) {
         const unsigned lineA = 2 * pair;
         const unsigned b = lineA / MM;
@@ -388,7 +397,8 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                     if (lane == 0) atomic_max_sq(umax2 + b, lmax);
                 }
             }
-            zp_transform<T, L>(v, Sw, lane, t, lgcol, ttw);
+            // the regions may be overwritten only when all three warps have finished the combine of the last forward job
+            zp_transform<T, L>(v, Sw, lane, t, lgcol, ttw, nfwd > 0 ? cdone : nullptr, (nfwd - 1) & 1u);
             if (inv) {
 #pragma unroll
                 for (int ch = 0; ch < 16 / VPA; ++ch) {
@@ -420,7 +430,10 @@ z_pair_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM
                     Ob = Ol + (p0 ? 3 : 2) * cs;
                 }
                 zp_combine_store<T, L>(Ex, lgcol, Oa, Ob, q, t);
-                named_bar_sync(bar_id, 96);  // combine reads done before the regions are reused
+                // combine reads done: arrive (no wait here -- the wait is in the next zp_transform, before the regions are reused)
+                __syncwarp();
+                if (lane == 0) mbar_arrive(cdone);
+                ++nfwd;
             }
         }
     }
