@@ -29,6 +29,9 @@ EXPORTS_MG = [
     "ns_mg_create", "ns_mg_destroy", "ns_mg_set_spectral", "ns_mg_get_spectral", "ns_mg_rhs", "ns_mg_step", "ns_mg_step_cfl",
     "ns_mg_max_velocity", "ns_mg_time", "ns_mg_exchange_bytes", "ns_mg_kernel_launches", "ns_mg_device_bytes", "ns_mg_last_error",
 ]
+# include/ns_noalloc.h: the allocation-free entry point
+EXPORTS_NOALLOC = ["ns_noalloc_energy_spectrum"]
+NS_NOALLOC_MAX_VALUES = 16384
 # include/ns2d.h: the two-dimensional solver
 EXPORTS_2D = [
     "ns2d_create", "ns2d_destroy", "ns2d_set_initial", "ns2d_set_spectral", "ns2d_get_spectral", "ns2d_rhs", "ns2d_step", "ns2d_step_cfl",
@@ -128,6 +131,8 @@ def lib():
             getattr(L, name).restype = ctypes.c_longlong
         L.ns_mg_last_error.argtypes = [vp]
         L.ns_mg_last_error.restype = ctypes.c_char_p
+        # include/ns_noalloc.h
+        L.ns_noalloc_energy_spectrum.argtypes = [vp, i, i, i, i, vp, i, vp, ctypes.c_char_p, i]
         _lib = L
     return _lib
 
@@ -552,3 +557,25 @@ class SolverMG:
 
     def device_bytes(self):
         return int(lib().ns_mg_device_bytes(self._h))
+
+
+def energy_spectrum_noalloc(u_hat, N, nbins, out=None, stream=None):
+    """ns_noalloc_energy_spectrum (include/ns_noalloc.h): shell spectrum of a spectral state held by the caller in DEVICE memory
+    (torch CUDA tensor [batch][3][N][N][N/2+1], complex128 or complex64), accumulated in the library's static device scratch: no
+    allocation inside the call.  `out`: a torch CUDA float64 tensor or a numpy float64 array [batch][nbins] (default: a new numpy
+    array).  batch * nbins <= NS_NOALLOC_MAX_VALUES.  Argument marshalling only."""
+    if not _is_torch(u_hat) or not u_hat.is_cuda or not u_hat.is_contiguous():
+        raise TypeError("u_hat must be a contiguous torch CUDA tensor")
+    batch = int(u_hat.shape[0])
+    if tuple(u_hat.shape) != (batch, 3, int(N), int(N), int(N) // 2 + 1):
+        raise ValueError(f"u_hat has shape {tuple(u_hat.shape)}, expected [batch][3][N][N][N/2+1]")
+    dtype = NS_F64 if u_hat.element_size() == 16 else NS_F32
+    if out is None:
+        out = np.empty((batch, int(nbins)), dtype=np.float64)
+    p, ms, _k = _buf(out, writable=True)
+    err = ctypes.create_string_buffer(256)
+    rc = lib().ns_noalloc_energy_spectrum(ctypes.c_void_p(u_hat.data_ptr()), int(N), batch, dtype, int(nbins), p, ms,
+                                          ctypes.c_void_p(int(stream)) if stream else None, err, 256)
+    if rc != NS_OK:
+        raise NSError(rc, err.value.decode())
+    return out

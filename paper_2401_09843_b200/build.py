@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libns.so")
-SOURCES = ["ns_solver.cu", "ns2d_solver.cu", "ns_mg_solver.cu", "ns_fft_f64.cu", "ns_fft_f32.cu", "ns_fft_smooth_f64.cu", "ns_fft_smooth_f32.cu"]
+SOURCES = ["ns_solver.cu", "ns2d_solver.cu", "ns_mg_solver.cu", "ns_noalloc.cu", "ns_fft_f64.cu", "ns_fft_f32.cu", "ns_fft_smooth_f64.cu", "ns_fft_smooth_f32.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "--fmad=true"]
