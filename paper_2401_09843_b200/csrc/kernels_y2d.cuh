@@ -36,7 +36,8 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
     unsigned char* ubase = smem_raw + (size_t)unit * Geo::UNIT_BYTES;
     cx<T>* In = reinterpret_cast<cx<T>*>(ubase);
     cx<T>* Ex = In + Geo::IN_UNIT;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(Ex + 3 * REGION);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Ex + 3 * REGION);      // [PL][2] input ring, then [1] combine-done
+    uint64_t* cdone = bars + 2 * PL;
     cx<T>* Sw = Ex + q * REGION;
     const cx<T>* Ulg = In + (size_t)lg * Geo::LGPITCH;
     uint64_t* bar_lg = bars + lg * 2;
@@ -57,6 +58,7 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
 
     if (threadIdx.x % 96 == 0) {
         for (int k = 0; k < 2 * PL; ++k) mbar_init(bars + k, 1);
+        mbar_init(cdone, 3);            // one arrival per q warp (kernels_zpair.cuh: split arrive / wait)
         mbar_fence_init();
     }
     if (warp == 0) tmem_alloc(&tslot, NCOLS);
@@ -86,7 +88,8 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
         const cx<T>* Ua = Ulg + (it & 1) * SLOT;
         cx<T> v[16];
         zp_form_inverse<T, L>(v, Ua, Ua + L, q, t, tw3);
-        zp_transform<T, L>(v, Sw, lane, t, lgcol, ttw);
+        // the regions may be overwritten only when all three warps have finished the combine of the previous line
+        zp_transform<T, L>(v, Sw, lane, t, lgcol, ttw, it > 0 ? cdone : nullptr, (uint32_t)((it - 1) & 1));
         // physical values u1 + i u2 at the points p = t + G j (register zp_perm(j)); flux, conjugated, in natural order
         cx<T> w[16];
         if (umax2 != nullptr) {
@@ -107,7 +110,8 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
         // all three warps have consumed this line's slot: refill it with the line after next
         if (issuer && line + 2 * (unsigned long long)stride < total_lines) issue(line + 2 * stride, it + 2);
         zp_combine_store<T, L>(Ex, lgcol, Oa, Oa + cs, q, t);
-        named_bar_sync(bar_id, 96);
+        __syncwarp();                     // combine reads done: arrive; the wait is in the next inverse transform
+        if (lane == 0) mbar_arrive(cdone);
     }
     tmem_fence_before_sync();
     __syncthreads();
