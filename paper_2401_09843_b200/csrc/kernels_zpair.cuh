@@ -124,10 +124,13 @@ __device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, i
     };
     // q = 0: n = t + G i, i < 4;  q = 1: n = 4G + t + G i, i < 2;  q = 2: n = 6G + t + G i, i < 2;  n = 8G = L/2: lane t = 0 of q = 2
     const int n0 = q == 0 ? t : (q == 1 ? 4 * G + t : 6 * G + t);
+    // The regions hold the CONJUGATES of F_0, G_1, G_2 (zp_post_forward stores the raw output of the inverse butterflies: the
+    // conjugation of F(x) = conj(F^-1(conj x)) costs nothing here, it is only signs in the additions below).  With f0, g1, g2 the
+    // stored values: A' = f0 + S = conj(A),  C' = f0 - S/2 - i (sqrt3/2) D = conj(C).
     auto one = [&](cx<T> f0, cx<T> g1, cx<T> g2, cx<T>& A, cx<T>& C) {
         const cx<T> S = g1 + g2, D = g1 - g2;
         A = f0 + S;
-        C = mk<T>(f0.x - (T)0.5 * S.x - h3 * D.y, f0.y - (T)0.5 * S.y + h3 * D.x);
+        C = mk<T>(f0.x - (T)0.5 * S.x + h3 * D.y, f0.y - (T)0.5 * S.y - h3 * D.x);
     };
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
@@ -146,15 +149,16 @@ __device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, i
             cx<T> An, Cn, Am, Cm;
             one(f0[k], g1[k], g2[k], An, Cn);
             one(f0m[k], g1m[k], g2m[k], Am, Cm);
+            // (An, Cn, Am, Cm are the conjugates A', C' of the quantities in the formulas of kernels_z.cuh)
             if (n == 0) {
                 stg_stream(Oa, mk<T>(An.x + An.x, 0));
-                stg_stream(Ob, mk<T>(An.y + An.y, 0));
+                stg_stream(Ob, mk<T>(-An.y - An.y, 0));
             } else {
                 const int m = L - n;
-                stg_stream(Oa + n, mk<T>(An.x + Cm.x, An.y - Cm.y));
-                stg_stream(Ob + n, mk<T>(An.y + Cm.y, Cm.x - An.x));
-                stg_stream(Oa + m, mk<T>(Am.x + Cn.x, Am.y - Cn.y));
-                stg_stream(Ob + m, mk<T>(Am.y + Cn.y, Cn.x - Am.x));
+                stg_stream(Oa + n, mk<T>(An.x + Cm.x, Cm.y - An.y));
+                stg_stream(Ob + n, mk<T>(-An.y - Cm.y, Cm.x - An.x));
+                stg_stream(Oa + m, mk<T>(Am.x + Cn.x, Cn.y - Am.y));
+                stg_stream(Ob + m, mk<T>(-Am.y - Cn.y, Cn.x - Am.x));
             }
         }
     }
@@ -162,8 +166,8 @@ __device__ __forceinline__ void zp_combine_store(const cx<T>* __restrict__ Su, i
         constexpr int n = L / 2;
         cx<T> An, Cn;
         one(at(0, n), at(1, n), at(2, n), An, Cn);
-        stg_stream(Oa + n, mk<T>(An.x + Cn.x, An.y - Cn.y));
-        stg_stream(Ob + n, mk<T>(An.y + Cn.y, Cn.x - An.x));
+        stg_stream(Oa + n, mk<T>(An.x + Cn.x, Cn.y - An.y));
+        stg_stream(Ob + n, mk<T>(-An.y - Cn.y, Cn.x - An.x));
     }
 }
 
@@ -226,8 +230,8 @@ __device__ __forceinline__ void zp_form_inverse(cx<T> (&v)[16], const cx<T>* __r
     }
 }
 
-// Output of a forward job (run through the inverse butterflies on conjugated input): G_q[k] = conj(v) W^{-qk} into the warp's
-// region in natural order, k = t + G j at row j, column lane.
+// Output of a forward job (run through the inverse butterflies on conjugated input): G_q[k] = conj(v) W^{-qk}; its CONJUGATE
+// v W^{qk} goes into the warp's region in natural order, k = t + G j at row j, column lane (zp_combine_store undoes it in its signs).
 template <typename T, int L>
 __device__ __forceinline__ void zp_post_forward(const cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int q, uint32_t tw3) {
     constexpr int G = ZPGeo<T, L>::G, CH = tmem_cx_chunk<T>();
@@ -240,10 +244,10 @@ __device__ __forceinline__ void zp_post_forward(const cx<T> (&v)[16], cx<T>* __r
         for (int e = 0; e < CH; ++e) {
             const int j = ch * CH + e;
             const cx<T> y = v[zp_perm<G>(j)];
-            cx<T> w = mk<T>(y.x, -y.y);
-            if (q > 0) {   // conj(y) conj(r) = conj(y r), r = W^{qk}
+            cx<T> w = y;
+            if (q > 0) {   // G_q = conj(y) conj(r) = conj(y r), r = W^{qk}: y r is stored, the conjugation is done by the combine
                 const T rx = wr[e], ry = sg * wi[e];
-                w = mk<T>(y.x * rx - y.y * ry, -(y.x * ry + y.y * rx));
+                w = mk<T>(y.x * rx - y.y * ry, y.x * ry + y.y * rx);
             }
             Sw[j * 32 + (lane ^ (j & 7))] = w;
         }
