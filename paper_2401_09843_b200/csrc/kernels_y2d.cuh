@@ -87,7 +87,7 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
         mbar_wait(bar_lg + (it & 1), (uint32_t)((it >> 1) & 1));
         const cx<T>* Ua = Ulg + (it & 1) * SLOT;
         cx<T> v[16];
-        zp_form_inverse<T, L>(v, Ua, Ua + L, q, t, tw3);
+        zp_form_inverse<T, L, false>(v, Ua, Ua + L, q, t, tw3);
         // the regions may be overwritten only when all three warps have finished the combine of the previous line
         zp_transform<T, L>(v, Sw, lane, t, lgcol, ttw, it > 0 ? cdone : nullptr, (uint32_t)((it - 1) & 1));
         // physical values u1 + i u2 at the points p = t + G j (register zp_perm(j)); flux, conjugated, in natural order
@@ -105,7 +105,7 @@ y2d_kernel(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, unsigned MM, u
             w[j] = mk<T>(u.x * u.x - u.y * u.y, -(u.x * u.y));
         }
         zp_transform<T, L>(w, Sw, lane, t, lgcol, ttw);
-        zp_post_forward<T, L>(w, Sw, lane, q, tw3);
+        zp_post_forward<T, L, false>(w, Sw, lane, q, tw3);
         named_bar_sync(bar_id, 96);
         // all three warps have consumed this line's slot: refill it with the line after next
         if (issuer && line + 2 * (unsigned long long)stride < total_lines) issue(line + 2 * stride, it + 2);

@@ -197,18 +197,27 @@ __device__ __forceinline__ void zp_park_twiddles(uint32_t ttw, uint32_t tw3, int
     tmem_wait_st();
 }
 
+// x with its sign flipped where `flip` is set: an integer XOR on the sign bit (ALU pipe) instead of a multiplication by +-1 (the
+// fp64 pipe is the busy one in these kernels)
+__device__ __forceinline__ double flip_sign(double x, bool flip) {
+    return __hiloint2double(__double2hiint(x) ^ (flip ? (int)0x80000000u : 0), __double2loint(x));
+}
+__device__ __forceinline__ float flip_sign(float x, bool flip) { return __int_as_float(__float_as_int(x) ^ (flip ? (int)0x80000000u : 0)); }
+
 // Input of an inverse job: v[j] = s_q[t + G j] for the two-for-one field ua + i ub with half spectra Ua, Ub (shared memory).
 // Radix-3 pruning of warp q: s_q[n] = (a_n + c_n (alpha + i beta)) W^{qn},  alpha + i beta = w3^{-q}, with the third
 // sub-transform taken as q = -1 (physical points 3r - 1 instead of 3r + 2: the physical order along the contiguous axis never
 // leaves the kernel), so that both q != 0 warps use the same twiddles W^{n}, one of them conjugated.
 // a_n = Ua[n] + i Ub[n], c_n = conj(Ua[L-n]) + i conj(Ub[L-n]) (kernels_z.cuh); n = 0: real parts only, c = 0.
-template <typename T, int L>
+// XORSIGN: the sign of the twiddle's imaginary part by flip_sign (measured faster in z_pair_kernel) or by a multiplication with
+// +-1 (measured faster in y2d_kernel, whose two transforms per line leave the fp64 pipe less loaded)
+template <typename T, int L, bool XORSIGN = true>
 __device__ __forceinline__ void zp_form_inverse(cx<T> (&v)[16], const cx<T>* __restrict__ Ua, const cx<T>* __restrict__ Ub, int q, int t,
                                                 uint32_t tw3) {
     constexpr int G = ZPGeo<T, L>::G, CH = tmem_cx_chunk<T>();
     const T alpha = q == 0 ? (T)1 : (T)-0.5;
     const T beta = q == 0 ? (T)0 : (q == 1 ? (T)-0.86602540378443864676L : (T)0.86602540378443864676L);
-    const T sg = q == 2 ? (T)-1 : (T)1;     // sign of the imaginary part of the twiddle: W^{+n} (q = 1), W^{-n} (q = -1)
+    const bool neg = q == 2;                // sign of the imaginary part of the twiddle: W^{+n} (q = 1), W^{-n} (q = -1)
 #pragma unroll
     for (int ch = 0; ch < 16 / CH; ++ch) {
         T wr[CH], wi[CH];
@@ -224,7 +233,7 @@ __device__ __forceinline__ void zp_form_inverse(cx<T> (&v)[16], const cx<T>* __r
             if (j == 0 && n == 0) { a = mk<T>(pa.x, pb.x); c = mk<T>(0, 0); }
             // z = a + c (alpha + i beta)
             cx<T> z = mk<T>(a.x + alpha * c.x - beta * c.y, a.y + alpha * c.y + beta * c.x);
-            if (q > 0) z = cmul(z, mk<T>(wr[e], sg * wi[e]));
+            if (q > 0) z = cmul(z, mk<T>(wr[e], XORSIGN ? flip_sign(wi[e], neg) : (neg ? (T)-1 : (T)1) * wi[e]));
             v[j] = z;
         }
     }
@@ -232,10 +241,10 @@ __device__ __forceinline__ void zp_form_inverse(cx<T> (&v)[16], const cx<T>* __r
 
 // Output of a forward job (run through the inverse butterflies on conjugated input): G_q[k] = conj(v) W^{-qk}; its CONJUGATE
 // v W^{qk} goes into the warp's region in natural order, k = t + G j at row j, column lane (zp_combine_store undoes it in its signs).
-template <typename T, int L>
+template <typename T, int L, bool XORSIGN = true>
 __device__ __forceinline__ void zp_post_forward(const cx<T> (&v)[16], cx<T>* __restrict__ Sw, int lane, int q, uint32_t tw3) {
     constexpr int G = ZPGeo<T, L>::G, CH = tmem_cx_chunk<T>();
-    const T sg = q == 2 ? (T)-1 : (T)1;
+    const bool neg = q == 2;
 #pragma unroll
     for (int ch = 0; ch < 16 / CH; ++ch) {
         T wr[CH], wi[CH];
@@ -246,7 +255,7 @@ __device__ __forceinline__ void zp_post_forward(const cx<T> (&v)[16], cx<T>* __r
             const cx<T> y = v[zp_perm<G>(j)];
             cx<T> w = y;
             if (q > 0) {   // G_q = conj(y) conj(r) = conj(y r), r = W^{qk}: y r is stored, the conjugation is done by the combine
-                const T rx = wr[e], ry = sg * wi[e];
+                const T rx = wr[e], ry = XORSIGN ? flip_sign(wi[e], neg) : (neg ? (T)-1 : (T)1) * wi[e];
                 w = mk<T>(y.x * rx - y.y * ry, y.x * ry + y.y * rx);
             }
             Sw[j * 32 + (lane ^ (j & 7))] = w;
